@@ -1,0 +1,16 @@
+"""B200-native exhaustive mutual-information maps (hot path of arxiv 1909.10690, "MICUDA").
+
+The product is the C-ABI shared library built from `csrc/` (declared in `include/mi.h`);
+`binding` is a thin ctypes layer with the same names.  There is no CPU fallback: using any API
+function without the built CUDA library raises.  `phantoms` is the seeded input generator
+(numpy only) and can be imported without the library.
+"""
+_API = ("mi_create", "mi_destroy", "mi_eval_batch", "mi_map", "mi_set_tsallis_form",
+        "mi_last_error", "MIContext", "MIError")
+
+
+def __getattr__(name):
+    if name in _API or name == "binding":
+        from . import binding
+        return binding if name == "binding" else getattr(binding, name)
+    raise AttributeError(name)
