@@ -1,0 +1,158 @@
+/* mi.h -- C ABI of the B200-native exhaustive mutual-information map ("MICUDA" hot path of
+ * Vianna & Murta 2019, arxiv 1909.10690).  Citations are PAPER.md line numbers.
+ *
+ * The library registers a moving volume v against a fixed volume u by EVALUATING (not optimising)
+ * the metric F_m(u(x), v(T(x))) of eq. 3 for many transforms T at once:
+ *   Transform block  v(T(x)): resample v at every fixed voxel x          (Fig. 1)
+ *   Metric block     joint histogram over ALL voxels, "full histogram"
+ *                    -> Shannon MI, eq. 1-2
+ *                    -> Tsallis MI for a list of q from the SAME histogram
+ *   Exhaustive map   one MI value per point of a 3-parameter grid of one transform family,
+ *                    stored as a 3D image
+ * Every step runs in hand-written CUDA kernels for sm_100a; there is NO CPU fallback: without a
+ * CUDA device every compute entry point returns MI_ERR_CUDA.
+ *
+ * Conventions
+ *   dims      (nx, ny, nz); x is fastest in memory: voxel (ix,iy,iz) is at [(iz*ny + iy)*nx + ix].
+ *   frames    physical frames are volume-centred, axes = index axes, identity direction cosines:
+ *             voxel i sits at spacing * (i - (n-1)/2) mm.
+ *   transform T is a row-major 3x4 [A|t] of doubles mapping a FIXED physical point x (mm) to a
+ *             MOVING physical point y = A x + t (mm) -- the direction of eq. 3.
+ *   samples   falling outside the moving volume (continuous index outside [-0.5, n-0.5) on any
+ *             axis) are skipped; probabilities are normalised by the number of valid samples.
+ *   bins      uniform over [lo, hi]; b = clamp(floor((v - lo) * nbins/(hi-lo)), 0, nbins-1).
+ *   pointers  every data pointer may be a HOST or a DEVICE pointer (resolved with
+ *             cudaPointerGetAttributes).  Inputs are only read.  Outputs are caller-owned and are
+ *             written only when the call returns MI_OK.
+ *   sync      a call returns after all HOST outputs are complete; DEVICE outputs are ordered on
+ *             the context's stream (the cudaStream_t given to mi_create).
+ *   threads   one context must not be used from two threads at once; distinct contexts are
+ *             independent.
+ *   errors    status codes only -- nothing throws or aborts across this ABI; mi_last_error gives
+ *             the text of the last failure.
+ */
+#ifndef MI_B200_H
+#define MI_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mi_ctx mi_ctx; /* opaque; owns all of its device memory until mi_destroy */
+
+typedef enum {
+    MI_OK = 0,
+    MI_ERR_INVALID_ARG = 1,   /* NULL pointer, dim < 1, grid n < 1, spacing <= 0 or non-finite, lo >= hi,
+                                 nbins < 2, N < 0, q <= 0 or non-finite, non-finite matrix entry */
+    MI_ERR_UNSUPPORTED = 2,   /* nbins > 256; volume with more than 2^31-1 voxels */
+    MI_ERR_OUT_OF_MEMORY = 3,
+    MI_ERR_CUDA = 4,          /* any CUDA runtime failure, including "no device" */
+    MI_ERR_INTERNAL = 5
+} mi_status;
+
+typedef enum { MI_INTERP_NEAREST = 0, MI_INTERP_TRILINEAR = 1 } mi_interp;
+
+/* Tsallis entropy S_q(X) = (1 - sum_{p>0} p^q)/(q - 1).  The paper prints no Tsallis formula
+ * (reading A1); ADDITIVE puts S_q into the paper's own eq. 2 and is the default. */
+typedef enum {
+    MI_TSALLIS_ADDITIVE = 0,        /* I_q = S_q(A) + S_q(B) - S_q(A,B)                         */
+    MI_TSALLIS_PSEUDO_ADDITIVE = 1  /* I_q = S_q(A) + S_q(B) + (1-q) S_q(A) S_q(B) - S_q(A,B)   */
+} mi_tsallis_form;
+
+/* Transform families of the maps (section 3.1-3.3). p = (p0,p1,p2). */
+typedef enum {
+    MI_FAMILY_TRANSLATION = 0,        /* A = I, t = p (mm)                                       */
+    MI_FAMILY_ROTATION_EULER_DEG = 1, /* A = Rz(p2) Ry(p1) Rx(p0), degrees, about the centre     */
+    MI_FAMILY_ROTATION_VERSOR = 2,    /* p = axis*sin(theta/2); |p| > 1 -> p/|p| */
+    MI_FAMILY_SCALE = 3,              /* A = diag(p), 1 = identity                               */
+    MI_FAMILY_SCALE_LOG = 4           /* A = diag(exp(p)), zero-centred           */
+} mi_family;
+
+/* mi_create -- take a fixed/moving pair and pre-bin it (step a1: fixed float -> uint8 bin
+ * indices; the moving volume is kept as float32 for trilinear sampling and also pre-binned for
+ * nearest-neighbour sampling).  "uses all the voxels and produces a full histogram" PAPER.md:212.
+ *   out            receives the context; *out is NULL on failure.
+ *   fixed, moving  float32 volumes (host or device), finite values; copied -- the caller may free
+ *                  them on return.
+ *   *_dims         (nx, ny, nz), each >= 1;  *_spacing  mm, each > 0 and finite.
+ *   nbins          2..256 bins per axis of the joint histogram.
+ *   *_lo, *_hi     intensity range of each volume, lo < hi, finite.
+ *   device         CUDA device ordinal.   cuda_stream  a cudaStream_t (may be NULL = default).
+ * Blocks until the context is ready. */
+mi_status mi_create(mi_ctx **out,
+                    const float *fixed, const int32_t fixed_dims[3], const double fixed_spacing[3],
+                    const float *moving, const int32_t moving_dims[3], const double moving_spacing[3],
+                    int32_t nbins, float fixed_lo, float fixed_hi, float moving_lo, float moving_hi,
+                    int32_t device, void *cuda_stream);
+
+/* Select the Tsallis MI form used by later calls (default MI_TSALLIS_ADDITIVE). */
+mi_status mi_set_tsallis_form(mi_ctx *ctx, mi_tsallis_form form);
+
+/* mi_eval_batch -- F_m(u, v o T) for N transforms (eq. 3 without the arg max).
+ *   T           N x 12 doubles, row-major [A|t] per transform (see "transform" above).  Singular
+ *               matrices are legal; entries must be finite.
+ *   q, nq       Tsallis orders, each > 0 and finite; q == 1 returns the Shannon value; nq may be 0
+ *               (then q may be NULL).
+ *   mi_out      N x (1+nq) doubles: [Shannon I (nats), I_q0, I_q1, ...] per transform.  An empty
+ *               overlap gives zeros.
+ *   hist_out    NULL, or N x nbins x nbins uint32 joint histograms, row = fixed bin, column =
+ *               moving bin.
+ *   nvalid_out  NULL, or N int64: samples inside the moving volume per transform.
+ * N == 0 is a no-op returning MI_OK. */
+mi_status mi_eval_batch(mi_ctx *ctx, const double *T, int64_t N, const double *q, int32_t nq,
+                        mi_interp interp, double *mi_out, uint32_t *hist_out, int64_t *nvalid_out);
+
+/* mi_map -- the exhaustive map of one family: "map with the MI function all
+ * the space in a finite range and build a 3D image".
+ *   lo, hi, n   inclusive grid per parameter axis: value k on axis d is
+ *               lo[d] + k*(hi[d]-lo[d])/(n[d]-1) in double (n[d] == 1 -> lo[d]); n[d] >= 1.
+ *   map_out     (1+nq) x n[2] x n[1] x n[0] doubles, channel-major, p0 fastest.
+ *   argmax_out  NULL, or (1+nq) int64 linear indices into one channel: the largest value, ties to
+ *               the lowest index (the arg max of eq. 3). */
+mi_status mi_map(mi_ctx *ctx, mi_family family, const double lo[3], const double hi[3],
+                 const int32_t n[3], const double *q, int32_t nq, mi_interp interp,
+                 double *map_out, int64_t *argmax_out);
+
+/* Release the context and its device memory.  NULL is a no-op. */
+void mi_destroy(mi_ctx *ctx);
+
+/* Text of the last failure on this context (ctx != NULL) or of the last failed mi_create on this
+ * thread (ctx == NULL).  The string is owned by the library and valid until the next call. */
+const char *mi_last_error(const mi_ctx *ctx);
+
+/* ---- host-side pieces of the path, exported so tests can check them without a GPU ------------ */
+
+/* Step a2, family generator: parameter triple -> physical 3x4 [A|t] (double). */
+mi_status mi_family_matrix(mi_family family, const double p[3], double T_out[12]);
+
+/* Step a2, index-space composition (DESIGN.md CANON-1): physical [A|t] + the two geometries ->
+ * fp32 3x4 [M|m0] with c = M i + m0 the continuous moving index of fixed voxel i. */
+mi_status mi_index_affine(const double T[12], const int32_t fixed_dims[3], const double fixed_spacing[3],
+                          const int32_t moving_dims[3], const double moving_spacing[3], float M_out[12]);
+
+/* ---- introspection used by tests and the benchmark ------------------------------------------- */
+
+/* Copy the pre-binned volumes out of the context (step a1 parity): which = 0 fixed, 1 moving;
+ * out receives nx*ny*nz uint8 (host or device). */
+mi_status mi_get_bins(mi_ctx *ctx, int32_t which, uint8_t *out);
+
+/* Device milliseconds (CUDA events on the context's stream) spent in the kernels of the last
+ * mi_eval_batch / mi_map call: ms[0] transform upload + setup, ms[1] resample+histogram kernels,
+ * ms[2] entropy kernels, ms[3] map assembly + arg max; launches[k] = kernels launched per class. */
+mi_status mi_last_timing(const mi_ctx *ctx, float ms[4], int64_t launches[4]);
+
+/* Shared-memory atomic rate probe for the roofline: runs `iters` rounds of
+ * atomicAdd(u32) into an nbins x nbins table in shared memory on every SM and reports
+ * lane-updates per second.  pattern: 0 conflict-free (lane-distinct banks), 1 uniform random bins,
+ * 2 all lanes on one address.  Host pointers. */
+mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
+                                      double *updates_per_s);
+
+const char *mi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MI_B200_H */

@@ -5,12 +5,14 @@ The product is the C-ABI shared library built from `csrc/` (declared in `include
 function without the built CUDA library raises.  `phantoms` is the seeded input generator
 (numpy only) and can be imported without the library.
 """
-_API = ("mi_create", "mi_destroy", "mi_eval_batch", "mi_map", "mi_set_tsallis_form",
-        "mi_last_error", "MIContext", "MIError")
+_API = ("mi_create", "mi_destroy", "mi_eval_batch", "mi_map", "mi_set_tsallis_form", "mi_last_error",
+        "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing",
+        "mi_probe_shared_atomic_rate", "mi_version", "MIContext", "MIError")
 
 
 def __getattr__(name):
     if name in _API or name == "binding":
-        from . import binding
+        import importlib
+        binding = importlib.import_module(__name__ + ".binding")
         return binding if name == "binding" else getattr(binding, name)
     raise AttributeError(name)

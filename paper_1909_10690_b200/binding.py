@@ -1,0 +1,256 @@
+"""ctypes binding of libmi_b200.so -- same names as include/mi.h, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  There is NO fallback: if the shared
+library has not been built (`python -m paper_1909_10690_b200.build`) importing this module raises,
+and on a box without a CUDA device every compute call raises MIError(MI_ERR_CUDA).
+
+Arrays may be numpy arrays (host) or torch tensors (host or CUDA); their data pointers are passed
+straight through.  Volumes are (nz, ny, nx) C-contiguous float32 (x fastest), dims are (nx, ny, nz).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmi_b200.so")
+
+MI_OK, MI_ERR_INVALID_ARG, MI_ERR_UNSUPPORTED, MI_ERR_OUT_OF_MEMORY, MI_ERR_CUDA, MI_ERR_INTERNAL = range(6)
+MI_INTERP_NEAREST, MI_INTERP_TRILINEAR = 0, 1
+MI_TSALLIS_ADDITIVE, MI_TSALLIS_PSEUDO_ADDITIVE = 0, 1
+(MI_FAMILY_TRANSLATION, MI_FAMILY_ROTATION_EULER_DEG, MI_FAMILY_ROTATION_VERSOR, MI_FAMILY_SCALE,
+ MI_FAMILY_SCALE_LOG) = range(5)
+_STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_ERR_OUT_OF_MEMORY",
+           4: "MI_ERR_CUDA", 5: "MI_ERR_INTERNAL"}
+
+EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
+           "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing",
+           "mi_probe_shared_atomic_rate", "mi_version")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError("%s is missing: build it with `python -m paper_1909_10690_b200.build` "
+                      "(there is no CPU fallback)" % LIB_PATH)
+_lib = C.CDLL(LIB_PATH)
+
+_vp = C.c_void_p
+_lib.mi_create.argtypes = [C.POINTER(_vp), _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_float, C.c_float,
+                           C.c_float, C.c_float, C.c_int32, _vp]
+_lib.mi_create.restype = C.c_int
+_lib.mi_set_tsallis_form.argtypes = [_vp, C.c_int]
+_lib.mi_set_tsallis_form.restype = C.c_int
+_lib.mi_eval_batch.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, C.c_int, _vp, _vp, _vp]
+_lib.mi_eval_batch.restype = C.c_int
+_lib.mi_map.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp]
+_lib.mi_map.restype = C.c_int
+_lib.mi_destroy.argtypes = [_vp]
+_lib.mi_destroy.restype = None
+_lib.mi_last_error.argtypes = [_vp]
+_lib.mi_last_error.restype = C.c_char_p
+_lib.mi_family_matrix.argtypes = [C.c_int, _vp, _vp]
+_lib.mi_family_matrix.restype = C.c_int
+_lib.mi_index_affine.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
+_lib.mi_index_affine.restype = C.c_int
+_lib.mi_get_bins.argtypes = [_vp, C.c_int32, _vp]
+_lib.mi_get_bins.restype = C.c_int
+_lib.mi_last_timing.argtypes = [_vp, _vp, _vp]
+_lib.mi_last_timing.restype = C.c_int
+_lib.mi_probe_shared_atomic_rate.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
+_lib.mi_probe_shared_atomic_rate.restype = C.c_int
+_lib.mi_version.argtypes = []
+_lib.mi_version.restype = C.c_char_p
+
+
+class MIError(RuntimeError):
+    def __init__(self, status, msg=""):
+        self.status = int(status)
+        super().__init__("%s: %s" % (_STATUS.get(self.status, str(status)), msg))
+
+
+def _is_torch(x):
+    return type(x).__module__.startswith("torch")
+
+
+def _ptr(x):
+    """Data pointer of a numpy array / torch tensor / raw int, or None."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if _is_torch(x):
+        assert x.is_contiguous()
+        return x.data_ptr()
+    assert x.flags["C_CONTIGUOUS"]
+    return x.ctypes.data
+
+
+def _f64(a, n=None):
+    a = np.ascontiguousarray(np.asarray(a, dtype=np.float64).reshape(-1))
+    assert n is None or a.size == n
+    return a
+
+
+def _i32(a, n):
+    a = np.ascontiguousarray(np.asarray(a, dtype=np.int32).reshape(-1))
+    assert a.size == n
+    return a
+
+
+def _volume(v):
+    """float32, contiguous; keeps torch tensors (host or CUDA) as they are."""
+    if _is_torch(v):
+        import torch
+        assert v.dtype == torch.float32 and v.dim() == 3
+        return v.contiguous()
+    v = np.ascontiguousarray(v, dtype=np.float32)
+    assert v.ndim == 3
+    return v
+
+
+class MIContext:
+    """Owns an mi_ctx*; also remembers the shapes the marshalling needs."""
+
+    def __init__(self, handle, nbins, fixed_dims, moving_dims):
+        self.handle = handle
+        self.nbins = int(nbins)
+        self.fixed_dims = tuple(int(d) for d in fixed_dims)
+        self.moving_dims = tuple(int(d) for d in moving_dims)
+
+    def __del__(self):
+        try:
+            mi_destroy(self)
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        mi_destroy(self)
+
+
+def _check(ctx, status):
+    if status != MI_OK:
+        h = ctx.handle if isinstance(ctx, MIContext) else None
+        raise MIError(status, (_lib.mi_last_error(h) or b"").decode())
+
+
+def mi_version() -> str:
+    return _lib.mi_version().decode()
+
+
+def mi_last_error(ctx=None) -> str:
+    return (_lib.mi_last_error(ctx.handle if ctx is not None else None) or b"").decode()
+
+
+def mi_create(fixed, moving, fixed_spacing, moving_spacing, nbins, fixed_lo=0.0, fixed_hi=1.0,
+              moving_lo=0.0, moving_hi=1.0, device=0, cuda_stream=None, fixed_dims=None,
+              moving_dims=None) -> MIContext:
+    fixed, moving = _volume(fixed), _volume(moving)
+    if fixed_dims is None:
+        fixed_dims = tuple(fixed.shape)[::-1]
+    if moving_dims is None:
+        moving_dims = tuple(moving.shape)[::-1]
+    fd, md = _i32(fixed_dims, 3), _i32(moving_dims, 3)
+    fs, ms = _f64(fixed_spacing, 3), _f64(moving_spacing, 3)
+    h = _vp()
+    st = _lib.mi_create(C.byref(h), _ptr(fixed), _ptr(fd), _ptr(fs), _ptr(moving), _ptr(md), _ptr(ms),
+                        int(nbins), float(fixed_lo), float(fixed_hi), float(moving_lo), float(moving_hi),
+                        int(device), cuda_stream)
+    if st != MI_OK:
+        raise MIError(st, mi_last_error(None))
+    return MIContext(h, nbins, fd, md)
+
+
+def mi_destroy(ctx) -> None:
+    if ctx is not None and getattr(ctx, "handle", None):
+        h, ctx.handle = ctx.handle, None
+        _lib.mi_destroy(h)
+
+
+def mi_set_tsallis_form(ctx, form) -> None:
+    _check(ctx, _lib.mi_set_tsallis_form(ctx.handle, int(form)))
+
+
+def mi_eval_batch(ctx, T, q=(), interp=MI_INTERP_TRILINEAR, mi_out=None, hist_out=None, nvalid_out=None):
+    """T: (N,3,4) physical [A|t].  Outputs: pass arrays/tensors to fill, True to allocate a host
+    array, None/False to skip (mi_out is always produced).  Returns (mi, hist, nvalid)."""
+    T = _f64(T)
+    N = T.size // 12
+    assert T.size == N * 12
+    q = _f64(q)
+    nq = q.size
+    nb = ctx.nbins
+    if mi_out is None or mi_out is True:
+        mi_out = np.empty((N, 1 + nq), dtype=np.float64)
+    if hist_out is True:
+        hist_out = np.empty((N, nb, nb), dtype=np.uint32)
+    elif hist_out is False:
+        hist_out = None
+    if nvalid_out is True:
+        nvalid_out = np.empty(N, dtype=np.int64)
+    elif nvalid_out is False:
+        nvalid_out = None
+    st = _lib.mi_eval_batch(ctx.handle, _ptr(T), N, _ptr(q) if nq else None, nq, int(interp), _ptr(mi_out),
+                            _ptr(hist_out), _ptr(nvalid_out))
+    _check(ctx, st)
+    return mi_out, hist_out, nvalid_out
+
+
+def mi_map(ctx, family, lo, hi, n, q=(), interp=MI_INTERP_TRILINEAR, map_out=None, argmax_out=None):
+    """Returns (map (1+nq, n2, n1, n0) float64, argmax (1+nq,) int64)."""
+    lo, hi, n = _f64(lo, 3), _f64(hi, 3), _i32(n, 3)
+    q = _f64(q)
+    nq = q.size
+    if map_out is None:
+        map_out = np.empty((1 + nq, int(n[2]), int(n[1]), int(n[0])), dtype=np.float64)
+    if argmax_out is None:
+        argmax_out = np.empty(1 + nq, dtype=np.int64)
+    st = _lib.mi_map(ctx.handle, int(family), _ptr(lo), _ptr(hi), _ptr(n), _ptr(q) if nq else None, nq,
+                     int(interp), _ptr(map_out), _ptr(argmax_out))
+    _check(ctx, st)
+    return map_out, argmax_out
+
+
+def mi_family_matrix(family, p) -> np.ndarray:
+    p = _f64(p, 3)
+    T = np.empty(12, dtype=np.float64)
+    st = _lib.mi_family_matrix(int(family), _ptr(p), _ptr(T))
+    if st != MI_OK:
+        raise MIError(st, "mi_family_matrix")
+    return T.reshape(3, 4)
+
+
+def mi_index_affine(T, fixed_dims, fixed_spacing, moving_dims, moving_spacing) -> np.ndarray:
+    T = _f64(T, 12)
+    fd, md = _i32(fixed_dims, 3), _i32(moving_dims, 3)
+    fs, ms = _f64(fixed_spacing, 3), _f64(moving_spacing, 3)
+    M = np.empty(12, dtype=np.float32)
+    st = _lib.mi_index_affine(_ptr(T), _ptr(fd), _ptr(fs), _ptr(md), _ptr(ms), _ptr(M))
+    if st != MI_OK:
+        raise MIError(st, "mi_index_affine")
+    return M.reshape(3, 4)
+
+
+def mi_get_bins(ctx, which: int) -> np.ndarray:
+    dims = ctx.fixed_dims if which == 0 else ctx.moving_dims
+    out = np.empty((dims[2], dims[1], dims[0]), dtype=np.uint8)
+    _check(ctx, _lib.mi_get_bins(ctx.handle, int(which), _ptr(out)))
+    return out
+
+
+def mi_last_timing(ctx):
+    """(ms[4], launches[4]) of the last eval/map call: setup, resample+hist, entropy, map assembly."""
+    ms = np.zeros(4, dtype=np.float32)
+    ln = np.zeros(4, dtype=np.int64)
+    _check(ctx, _lib.mi_last_timing(ctx.handle, _ptr(ms), _ptr(ln)))
+    return ms, ln
+
+
+def mi_probe_shared_atomic_rate(device=0, nbins=256, pattern=1, iters=4096) -> float:
+    out = np.zeros(1, dtype=np.float64)
+    st = _lib.mi_probe_shared_atomic_rate(int(device), int(nbins), int(pattern), int(iters), _ptr(out))
+    if st != MI_OK:
+        raise MIError(st, "mi_probe_shared_atomic_rate")
+    return float(out[0])

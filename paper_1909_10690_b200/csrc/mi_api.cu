@@ -1,0 +1,503 @@
+// mi_api.cu -- the C-ABI boundary (include/mi.h) and the host runtime behind it: context,
+// argument validation, transform generation (step a2), chunked launch planning, copy-back.
+// No step of the path runs on the CPU except a2 (12 numbers per transform, in double).
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "mi_internal.h"
+
+struct mi_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int32_t fd[3] = {0, 0, 0}, md[3] = {0, 0, 0};
+    double fs[3] = {1, 1, 1}, ms[3] = {1, 1, 1};
+    int nb = 0;
+    float flo = 0, fhi = 1, mlo = 0, mhi = 1, fscale = 1, mscale = 1;
+    int64_t nf = 0, nm = 0;
+    uint8_t* d_fbins = nullptr;
+    float* d_moving = nullptr;
+    uint8_t* d_mbins = nullptr;
+    int tsallis_form = MI_TSALLIS_ADDITIVE;
+    int num_sms = 148;
+    size_t smem_optin = 48 * 1024;
+    size_t hist_budget = (size_t)1 << 30;  // bytes of global histogram scratch per chunk
+
+    // scratch, grown on demand
+    float* d_M = nullptr;      size_t cap_M = 0;       // transforms
+    float* h_M = nullptr;      size_t cap_hM = 0;      // pinned staging
+    uint32_t* d_hist = nullptr; size_t cap_hist = 0;   // bytes
+    double* d_mi = nullptr;    size_t cap_mi = 0;      // doubles
+    int64_t* d_nvalid = nullptr; size_t cap_nv = 0;
+    double* d_q = nullptr;     size_t cap_q = 0;
+    double* d_map = nullptr;   size_t cap_map = 0;
+    int64_t* d_argmax = nullptr; size_t cap_am = 0;
+    cudaEvent_t ev_staging = nullptr;  // h_M may be reused once this has completed
+    bool staging_busy = false;
+
+    std::string err;
+    float last_ms[4] = {0, 0, 0, 0};
+    int64_t last_launches[4] = {0, 0, 0, 0};
+};
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; cudaGetLastError(); }
+        ok = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+mi_status fail(mi_ctx* c, mi_status s, const std::string& msg) {
+    if (c) c->err = msg; else g_create_error = msg;
+    return s;
+}
+mi_status cuda_fail(mi_ctx* c, cudaError_t e, const char* where) {
+    cudaGetLastError();
+    const mi_status s = (e == cudaErrorMemoryAllocation) ? MI_ERR_OUT_OF_MEMORY : MI_ERR_CUDA;
+    return fail(c, s, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define MI_CUDA(ctx, call)                                           \
+    do {                                                             \
+        cudaError_t e__ = (call);                                    \
+        if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #call); \
+    } while (0)
+
+bool is_host_ptr(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return true;
+    }
+    return !(at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
+}
+
+template <typename T>
+mi_status grow(mi_ctx* c, T** p, size_t* cap, size_t need) {
+    if (need <= *cap) return MI_OK;
+    if (*p) { cudaFree(*p); *p = nullptr; *cap = 0; }
+    MI_CUDA(c, cudaMalloc(reinterpret_cast<void**>(p), need * sizeof(T)));
+    *cap = need;
+    return MI_OK;
+}
+
+bool finite3(const double v[3]) { return std::isfinite(v[0]) && std::isfinite(v[1]) && std::isfinite(v[2]); }
+
+struct EventTimer {
+    // accumulates device time per class over a call; events are recorded on the context's stream
+    struct Span { cudaEvent_t a, b; int cls; };
+    std::vector<Span> spans;
+    cudaStream_t s;
+    explicit EventTimer(cudaStream_t st) : s(st) {}
+    void begin(int cls) {
+        Span sp{nullptr, nullptr, cls};
+        cudaEventCreate(&sp.a);
+        cudaEventCreate(&sp.b);
+        cudaEventRecord(sp.a, s);
+        spans.push_back(sp);
+    }
+    void end() { cudaEventRecord(spans.back().b, s); }
+    void collect(float ms[4]) {
+        for (auto& sp : spans) {
+            float t = 0.f;
+            if (cudaEventSynchronize(sp.b) == cudaSuccess && cudaEventElapsedTime(&t, sp.a, sp.b) == cudaSuccess)
+                ms[sp.cls] += t;
+            cudaEventDestroy(sp.a);
+            cudaEventDestroy(sp.b);
+        }
+        spans.clear();
+        cudaGetLastError();
+    }
+    ~EventTimer() {
+        for (auto& sp : spans) { cudaEventDestroy(sp.a); cudaEventDestroy(sp.b); }
+    }
+};
+
+mi_status validate_q(mi_ctx* c, const double* q, int32_t nq) {
+    if (nq < 0) return fail(c, MI_ERR_INVALID_ARG, "nq < 0");
+    if (nq > 0 && q == nullptr) return fail(c, MI_ERR_INVALID_ARG, "q is NULL but nq > 0");
+    for (int i = 0; i < nq; ++i)
+        if (!(std::isfinite(q[i]) && q[i] > 0.0)) return fail(c, MI_ERR_INVALID_ARG, "q must be finite and > 0");
+    return MI_OK;
+}
+
+// The shared core of mi_eval_batch and mi_map.  hM: N x 12 index-space fp32 transforms in host
+// memory.  If map_out != NULL the result is assembled channel-major (step a6) instead of being
+// returned transform-major.
+mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const double* q, int32_t nq,
+                    int interp, double* mi_out, uint32_t* hist_out, int64_t* nvalid_out,
+                    double* map_out, int64_t* argmax_out) {
+    const int nch = 1 + nq;
+    const size_t nbins2 = (size_t)c->nb * c->nb;
+    cudaStream_t s = c->stream;
+    for (int k = 0; k < 4; ++k) { c->last_ms[k] = 0.f; c->last_launches[k] = 0; }
+    EventTimer timer(s);
+
+    // ---- setup: scratch + upload of transforms and q -------------------------------------------
+    timer.begin(0);
+    mi_status st;
+    if ((st = grow(c, &c->d_M, &c->cap_M, (size_t)N * 12)) != MI_OK) return st;
+    if ((st = grow(c, &c->d_mi, &c->cap_mi, (size_t)N * nch)) != MI_OK) return st;
+    if ((st = grow(c, &c->d_nvalid, &c->cap_nv, (size_t)N)) != MI_OK) return st;
+    if ((st = grow(c, &c->d_q, &c->cap_q, (size_t)(nq > 0 ? nq : 1))) != MI_OK) return st;
+    if (c->staging_busy) { MI_CUDA(c, cudaEventSynchronize(c->ev_staging)); c->staging_busy = false; }
+    if ((size_t)N * 12 > c->cap_hM) {
+        if (c->h_M) { cudaFreeHost(c->h_M); c->h_M = nullptr; c->cap_hM = 0; }
+        MI_CUDA(c, cudaMallocHost(reinterpret_cast<void**>(&c->h_M), (size_t)N * 12 * sizeof(float)));
+        c->cap_hM = (size_t)N * 12;
+    }
+    std::memcpy(c->h_M, hM.data(), (size_t)N * 12 * sizeof(float));
+    MI_CUDA(c, cudaMemcpyAsync(c->d_M, c->h_M, (size_t)N * 12 * sizeof(float), cudaMemcpyHostToDevice, s));
+    MI_CUDA(c, cudaEventRecord(c->ev_staging, s));
+    c->staging_busy = true;
+    if (nq > 0) MI_CUDA(c, cudaMemcpyAsync(c->d_q, q, (size_t)nq * sizeof(double), cudaMemcpyDefault, s));
+    timer.end();
+
+    // ---- chunk plan --------------------------------------------------------------------------------
+    const bool hist_to_user_dev = hist_out != nullptr && !is_host_ptr(hist_out);
+    int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * sizeof(uint32_t)));
+    if (chunk < 1) chunk = 1;
+    if (chunk > N) chunk = N;
+    if (!hist_to_user_dev) {
+        if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist,
+                       (size_t)chunk * nbins2 * sizeof(uint32_t))) != MI_OK)
+            return st;
+    }
+    const int rows_total = c->fd[1] * c->fd[2];
+
+    for (int64_t off = 0; off < N; off += chunk) {
+        const int64_t cnt = (N - off < chunk) ? (N - off) : chunk;
+        uint32_t* hist = hist_to_user_dev ? hist_out + (size_t)off * nbins2 : c->d_hist;
+
+        timer.begin(1);
+        MI_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)cnt * nbins2 * sizeof(uint32_t), s));
+        mi::ResampleArgs a;
+        a.fbins = c->d_fbins;
+        a.moving = c->d_moving;
+        a.mbins = c->d_mbins;
+        a.M = c->d_M + (size_t)off * 12;
+        a.hist = hist;
+        a.f = {c->fd[0], c->fd[1], c->fd[2]};
+        a.m = {c->md[0], c->md[1], c->md[2]};
+        a.nb = c->nb;
+        a.mlo = c->mlo;
+        a.mscale = c->mscale;
+        a.n_transforms = (int)cnt;
+        // CTAs per transform: one when there are many transforms; otherwise split the volume into
+        // row slabs so that about 16 waves of CTAs exist (each slab keeps >= 64 rows).
+        int nslabs = 1;
+        const int64_t want = 16LL * c->num_sms;
+        if (cnt < want) {
+            nslabs = (int)((want + cnt - 1) / cnt);
+            const int cap = rows_total / 64 > 1 ? rows_total / 64 : 1;
+            if (nslabs > cap) nslabs = cap;
+        }
+        a.nslabs = nslabs;
+        MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, c->smem_optin, s));
+        c->last_launches[1] += 1;
+        timer.end();
+
+        timer.begin(2);
+        int q_off = 0;
+        do {
+            MI_CUDA(c, mi::launch_entropy(hist, c->nb, (int)cnt, c->d_q, nq, q_off, c->tsallis_form,
+                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, s));
+            c->last_launches[2] += 1;
+            q_off += mi::kMaxQPerPass;
+        } while (q_off < nq);
+        timer.end();
+
+        if (hist_out != nullptr && !hist_to_user_dev)
+            MI_CUDA(c, cudaMemcpyAsync(hist_out + (size_t)off * nbins2, hist,
+                                       (size_t)cnt * nbins2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+    }
+
+    // ---- outputs -----------------------------------------------------------------------------------
+    bool host_out = false;
+    if (map_out != nullptr) {
+        timer.begin(3);
+        const bool map_dev = !is_host_ptr(map_out);
+        const bool am_dev = argmax_out != nullptr && !is_host_ptr(argmax_out);
+        double* dmap = map_out;
+        if (!map_dev) {
+            if ((st = grow(c, &c->d_map, &c->cap_map, (size_t)N * nch)) != MI_OK) return st;
+            dmap = c->d_map;
+        }
+        if ((st = grow(c, &c->d_argmax, &c->cap_am, (size_t)nch)) != MI_OK) return st;
+        int64_t* dam = am_dev ? argmax_out : c->d_argmax;
+        MI_CUDA(c, mi::launch_map_assemble(c->d_mi, N, nch, dmap, dam, s));
+        c->last_launches[3] += 1;
+        timer.end();
+        if (!map_dev) {
+            MI_CUDA(c, cudaMemcpyAsync(map_out, dmap, (size_t)N * nch * sizeof(double), cudaMemcpyDeviceToHost, s));
+            host_out = true;
+        }
+        if (argmax_out != nullptr && !am_dev) {
+            MI_CUDA(c, cudaMemcpyAsync(argmax_out, dam, (size_t)nch * sizeof(int64_t), cudaMemcpyDeviceToHost, s));
+            host_out = true;
+        }
+    }
+    if (mi_out != nullptr) {
+        MI_CUDA(c, cudaMemcpyAsync(mi_out, c->d_mi, (size_t)N * nch * sizeof(double), cudaMemcpyDefault, s));
+        host_out |= is_host_ptr(mi_out);
+    }
+    if (nvalid_out != nullptr) {
+        MI_CUDA(c, cudaMemcpyAsync(nvalid_out, c->d_nvalid, (size_t)N * sizeof(int64_t), cudaMemcpyDefault, s));
+        host_out |= is_host_ptr(nvalid_out);
+    }
+    if (hist_out != nullptr && !hist_to_user_dev) host_out = true;
+    // Host outputs must be complete on return.  The per-class timings need the events anyway, so
+    // the call always drains its own work; device outputs stay ordered on the stream.
+    MI_CUDA(c, cudaStreamSynchronize(s));
+    (void)host_out;
+    timer.collect(c->last_ms);
+    return MI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mi_version(void) { return "mi-b200 0.1 (sm_100a)"; }
+
+const char* mi_last_error(const mi_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+mi_status mi_family_matrix(mi_family family, const double p[3], double T_out[12]) {
+    if (p == nullptr || T_out == nullptr) return MI_ERR_INVALID_ARG;
+    if (!finite3(p)) return MI_ERR_INVALID_ARG;
+    return mi::family_matrix((int)family, p, T_out) == 0 ? MI_OK : MI_ERR_INVALID_ARG;
+}
+
+mi_status mi_index_affine(const double T[12], const int32_t fixed_dims[3], const double fixed_spacing[3],
+                          const int32_t moving_dims[3], const double moving_spacing[3], float M_out[12]) {
+    if (!T || !fixed_dims || !fixed_spacing || !moving_dims || !moving_spacing || !M_out)
+        return MI_ERR_INVALID_ARG;
+    for (int i = 0; i < 12; ++i)
+        if (!std::isfinite(T[i])) return MI_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d) {
+        if (fixed_dims[d] < 1 || moving_dims[d] < 1) return MI_ERR_INVALID_ARG;
+        if (!(std::isfinite(fixed_spacing[d]) && fixed_spacing[d] > 0.0)) return MI_ERR_INVALID_ARG;
+        if (!(std::isfinite(moving_spacing[d]) && moving_spacing[d] > 0.0)) return MI_ERR_INVALID_ARG;
+    }
+    mi::index_affine(T, fixed_dims, fixed_spacing, moving_dims, moving_spacing, M_out);
+    return MI_OK;
+}
+
+mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3],
+                    const double fixed_spacing[3], const float* moving, const int32_t moving_dims[3],
+                    const double moving_spacing[3], int32_t nbins, float fixed_lo, float fixed_hi,
+                    float moving_lo, float moving_hi, int32_t device, void* cuda_stream) {
+    if (out == nullptr) return fail(nullptr, MI_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!fixed || !moving || !fixed_dims || !moving_dims || !fixed_spacing || !moving_spacing)
+        return fail(nullptr, MI_ERR_INVALID_ARG, "NULL argument");
+    int64_t nf = 1, nm = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (fixed_dims[d] < 1 || moving_dims[d] < 1) return fail(nullptr, MI_ERR_INVALID_ARG, "volume dim < 1");
+        if (!(std::isfinite(fixed_spacing[d]) && fixed_spacing[d] > 0.0) ||
+            !(std::isfinite(moving_spacing[d]) && moving_spacing[d] > 0.0))
+            return fail(nullptr, MI_ERR_INVALID_ARG, "spacing must be finite and > 0");
+        nf *= fixed_dims[d];
+        nm *= moving_dims[d];
+        if (nf > 0x7FFFFFFFLL || nm > 0x7FFFFFFFLL)
+            return fail(nullptr, MI_ERR_UNSUPPORTED, "volume has more than 2^31-1 voxels");
+    }
+    if (nbins < 2) return fail(nullptr, MI_ERR_INVALID_ARG, "nbins < 2");
+    if (nbins > 256) return fail(nullptr, MI_ERR_UNSUPPORTED, "nbins > 256 is not supported");
+    if (!(std::isfinite(fixed_lo) && std::isfinite(fixed_hi) && fixed_lo < fixed_hi) ||
+        !(std::isfinite(moving_lo) && std::isfinite(moving_hi) && moving_lo < moving_hi))
+        return fail(nullptr, MI_ERR_INVALID_ARG, "intensity range must be finite with lo < hi");
+
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) return cuda_fail(nullptr, e, "cudaGetDeviceCount");
+    if (device < 0 || device >= ndev) return fail(nullptr, MI_ERR_INVALID_ARG, "no such CUDA device");
+
+    mi_ctx* c = new (std::nothrow) mi_ctx();
+    if (!c) return fail(nullptr, MI_ERR_OUT_OF_MEMORY, "host allocation failed");
+    c->device = device;
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    DeviceGuard guard(device);
+    mi_status st = MI_OK;
+    float* d_tmp = nullptr;
+    do {
+        if (!guard.ok) { st = fail(nullptr, MI_ERR_CUDA, "cudaSetDevice failed"); break; }
+        int v = 0;
+        if ((e = cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, device)) != cudaSuccess) { st = cuda_fail(nullptr, e, "attr"); break; }
+        c->num_sms = v;
+        if ((e = cudaDeviceGetAttribute(&v, cudaDevAttrMaxSharedMemoryPerBlockOptin, device)) != cudaSuccess) { st = cuda_fail(nullptr, e, "attr"); break; }
+        c->smem_optin = (size_t)v;
+        for (int d = 0; d < 3; ++d) {
+            c->fd[d] = fixed_dims[d]; c->md[d] = moving_dims[d];
+            c->fs[d] = fixed_spacing[d]; c->ms[d] = moving_spacing[d];
+        }
+        c->nb = nbins; c->nf = nf; c->nm = nm;
+        c->flo = fixed_lo; c->fhi = fixed_hi; c->mlo = moving_lo; c->mhi = moving_hi;
+        c->fscale = mi::bin_scale(nbins, fixed_lo, fixed_hi);
+        c->mscale = mi::bin_scale(nbins, moving_lo, moving_hi);
+        // +16 bytes of slack so 16-byte vector stores of the last partial group stay inside
+        if ((e = cudaMalloc((void**)&c->d_fbins, (size_t)nf + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc fixed bins"); break; }
+        if ((e = cudaMalloc((void**)&c->d_mbins, (size_t)nm + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bins"); break; }
+        if ((e = cudaMalloc((void**)&c->d_moving, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
+        if ((e = cudaMalloc((void**)&d_tmp, (size_t)nf * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
+        if ((e = cudaEventCreateWithFlags(&c->ev_staging, cudaEventDisableTiming)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaEventCreate"); break; }
+        cudaStream_t s = c->stream;
+        if ((e = cudaMemcpyAsync(d_tmp, fixed, (size_t)nf * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy fixed"); break; }
+        if ((e = cudaMemcpyAsync(c->d_moving, moving, (size_t)nm * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy moving"); break; }
+        if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
+        if ((e = mi::launch_prebin(c->d_moving, c->d_mbins, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
+    } while (false);
+    if (d_tmp) cudaFree(d_tmp);
+    if (st != MI_OK) {
+        mi_destroy(c);
+        return st;
+    }
+    *out = c;
+    return MI_OK;
+}
+
+void mi_destroy(mi_ctx* c) {
+    if (!c) return;
+    DeviceGuard guard(c->device);
+    if (guard.ok) {
+        cudaStreamSynchronize(c->stream);
+        cudaFree(c->d_fbins); cudaFree(c->d_moving); cudaFree(c->d_mbins);
+        cudaFree(c->d_M); cudaFree(c->d_hist); cudaFree(c->d_mi); cudaFree(c->d_nvalid);
+        cudaFree(c->d_q); cudaFree(c->d_map); cudaFree(c->d_argmax);
+        if (c->h_M) cudaFreeHost(c->h_M);
+        if (c->ev_staging) cudaEventDestroy(c->ev_staging);
+        cudaGetLastError();
+    }
+    delete c;
+}
+
+mi_status mi_set_tsallis_form(mi_ctx* c, mi_tsallis_form form) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (form != MI_TSALLIS_ADDITIVE && form != MI_TSALLIS_PSEUDO_ADDITIVE)
+        return fail(c, MI_ERR_INVALID_ARG, "unknown Tsallis form");
+    c->tsallis_form = (int)form;
+    return MI_OK;
+}
+
+mi_status mi_eval_batch(mi_ctx* c, const double* T, int64_t N, const double* q, int32_t nq,
+                        mi_interp interp, double* mi_out, uint32_t* hist_out, int64_t* nvalid_out) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (N < 0) return fail(c, MI_ERR_INVALID_ARG, "N < 0");
+    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
+        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
+    mi_status st = validate_q(c, q, nq);
+    if (st != MI_OK) return st;
+    if (N == 0) return MI_OK;
+    if (T == nullptr || mi_out == nullptr) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
+    if (N > 0x7FFFFFFFLL / 16) return fail(c, MI_ERR_UNSUPPORTED, "too many transforms in one call");
+    std::vector<float> hM;
+    try {
+        hM.resize((size_t)N * 12);
+    } catch (const std::bad_alloc&) {
+        return fail(c, MI_ERR_OUT_OF_MEMORY, "host allocation failed");
+    }
+    for (int64_t t = 0; t < N; ++t) {
+        const double* Tt = T + t * 12;
+        for (int i = 0; i < 12; ++i)
+            if (!std::isfinite(Tt[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite matrix entry");
+        mi::index_affine(Tt, c->fd, c->fs, c->md, c->ms, hM.data() + t * 12);
+    }
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    return eval_core(c, hM, N, q, nq, (int)interp, mi_out, hist_out, nvalid_out, nullptr, nullptr);
+}
+
+mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
+                 const double* q, int32_t nq, mi_interp interp, double* map_out, int64_t* argmax_out) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (!lo || !hi || !n || !map_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
+    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
+        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
+    if ((int)family < 0 || (int)family > MI_FAMILY_SCALE_LOG) return fail(c, MI_ERR_INVALID_ARG, "unknown family");
+    if (!finite3(lo) || !finite3(hi)) return fail(c, MI_ERR_INVALID_ARG, "non-finite grid bound");
+    int64_t N = 1;
+    for (int d = 0; d < 3; ++d) {
+        if (n[d] < 1) return fail(c, MI_ERR_INVALID_ARG, "grid n < 1");
+        N *= n[d];
+        if (N > 0x7FFFFFFFLL / 16) return fail(c, MI_ERR_UNSUPPORTED, "too many transforms in one call");
+    }
+    mi_status st = validate_q(c, q, nq);
+    if (st != MI_OK) return st;
+    std::vector<float> hM;
+    try {
+        hM.resize((size_t)N * 12);
+    } catch (const std::bad_alloc&) {
+        return fail(c, MI_ERR_OUT_OF_MEMORY, "host allocation failed");
+    }
+    // step a2: one transform per grid node, p0 fastest
+    for (int k2 = 0; k2 < n[2]; ++k2)
+        for (int k1 = 0; k1 < n[1]; ++k1)
+            for (int k0 = 0; k0 < n[0]; ++k0) {
+                const int kk[3] = {k0, k1, k2};
+                double p[3], T[12];
+                for (int d = 0; d < 3; ++d)
+                    p[d] = n[d] == 1 ? lo[d] : lo[d] + (double)kk[d] * (hi[d] - lo[d]) / (double)(n[d] - 1);
+                mi::family_matrix((int)family, p, T);
+                for (int i = 0; i < 12; ++i)
+                    if (!std::isfinite(T[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite matrix entry");
+                const int64_t t = ((int64_t)k2 * n[1] + k1) * n[0] + k0;
+                mi::index_affine(T, c->fd, c->fs, c->md, c->ms, hM.data() + t * 12);
+            }
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    return eval_core(c, hM, N, q, nq, (int)interp, nullptr, nullptr, nullptr, map_out, argmax_out);
+}
+
+mi_status mi_get_bins(mi_ctx* c, int32_t which, uint8_t* out) {
+    if (!c || !out) return MI_ERR_INVALID_ARG;
+    if (which != 0 && which != 1) return fail(c, MI_ERR_INVALID_ARG, "which must be 0 or 1");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    const uint8_t* src = which == 0 ? c->d_fbins : c->d_mbins;
+    const size_t n = (size_t)(which == 0 ? c->nf : c->nm);
+    MI_CUDA(c, cudaMemcpyAsync(out, src, n, cudaMemcpyDefault, c->stream));
+    MI_CUDA(c, cudaStreamSynchronize(c->stream));
+    return MI_OK;
+}
+
+mi_status mi_last_timing(const mi_ctx* c, float ms[4], int64_t launches[4]) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    for (int k = 0; k < 4; ++k) {
+        if (ms) ms[k] = c->last_ms[k];
+        if (launches) launches[k] = c->last_launches[k];
+    }
+    return MI_OK;
+}
+
+mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
+                                      double* updates_per_s) {
+    if (!updates_per_s || nbins < 8 || nbins > 256 || pattern < 0 || pattern > 2 || iters < 1)
+        return MI_ERR_INVALID_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
+    if (device < 0 || device >= ndev) return MI_ERR_INVALID_ARG;
+    DeviceGuard guard(device);
+    if (!guard.ok) return MI_ERR_CUDA;
+    int sms = 0, smem = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return MI_ERR_CUDA;
+    if (cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, device) != cudaSuccess) return MI_ERR_CUDA;
+    const cudaError_t e = mi::run_shared_atomic_probe(nbins, pattern, iters, sms, (size_t)smem, updates_per_s);
+    if (e != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
+    return MI_OK;
+}
+
+}  // extern "C"

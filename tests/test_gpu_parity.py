@@ -1,0 +1,268 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Bars (BASELINE.json north_star): nearest-neighbour joint histograms bit-exact;
+trilinear: at most 1e-5 of the voxels may change bin; every MI value within 1e-4 nats; identical
+arg max of the maps."""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_1909_10690_b200 import phantoms as ph
+
+pytestmark = pytest.mark.gpu
+
+MI_TOL = 1e-4          # nats, absolute (north_star)
+FLIP_FRAC = 1e-5       # fraction of voxels allowed to change bin in trilinear mode (north_star)
+
+
+@pytest.fixture(scope="module")
+def mi():
+    from paper_1909_10690_b200 import build
+    build.build()
+    from paper_1909_10690_b200 import binding
+    return binding
+
+
+def make_ctx(mi, fixed, moving, fs, ms, nb, ranges=(0, 1, 0, 1)):
+    return mi.mi_create(fixed, moving, fs, ms, nb, *ranges)
+
+
+def rand_physical(rng, n, rot_deg=8.0, shift=3.0, scale=0.08):
+    Ts = []
+    for _ in range(n):
+        R = ph.euler_deg_matrix(rng.uniform(-rot_deg, rot_deg, 3))[:, :3]
+        A = R @ np.diag(1 + rng.uniform(-scale, scale, 3))
+        Ts.append(np.concatenate([A, rng.uniform(-shift, shift, 3)[:, None]], axis=1))
+    return np.stack(Ts)
+
+
+def check_batch(mi, fixed, moving, fs, ms, nb, T, q, ranges=(0, 1, 0, 1), form=0):
+    """Compare hist / nvalid / MI of both interpolators against the oracle for transforms T."""
+    fd, md = fixed.shape[::-1], moving.shape[::-1]
+    M = orc.physical_to_index(T, fd, fs, md, ms)
+    with make_ctx(mi, fixed, moving, fs, ms, nb, ranges) as ctx:
+        mi.mi_set_tsallis_form(ctx, form)
+        for interp in (mi.MI_INTERP_NEAREST, mi.MI_INTERP_TRILINEAR):
+            ref = orc.eval_batch(fixed, moving, M, nb, *ranges, interp, q=q, form=form, want_hist=True)
+            vals, hist, nvalid = mi.mi_eval_batch(ctx, T, q, interp, hist_out=True, nvalid_out=True)
+            moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
+            if interp == mi.MI_INTERP_NEAREST:
+                assert np.array_equal(hist, ref["hist"]), "NN histograms must be bit-exact"
+                assert np.array_equal(nvalid, ref["nvalid"])
+            else:
+                assert np.all(moved <= FLIP_FRAC * fixed.size), moved.max()
+                assert np.all(np.abs(nvalid - ref["nvalid"]) <= FLIP_FRAC * fixed.size)
+            assert np.array_equal(hist.sum(axis=(1, 2)), nvalid)
+            assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL, np.max(np.abs(vals - ref["mi"]))
+    return True
+
+
+# ------------------------------------------------------------------------------------------------
+def test_prebin_bit_exact(mi):
+    rng = np.random.default_rng(0)
+    fixed = (rng.normal(0.4, 0.4, (13, 21, 37))).astype(np.float32)     # ragged, values outside range
+    moving = (rng.normal(10, 5, (9, 17, 50))).astype(np.float32)
+    for nb in (2, 64, 255, 256):
+        with make_ctx(mi, fixed, moving, (1, 1, 1), (1, 1, 1), nb, (0, 1, 2.5, 19.0)) as ctx:
+            assert np.array_equal(mi.mi_get_bins(ctx, 0), orc.prebin(fixed, nb, 0, 1))
+            assert np.array_equal(mi.mi_get_bins(ctx, 1), orc.prebin(moving, nb, 2.5, 19.0))
+    cfg = ph.get_config("C1")
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 64) as ctx:
+        assert np.array_equal(mi.mi_get_bins(ctx, 0), orc.prebin(cfg.fixed, 64, 0, 1))
+
+
+def test_c1_batch_both_interpolators(mi):
+    cfg = ph.get_config("C1")
+    rng = np.random.default_rng(1)
+    T = np.concatenate([rand_physical(rng, 12), np.stack([orc.family_matrix(0, p) for p in
+                        [(0, 0, 0), (1.5, -2, 0.5), (0.5, 0.5, 0.5), (-2, 2, 1)]])])
+    check_batch(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 64, T, cfg.q)
+    check_batch(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 64, T, (0.5, 2.0), form=1)
+
+
+def test_c2_small_128_bins(mi):
+    cfg = ph.get_config("C2", size=64, grid_n=3)
+    rng = np.random.default_rng(2)
+    check_batch(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 128, rand_physical(rng, 6), cfg.q)
+
+
+def test_256_bins_ragged_anisotropic_multimodal(mi):
+    """C5-shaped at 1/4 resolution: different dims and spacings, 256 bins (packed 16-bit path),
+    sizes that span several tiles with ragged rows (65 = 2*32 + 1)."""
+    cfg = ph.get_config("C5", res=0.25, grid_n=3)
+    rng = np.random.default_rng(3)
+    T = np.concatenate([rand_physical(rng, 5, shift=8.0),
+                        np.stack([orc.family_matrix(0, p) for p in [(3.2, -4.7, 1.1), (-10, 10, -10)]])])
+    check_batch(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256, T, (0.2, 1.5))
+
+
+def test_many_transforms_one_cta_each_and_two_q_passes(mi):
+    """>= 16 waves of transforms -> one CTA per transform (nslabs = 1); 10 q values -> two entropy passes."""
+    rng = np.random.default_rng(4)
+    fixed = ph.random_volume((16, 12, 10), 5)
+    moving = ph.random_volume((14, 13, 11), 6)
+    T = rand_physical(rng, 2500, rot_deg=20, shift=2.0)
+    q = (0.2, 0.5, 0.8, 0.9, 1.0, 1.1, 1.5, 2.0, 2.5, 3.0)
+    check_batch(mi, fixed, moving, (1, 1, 1), (1.1, 0.9, 1.0), 32, T, q)
+
+
+def test_packed_counter_drain_and_hot_bin(mi):
+    """Constant images put every voxel in ONE bin: exercises the 2^15 drain of the packed 16-bit
+    counters (256 bins) and, for bin (0,0), the private hot-bin counter."""
+    n = (64, 64, 40)
+    ident = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)[None]
+    for fv, mv in [(0.3, 0.7), (0.0, 0.0), (0.0, 0.5)]:
+        fixed = np.full(n[::-1], fv, dtype=np.float32)
+        moving = np.full(n[::-1], mv, dtype=np.float32)
+        for nb in (256, 128):
+            with make_ctx(mi, fixed, moving, (1, 1, 1), (1, 1, 1), nb) as ctx:
+                for interp in (0, 1):
+                    vals, hist, nvalid = mi.mi_eval_batch(ctx, ident, (0.5,), interp, hist_out=True, nvalid_out=True)
+                    assert nvalid[0] == fixed.size
+                    a, b = min(int(fv * nb), nb - 1), min(int(mv * nb), nb - 1)
+                    assert hist[0, a, b] == fixed.size and hist.sum() == fixed.size
+                    assert np.all(np.abs(vals) < 1e-9)
+    # half the volume in one bin, the rest random: drain + ordinary traffic together
+    fixed = ph.random_volume(n, 7); fixed[:20] = 0.25
+    moving = ph.random_volume(n, 8); moving[:20] = 0.75
+    check_batch(mi, fixed, moving, (1, 1, 1), (1, 1, 1), 256, ident, (2.0,))
+
+
+def test_degenerate_cases(mi):
+    cfg = ph.get_config("C1")
+    far = orc.family_matrix(0, (1000, 0, 0))[None]
+    zero = np.zeros((1, 3, 4)); zero[0, :, 3] = (0.3, -0.2, 0.1)        # singular: every voxel samples one point
+    flip = np.concatenate([np.diag([-1.0, 1, 1]), np.zeros((3, 1))], axis=1)[None]
+    T = np.concatenate([far, zero, flip])
+    check_batch(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 64, T, (0.5, 2.0))
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 64) as ctx:
+        vals, _, nvalid = mi.mi_eval_batch(ctx, far, (0.5, 2.0), 1, nvalid_out=True)
+        assert nvalid[0] == 0 and np.all(vals == 0.0)                   # empty overlap -> zeros
+        out = mi.mi_eval_batch(ctx, np.zeros((0, 3, 4)), (), 1)[0]      # N = 0 is a no-op
+        assert out.shape == (0, 1)
+        with pytest.raises(mi.MIError) as ei:
+            mi.mi_eval_batch(ctx, far, (-1.0,), 1)
+        assert ei.value.status == mi.MI_ERR_INVALID_ARG
+        bad = far.copy(); bad[0, 0, 0] = np.nan
+        with pytest.raises(mi.MIError):
+            mi.mi_eval_batch(ctx, bad, (), 1)
+    # tiny volumes: 1 voxel, 2 bins; rows shorter than a warp
+    one = np.full((1, 1, 1), 0.6, dtype=np.float32)
+    ident = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)[None]
+    check_batch(mi, one, one, (1, 1, 1), (1, 1, 1), 2, ident, (2.0,))
+    small = ph.random_volume((5, 3, 2), 11)
+    check_batch(mi, small, ph.random_volume((4, 6, 3), 12), (1, 1, 1), (1, 1, 1), 8, rand_physical(np.random.default_rng(5), 4, shift=1.0), ())
+
+
+def test_identity_self_pair_is_diagonal(mi):
+    cfg = ph.get_config("C1")
+    ident = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)[None]
+    with make_ctx(mi, cfg.fixed, cfg.fixed, cfg.fixed_spacing, cfg.fixed_spacing, 64) as ctx:
+        vals, hist, nvalid = mi.mi_eval_batch(ctx, ident, (), 1, hist_out=True, nvalid_out=True)
+        assert nvalid[0] == cfg.fixed.size
+        assert np.count_nonzero(hist[0] - np.diag(np.diag(hist[0]))) == 0
+        p = np.diag(hist[0]) / cfg.fixed.size
+        assert vals[0, 0] == pytest.approx(-np.sum(p[p > 0] * np.log(p[p > 0])), abs=1e-9)
+
+
+def test_device_pointers_in_and_out(mi):
+    import torch
+    cfg = ph.get_config("C1")
+    rng = np.random.default_rng(6)
+    T = rand_physical(rng, 5)
+    q = (0.5, 2.0)
+    dev = torch.device("cuda:0")
+    fx, mv = torch.from_numpy(cfg.fixed).to(dev), torch.from_numpy(cfg.moving).to(dev)
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx_d = mi.mi_create(fx, mv, cfg.fixed_spacing, cfg.moving_spacing, 64, cuda_stream=stream)
+    ctx_h = make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 64)
+    try:
+        vd = torch.empty((5, 3), dtype=torch.float64, device=dev)
+        hd = torch.empty((5, 64, 64), dtype=torch.int32, device=dev)
+        nd = torch.empty(5, dtype=torch.int64, device=dev)
+        mi.mi_eval_batch(ctx_d, T, q, 1, mi_out=vd, hist_out=hd, nvalid_out=nd)
+        torch.cuda.synchronize()
+        vh, hh, nh = mi.mi_eval_batch(ctx_h, T, q, 1, hist_out=True, nvalid_out=True)
+        assert np.array_equal(vd.cpu().numpy(), vh)
+        assert np.array_equal(hd.cpu().numpy().view(np.uint32), hh)
+        assert np.array_equal(nd.cpu().numpy(), nh)
+        md = torch.empty((3, 3, 3, 3), dtype=torch.float64, device=dev)
+        ad = torch.empty(3, dtype=torch.int64, device=dev)
+        mi.mi_map(ctx_d, 0, (-1,) * 3, (1,) * 3, (3,) * 3, q, 1, map_out=md, argmax_out=ad)
+        torch.cuda.synchronize()
+        mh, ah = mi.mi_map(ctx_h, 0, (-1,) * 3, (1,) * 3, (3,) * 3, q, 1)
+        assert np.array_equal(md.cpu().numpy(), mh) and np.array_equal(ad.cpu().numpy(), ah)
+    finally:
+        mi.mi_destroy(ctx_d)
+        mi.mi_destroy(ctx_h)
+
+
+# ------------------------------------------------------------------------------------------------ maps
+def check_map(mi, cfg, interp, form=0, atol=MI_TOL):
+    ref = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                     cfg.family, cfg.lo, cfg.hi, cfg.n, q=cfg.q, form=form, interp=interp)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins, cfg.ranges) as ctx:
+        mi.mi_set_tsallis_form(ctx, form)
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, interp)
+    assert m.shape == ref["map"].shape
+    assert np.max(np.abs(m - ref["map"])) <= atol
+    assert np.array_equal(am, ref["argmax"]), (am, ref["argmax"])
+    return m, am
+
+
+def test_c1_full_map_both_interpolators_and_forms(mi):
+    cfg = ph.get_config("C1")
+    for interp in (0, 1):
+        m, am = check_map(mi, cfg, interp)
+    check_map(mi, cfg, 1, form=1)
+    k2, k1, k0 = np.unravel_index(am[0], m.shape[1:])
+    p = [cfg.lo[d] + k * (cfg.hi[d] - cfg.lo[d]) / (cfg.n[d] - 1) for d, k in enumerate((k0, k1, k2))]
+    assert max(abs(p[d] - cfg.truth[d]) for d in range(3)) <= 1.0       # pin P11 on the GPU map too
+
+
+def test_c1_half_step_map_exercises_trilinear_weights(mi):
+    cfg = ph.config_c1(grid_n=9)
+    check_map(mi, cfg, 1)
+
+
+def test_c2_reduced_map(mi):
+    check_map(mi, ph.get_config("C2", size=64, grid_n=7, half_range=3.0), 1)
+
+
+def test_c3_c4_reduced_maps_rotation_and_scale(mi):
+    check_map(mi, ph.get_config("C3", res=0.25, grid_n=5), 1)
+    check_map(mi, ph.get_config("C4", res=0.25, grid_n=5), 1)
+    c3 = ph.get_config("C3", res=0.25, grid_n=5)
+    c3v = ph.Config("C3v", c3.fixed, c3.moving, c3.fixed_spacing, c3.moving_spacing, 256, 2,
+                    (-0.06,) * 3, (0.06,) * 3, (3, 3, 3), (1.1,), c3.truth)
+    check_map(mi, c3v, 0)                                               # versor family, NN
+    c4 = ph.get_config("C4", res=0.25, grid_n=5)
+    c4l = ph.Config("C4l", c4.fixed, c4.moving, c4.fixed_spacing, c4.moving_spacing, 256, 4,
+                    (-0.1,) * 3, (0.1,) * 3, (3, 3, 3), (0.5,), c4.truth)
+    check_map(mi, c4l, 1)                                               # log-scale family
+
+
+def test_c5_reduced_map(mi):
+    check_map(mi, ph.get_config("C5", res=0.25, grid_n=7), 1)
+    check_map(mi, ph.get_config("C5", res=0.25, grid_n=5), 0)
+
+
+def test_c5_full_size_sampled_against_oracle(mi):
+    """BASELINE.json's full 260x311x260 / 182x218x182, 256-bin pair in the configuration bench.py
+    times; sampled transforms of the 41^3 grid are checked one by one against the oracle."""
+    cfg = ph.get_config("C5")
+    assert cfg.fixed.shape == (260, 311, 260) and cfg.moving.shape == (182, 218, 182)
+    nodes = [(0, 0, 0), (40, 40, 40), (26, 11, 22), (27, 10, 23), (13, 35, 7), (20, 20, 20)]
+    step = 20.0 / 40
+    T = np.stack([orc.family_matrix(0, [-10 + k * step for k in node]) for node in nodes])
+    fd, md = cfg.fixed.shape[::-1], cfg.moving.shape[::-1]
+    M = orc.physical_to_index(T, fd, cfg.fixed_spacing, md, cfg.moving_spacing)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
+        for interp in (0, 1):
+            ref = orc.eval_batch(cfg.fixed, cfg.moving, M, 256, 0, 1, 0, 1, interp, q=(0.5,), want_hist=True)
+            vals, hist, nvalid = mi.mi_eval_batch(ctx, T, (0.5,), interp, hist_out=True, nvalid_out=True)
+            moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
+            if interp == 0:
+                assert np.array_equal(hist, ref["hist"]) and np.array_equal(nvalid, ref["nvalid"])
+            else:
+                assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
+            assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
