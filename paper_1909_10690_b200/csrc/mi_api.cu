@@ -20,9 +20,13 @@ struct mi_ctx {
     int nb = 0;
     float flo = 0, fhi = 1, mlo = 0, mhi = 1, fscale = 1, mscale = 1;
     int64_t nf = 0, nm = 0;
-    uint8_t* d_fbins = nullptr;
-    float* d_moving = nullptr;
+    uint8_t* d_fbins = nullptr;         // fixed bins (CANON-5), as mi_get_bins returns them
+    uint8_t* d_fbins_ranked = nullptr;  // fixed bins replaced by their population rank
+    uint8_t* d_rank = nullptr;          // 256: fixed bin -> rank
+    int* d_rank_inv = nullptr;          // 256: rank -> fixed bin
+    float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
+    int rows_smem = 0;
     int tsallis_form = MI_TSALLIS_ADDITIVE;
     int num_sms = 148;
     size_t smem_optin = 48 * 1024;
@@ -185,9 +189,11 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         timer.begin(1);
         MI_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)cnt * nbins2 * sizeof(uint32_t), s));
         mi::ResampleArgs a;
-        a.fbins = c->d_fbins;
-        a.moving = c->d_moving;
+        a.fbins_ranked = c->d_fbins_ranked;
+        a.rank_inv = c->d_rank_inv;
+        a.moving_pad = c->d_moving_pad;
         a.mbins = c->d_mbins;
+        a.rows_smem = c->rows_smem;
         a.M = c->d_M + (size_t)off * 12;
         a.hist = hist;
         a.f = {c->fd[0], c->fd[1], c->fd[2]};
@@ -206,7 +212,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             if (nslabs > cap) nslabs = cap;
         }
         a.nslabs = nslabs;
-        MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, c->smem_optin, s));
+        MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, s));
         c->last_launches[1] += 1;
         timer.end();
 
@@ -314,7 +320,11 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         nm *= moving_dims[d];
         if (nf > 0x7FFFFFFFLL || nm > 0x7FFFFFFFLL)
             return fail(nullptr, MI_ERR_UNSUPPORTED, "volume has more than 2^31-1 voxels");
+        if (moving_dims[d] > 4194302)  // the kernels' floor trick needs |index| < 2^22
+            return fail(nullptr, MI_ERR_UNSUPPORTED, "moving volume dimension > 4194302");
     }
+    const int64_t npad = ((int64_t)moving_dims[0] + 2) * ((int64_t)moving_dims[1] + 2) * ((int64_t)moving_dims[2] + 2);
+    if (npad > 0x7FFFFFFFLL) return fail(nullptr, MI_ERR_UNSUPPORTED, "padded moving volume has more than 2^31-1 voxels");
     if (nbins < 2) return fail(nullptr, MI_ERR_INVALID_ARG, "nbins < 2");
     if (nbins > 256) return fail(nullptr, MI_ERR_UNSUPPORTED, "nbins > 256 is not supported");
     if (!(std::isfinite(fixed_lo) && std::isfinite(fixed_hi) && fixed_lo < fixed_hi) ||
@@ -333,6 +343,8 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
     DeviceGuard guard(device);
     mi_status st = MI_OK;
     float* d_tmp = nullptr;
+    float* d_mov = nullptr;
+    unsigned long long* d_counts = nullptr;
     do {
         if (!guard.ok) { st = fail(nullptr, MI_ERR_CUDA, "cudaSetDevice failed"); break; }
         int v = 0;
@@ -351,17 +363,28 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         // +16 bytes of slack so 16-byte vector stores of the last partial group stay inside
         if ((e = cudaMalloc((void**)&c->d_fbins, (size_t)nf + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc fixed bins"); break; }
         if ((e = cudaMalloc((void**)&c->d_mbins, (size_t)nm + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bins"); break; }
-        if ((e = cudaMalloc((void**)&c->d_moving, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
+        if ((e = cudaMalloc((void**)&c->d_fbins_ranked, (size_t)nf + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc ranked bins"); break; }
+        if ((e = cudaMalloc((void**)&c->d_rank, 256)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank"); break; }
+        if ((e = cudaMalloc((void**)&c->d_rank_inv, 256 * sizeof(int))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank_inv"); break; }
+        if ((e = cudaMalloc((void**)&d_counts, 256 * sizeof(unsigned long long))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc counts"); break; }
+        if ((e = cudaMalloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
+        if ((e = cudaMalloc((void**)&d_mov, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
         if ((e = cudaMalloc((void**)&d_tmp, (size_t)nf * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
+        c->rows_smem = mi::hist_rows_in_smem(nbins, c->smem_optin);
+        if (c->rows_smem < 1) { st = fail(nullptr, MI_ERR_UNSUPPORTED, "device has too little shared memory"); break; }
         if ((e = cudaEventCreateWithFlags(&c->ev_staging, cudaEventDisableTiming)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaEventCreate"); break; }
         cudaStream_t s = c->stream;
         if ((e = cudaMemcpyAsync(d_tmp, fixed, (size_t)nf * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy fixed"); break; }
-        if ((e = cudaMemcpyAsync(c->d_moving, moving, (size_t)nm * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy moving"); break; }
+        if ((e = cudaMemcpyAsync(d_mov, moving, (size_t)nm * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy moving"); break; }
         if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
-        if ((e = mi::launch_prebin(c->d_moving, c->d_mbins, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
+        if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
+        if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
+        if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
     if (d_tmp) cudaFree(d_tmp);
+    if (d_mov) cudaFree(d_mov);
+    if (d_counts) cudaFree(d_counts);
     if (st != MI_OK) {
         mi_destroy(c);
         return st;
@@ -375,7 +398,8 @@ void mi_destroy(mi_ctx* c) {
     DeviceGuard guard(c->device);
     if (guard.ok) {
         cudaStreamSynchronize(c->stream);
-        cudaFree(c->d_fbins); cudaFree(c->d_moving); cudaFree(c->d_mbins);
+        cudaFree(c->d_fbins); cudaFree(c->d_fbins_ranked); cudaFree(c->d_rank); cudaFree(c->d_rank_inv);
+        cudaFree(c->d_moving_pad); cudaFree(c->d_mbins);
         cudaFree(c->d_M); cudaFree(c->d_hist); cudaFree(c->d_mi); cudaFree(c->d_nvalid);
         cudaFree(c->d_q); cudaFree(c->d_map); cudaFree(c->d_argmax);
         if (c->h_M) cudaFreeHost(c->h_M);

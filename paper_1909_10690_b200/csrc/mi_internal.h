@@ -24,11 +24,13 @@ struct VolumeDesc {
 };
 
 struct ResampleArgs {
-    const uint8_t* fbins;    // fixed bin indices, [fz][fy][fx]
-    const float* moving;     // moving float32 (trilinear)
-    const uint8_t* mbins;    // moving bin indices (nearest neighbour)
-    const float* M;          // n_transforms x 12 index-space affines (device)
-    uint32_t* hist;          // n_transforms x nb x nb, zero on entry
+    const uint8_t* fbins_ranked;  // fixed bins replaced by their population rank, [fz][fy][fx]
+    const int* rank_inv;          // rank -> fixed bin
+    const float* moving_pad;      // replicate-padded moving float32, dims (mx+2, my+2, mz+2)
+    const uint8_t* mbins;         // moving bin indices (nearest neighbour), unpadded
+    const float* M;               // n_transforms x 12 index-space affines (device)
+    uint32_t* hist;               // n_transforms x nb x nb (row = fixed bin), zero on entry
+    int rows_smem;                // ranked fixed-bin rows kept in shared memory
     VolumeDesc f, m;
     int nb;
     float mlo, mscale;       // moving binning (CANON-5)
@@ -38,8 +40,11 @@ struct ResampleArgs {
 
 cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, float scale, int nb,
                           cudaStream_t s);
-cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, size_t smem_optin,
-                                 cudaStream_t s);
+cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s);
+cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
+                                   uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s);
+int hist_rows_in_smem(int nb, size_t smem_optin);
+cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s);
 cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const double* q_dev, int nq,
                            int q_off, int form, double* mi_out /* n x (1+nq) */, int64_t* nvalid,
                            cudaStream_t s);

@@ -67,7 +67,95 @@ cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3 + a4: resample + joint histogram
+// a1b: helpers run once per context: replicate-padded moving volume, fixed-bin population ranks
+// ------------------------------------------------------------------------------------------------
+// pm has dims (nx+2, ny+2, nz+2); pm[z][y][x] = moving[clamp(z-1)][clamp(y-1)][clamp(x-1)].
+// Reading the 2x2x2 cell at padded index (jx+1, jy+1, jz+1), jk = floor(c_k) in [-1, n_k-1], gives
+// exactly the edge-clamped neighbours of CANON-4 (i0 = max(j,0), i1 = min(j+1, n-1)).
+__global__ void __launch_bounds__(256) pad_replicate_kernel(const float* __restrict__ src,
+                                                            float* __restrict__ dst, int nx, int ny, int nz) {
+    const int px = nx + 2, py = ny + 2, pz = nz + 2;
+    const int64_t total = (int64_t)px * py * pz;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % px);
+        const int64_t r = i / px;
+        const int y = (int)(r % py), z = (int)(r / py);
+        const int sx = min(max(x - 1, 0), nx - 1), sy = min(max(y - 1, 0), ny - 1), sz = min(max(z - 1, 0), nz - 1);
+        dst[i] = src[((int64_t)sz * ny + sy) * nx + sx];
+    }
+}
+
+cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s) {
+    const int64_t total = (int64_t)(nx + 2) * (ny + 2) * (nz + 2);
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    pad_replicate_kernel<<<(unsigned)blocks, 256, 0, s>>>(src, dst, nx, ny, nz);
+    return cudaGetLastError();
+}
+
+// 256-bin population count of a uint8 volume (CTA-private shared histogram, merged with atomics).
+__global__ void __launch_bounds__(256) bin_count_kernel(const uint8_t* __restrict__ bins, int64_t n,
+                                                        unsigned long long* __restrict__ counts) {
+    __shared__ unsigned sh[256];
+    sh[threadIdx.x] = 0u;
+    __syncthreads();
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        atomicAdd(&sh[bins[i]], 1u);
+    __syncthreads();
+    if (sh[threadIdx.x]) atomicAdd(&counts[threadIdx.x], (unsigned long long)sh[threadIdx.x]);
+}
+
+// rank[a] = position of fixed bin a when bins are sorted by falling population (ties: lower bin
+// first); inv[rank[a]] = a.  One CTA of 256 threads; counts has 256 entries.
+__global__ void __launch_bounds__(256) bin_rank_kernel(const unsigned long long* __restrict__ counts,
+                                                       uint8_t* __restrict__ rank, int* __restrict__ inv) {
+    __shared__ unsigned long long c[256];
+    c[threadIdx.x] = counts[threadIdx.x];
+    __syncthreads();
+    const unsigned long long mine = c[threadIdx.x];
+    int r = 0;
+    for (int j = 0; j < 256; ++j) r += (c[j] > mine) || (c[j] == mine && j < (int)threadIdx.x);
+    rank[threadIdx.x] = (uint8_t)r;
+    inv[r] = (int)threadIdx.x;
+}
+
+__global__ void __launch_bounds__(256) remap_bins_kernel(const uint8_t* __restrict__ in,
+                                                         uint8_t* __restrict__ out, int64_t n,
+                                                         const uint8_t* __restrict__ rank) {
+    __shared__ uint8_t lut[256];
+    lut[threadIdx.x] = rank[threadIdx.x];
+    __syncthreads();
+    const int64_t nvec = n >> 4;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        uint4 v = reinterpret_cast<const uint4*>(in)[i];
+        uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            w[k] = (uint32_t)lut[w[k] & 0xFF] | ((uint32_t)lut[(w[k] >> 8) & 0xFF] << 8) |
+                   ((uint32_t)lut[(w[k] >> 16) & 0xFF] << 16) | ((uint32_t)lut[w[k] >> 24] << 24);
+        reinterpret_cast<uint4*>(out)[i] = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+    const int64_t j = (nvec << 4) + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j < n) out[j] = lut[in[j]];
+}
+
+cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
+                                   uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(counts_scratch, 0, 256 * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return e;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks < 1) blocks = 1;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    bin_count_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, n, counts_scratch);
+    bin_rank_kernel<<<1, 256, 0, s>>>(counts_scratch, rank, inv);
+    remap_bins_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, ranked_bins, n, rank);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3 + a4: resample + joint histogram (generic affine)
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned warp_sum(unsigned v) {
 #pragma unroll
@@ -80,82 +168,87 @@ __device__ __forceinline__ float lerp_rn(float p, float q, float f) {
     return __fmaf_rn(f, __fsub_rn(q, p), p);
 }
 
-struct MovingView {
-    const float* __restrict__ vol;
-    const uint8_t* __restrict__ bins;
-    int nx, ny, nz;
-    float fx, fy, fz;  // (float)n
-    float lo, scale, top;
+// floor() of |c| < 2^22 without a conversion instruction: RD(c + 1.5*2^23) = 1.5*2^23 + floor(c)
+// exactly (ulp is 1 there), so the low mantissa bits ARE floor(c) as a two's-complement offset.
+constexpr float kFloorMagic = 12582912.0f;        // 1.5 * 2^23
+constexpr int kFloorMagicBits = 0x4B400000;
+
+struct Sample {
+    bool ok;   // inside the moving volume (CANON-3/4 validity)
+    int b;     // moving bin (meaningless if !ok)
 };
 
-// Moving bin of the sample at continuous index (cx,cy,cz), or -1 if it is outside the volume.
-// All loads use clamped (always in-bounds) addresses so they can be issued before the validity
-// test resolves.
+struct MovingView {
+    const float* __restrict__ pad;     // replicate-padded float volume, dims (nx+2, ny+2, nz+2)
+    const float* __restrict__ pad_y;   // pad + (nx+2)
+    const float* __restrict__ pad_z;   // pad + (nx+2)*(ny+2)
+    const float* __restrict__ pad_yz;  // pad + (nx+2)*(ny+2) + (nx+2)
+    const uint8_t* __restrict__ bins;  // unpadded bin volume (nearest neighbour)
+    int nx, ny;                        // unpadded dims (nearest neighbour indexing)
+    int pnx, pny;                      // padded dims
+    unsigned fold;                     // index constant folding the magic bits and the +1 padding
+    float fx, fy, fz;                  // (float)n
+    float hx, hy, hz;                  // (float)n - 0.5f
+    float lo, scale;
+    int top;                           // nb - 1
+};
+
 template <int INTERP>
-__device__ __forceinline__ int sample_bin(const MovingView& mv, float cx, float cy, float cz) {
+__device__ __forceinline__ Sample sample_bin(const MovingView& mv, float cx, float cy, float cz) {
+    Sample s;
     if (INTERP == MI_INTERP_NEAREST) {
-        // CANON-3: round half up, validity tested in float.
-        const float rx = floorf(__fadd_rn(cx, 0.5f));
-        const float ry = floorf(__fadd_rn(cy, 0.5f));
-        const float rz = floorf(__fadd_rn(cz, 0.5f));
-        const bool ok = rx >= 0.0f && rx < mv.fx && ry >= 0.0f && ry < mv.fy && rz >= 0.0f && rz < mv.fz;
-        const int jx = min(max(__float2int_rz(rx), 0), mv.nx - 1);
-        const int jy = min(max(__float2int_rz(ry), 0), mv.ny - 1);
-        const int jz = min(max(__float2int_rz(rz), 0), mv.nz - 1);
-        const int b = __ldg(mv.bins + ((jz * mv.ny + jy) * mv.nx + jx));
-        return ok ? b : -1;
+        // CANON-3: r = floor(c + 0.5) (round half up), validity tested on r in float.
+        const float tx = __fadd_rd(__fadd_rn(cx, 0.5f), kFloorMagic);
+        const float ty = __fadd_rd(__fadd_rn(cy, 0.5f), kFloorMagic);
+        const float tz = __fadd_rd(__fadd_rn(cz, 0.5f), kFloorMagic);
+        const float rx = __fsub_rn(tx, kFloorMagic), ry = __fsub_rn(ty, kFloorMagic), rz = __fsub_rn(tz, kFloorMagic);
+        s.ok = rx >= 0.0f && rx < mv.fx && ry >= 0.0f && ry < mv.fy && rz >= 0.0f && rz < mv.fz;
+        const int jx = __float_as_int(tx) - kFloorMagicBits, jy = __float_as_int(ty) - kFloorMagicBits,
+                  jz = __float_as_int(tz) - kFloorMagicBits;
+        unsigned idx = ((unsigned)jz * (unsigned)mv.ny + (unsigned)jy) * (unsigned)mv.nx + (unsigned)jx;
+        idx = s.ok ? idx : 0u;
+        s.b = __ldg(mv.bins + idx);
     } else {
-        // CANON-4: region [-0.5, n-0.5), edge clamp, x-lerps then y-lerps then the z-lerp.
-        const bool ok = cx >= -0.5f && cx < __fsub_rn(mv.fx, 0.5f) && cy >= -0.5f &&
-                        cy < __fsub_rn(mv.fy, 0.5f) && cz >= -0.5f && cz < __fsub_rn(mv.fz, 0.5f);
-        const float gx = floorf(cx), gy = floorf(cy), gz = floorf(cz);
-        const float tx = __fsub_rn(cx, gx), ty = __fsub_rn(cy, gy), tz = __fsub_rn(cz, gz);
-        const int jx = __float2int_rz(gx), jy = __float2int_rz(gy), jz = __float2int_rz(gz);
-        const int x0 = min(max(jx, 0), mv.nx - 1), x1 = max(min(jx + 1, mv.nx - 1), 0);
-        const int y0 = min(max(jy, 0), mv.ny - 1), y1 = max(min(jy + 1, mv.ny - 1), 0);
-        const int z0 = min(max(jz, 0), mv.nz - 1), z1 = max(min(jz + 1, mv.nz - 1), 0);
-        const int r00 = (z0 * mv.ny + y0) * mv.nx, r10 = (z0 * mv.ny + y1) * mv.nx;
-        const int r01 = (z1 * mv.ny + y0) * mv.nx, r11 = (z1 * mv.ny + y1) * mv.nx;
-        const float a000 = __ldg(mv.vol + r00 + x0), a100 = __ldg(mv.vol + r00 + x1);
-        const float a010 = __ldg(mv.vol + r10 + x0), a110 = __ldg(mv.vol + r10 + x1);
-        const float a001 = __ldg(mv.vol + r01 + x0), a101 = __ldg(mv.vol + r01 + x1);
-        const float a011 = __ldg(mv.vol + r11 + x0), a111 = __ldg(mv.vol + r11 + x1);
-        const float v00 = lerp_rn(a000, a100, tx);
-        const float v10 = lerp_rn(a010, a110, tx);
-        const float v01 = lerp_rn(a001, a101, tx);
-        const float v11 = lerp_rn(a011, a111, tx);
-        const float w0 = lerp_rn(v00, v10, ty);
-        const float w1 = lerp_rn(v01, v11, ty);
-        const float v = lerp_rn(w0, w1, tz);
-        const int b = bin_index(v, mv.lo, mv.scale, mv.top);
-        return ok ? b : -1;
+        // CANON-4: region [-0.5, n-0.5), edge clamp (via the padded copy), x- then y- then z-lerps.
+        s.ok = cx >= -0.5f && cx < mv.hx && cy >= -0.5f && cy < mv.hy && cz >= -0.5f && cz < mv.hz;
+        const float tx = __fadd_rd(cx, kFloorMagic), ty = __fadd_rd(cy, kFloorMagic), tz = __fadd_rd(cz, kFloorMagic);
+        const float wx = __fsub_rn(cx, __fsub_rn(tx, kFloorMagic));
+        const float wy = __fsub_rn(cy, __fsub_rn(ty, kFloorMagic));
+        const float wz = __fsub_rn(cz, __fsub_rn(tz, kFloorMagic));
+        unsigned idx = (__float_as_uint(tz) * (unsigned)mv.pny + __float_as_uint(ty)) * (unsigned)mv.pnx +
+                       __float_as_uint(tx) - mv.fold;
+        idx = s.ok ? idx : 0u;
+        const float a000 = __ldg(mv.pad + idx), a100 = __ldg(mv.pad + idx + 1);
+        const float a010 = __ldg(mv.pad_y + idx), a110 = __ldg(mv.pad_y + idx + 1);
+        const float a001 = __ldg(mv.pad_z + idx), a101 = __ldg(mv.pad_z + idx + 1);
+        const float a011 = __ldg(mv.pad_yz + idx), a111 = __ldg(mv.pad_yz + idx + 1);
+        const float v00 = lerp_rn(a000, a100, wx);
+        const float v10 = lerp_rn(a010, a110, wx);
+        const float v01 = lerp_rn(a001, a101, wx);
+        const float v11 = lerp_rn(a011, a111, wx);
+        const float w0 = lerp_rn(v00, v10, wy);
+        const float w1 = lerp_rn(v01, v11, wy);
+        const float v = lerp_rn(w0, w1, wz);
+        // CANON-5 with the floor/clamp done on the integer side (same result for finite v)
+        const float t = __fmul_rn(__fsub_rn(v, mv.lo), mv.scale);
+        s.b = min(max(__float2int_rd(t), 0), mv.top);
     }
+    return s;
 }
 
-// CTA-private histogram update.  PACK16: two 16-bit counters per word (256 bins -> 128 KB); a
-// counter that reaches 2^15 is drained to the global histogram by the thread whose add set bit 15,
-// so counters never carry into their neighbour (at most 1024 adds can land before the drain).
-template <bool PACK16>
-__device__ __forceinline__ void hist_add(uint32_t* sh, uint32_t* gh, int idx) {
-    if (PACK16) {
-        const unsigned shift = (idx & 1) << 4;
-        const unsigned old = atomicAdd(&sh[idx >> 1], 1u << shift);
-        if (((old >> shift) & 0xFFFFu) == 0x7FFFu) {
-            atomicSub(&sh[idx >> 1], 0x8000u << shift);
-            atomicAdd(&gh[idx], 0x8000u);
-        }
-    } else {
-        atomicAdd(&sh[idx], 1u);
-    }
-}
-
-template <int INTERP, bool PACK16, int UNROLL>
+// One CTA works on one (transform, row slab) item at a time.  The joint histogram lives in shared
+// memory as u32 counters updated with result-less atomics (the fastest shared atomic on sm_100a,
+// see profiles/).  Fixed bins arrive RANKED by population: the `rows_smem` most populated fixed-bin
+// rows are in shared memory, the rare tail (only when nb*nb*4 B exceeds shared memory, i.e. 256
+// bins) is added straight to the global histogram.
+template <int INTERP, int UNROLL>
 __global__ void __launch_bounds__(kHistThreads, 1)
 resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     extern __shared__ __align__(16) uint32_t sh_hist[];
     const int nb = a.nb;
     const int nbins2 = nb * nb;
-    const int words = PACK16 ? (nbins2 + 1) / 2 : nbins2;
+    const int rows_smem = a.rows_smem;
+    const int words = rows_smem * nb;
     for (int w = threadIdx.x; w < words; w += blockDim.x) sh_hist[w] = 0u;
     __syncthreads();
 
@@ -166,11 +259,19 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     const int rows_total = a.f.ny * a.f.nz;
 
     MovingView mv;
-    mv.vol = a.moving;
+    mv.pnx = a.m.nx + 2; mv.pny = a.m.ny + 2;
+    mv.pad = a.moving_pad;
+    mv.pad_y = a.moving_pad + mv.pnx;
+    mv.pad_z = a.moving_pad + (size_t)mv.pnx * mv.pny;
+    mv.pad_yz = mv.pad_z + mv.pnx;
     mv.bins = a.mbins;
-    mv.nx = a.m.nx; mv.ny = a.m.ny; mv.nz = a.m.nz;
+    mv.nx = a.m.nx; mv.ny = a.m.ny;
+    // padded index of cell (jx+1, jy+1, jz+1) from the raw float bits T_k = magic + j_k:
+    // ((Tz*pny + Ty)*pnx + Tx) - (magic-1)*(pny*pnx + pnx + 1), all modulo 2^32.
+    mv.fold = (unsigned)(kFloorMagicBits - 1) * (unsigned)(mv.pny * mv.pnx + mv.pnx + 1);
     mv.fx = (float)a.m.nx; mv.fy = (float)a.m.ny; mv.fz = (float)a.m.nz;
-    mv.lo = a.mlo; mv.scale = a.mscale; mv.top = (float)(nb - 1);
+    mv.hx = __fsub_rn(mv.fx, 0.5f); mv.hy = __fsub_rn(mv.fy, 0.5f); mv.hz = __fsub_rn(mv.fz, 0.5f);
+    mv.lo = a.mlo; mv.scale = a.mscale; mv.top = nb - 1;
 
     const long long nitems = (long long)a.n_transforms * a.nslabs;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
@@ -182,7 +283,6 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
 #pragma unroll
         for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
         uint32_t* gh = a.hist + (size_t)t * nbins2;
-        unsigned cnt0 = 0;  // private count of bin (0,0): the background-on-background hot spot
 
         for (int row = row_lo + warp; row < row_hi; row += nwarps) {
             const int iz = row / a.f.ny;
@@ -192,43 +292,40 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
             const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
             const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
             const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
-            const uint8_t* __restrict__ frow = a.fbins + (size_t)row * fnx;
+            const uint8_t* __restrict__ frow = a.fbins_ranked + (size_t)row * fnx;
             for (int ix0 = lane; ix0 < fnx; ix0 += 32 * UNROLL) {
-                int idx[UNROLL];
+                Sample smp[UNROLL];
+                int fa[UNROLL];
 #pragma unroll
                 for (int u = 0; u < UNROLL; ++u) {
-                    const int ix = ix0 + 32 * u;
-                    idx[u] = -1;
-                    if (ix < fnx) {
-                        const float fx = (float)ix;
-                        const float cx = __fmaf_rn(m[0], fx, rx);
-                        const float cy = __fmaf_rn(m[4], fx, ry);
-                        const float cz = __fmaf_rn(m[8], fx, rz);
-                        const int b = sample_bin<INTERP>(mv, cx, cy, cz);
-                        const int fa = __ldg(frow + ix);
-                        idx[u] = b >= 0 ? fa * nb + b : -1;
-                    }
+                    const int ix = min(ix0 + 32 * u, fnx - 1);   // clamped: always a legal voxel
+                    const float fx = (float)ix;
+                    const float cx = __fmaf_rn(m[0], fx, rx);
+                    const float cy = __fmaf_rn(m[4], fx, ry);
+                    const float cz = __fmaf_rn(m[8], fx, rz);
+                    smp[u] = sample_bin<INTERP>(mv, cx, cy, cz);
+                    smp[u].ok = smp[u].ok && (ix0 + 32 * u < fnx);
+                    fa[u] = __ldg(frow + ix);
                 }
 #pragma unroll
                 for (int u = 0; u < UNROLL; ++u) {
-                    if (idx[u] == 0) ++cnt0;
-                    else if (idx[u] > 0) hist_add<PACK16>(sh_hist, gh, idx[u]);
+                    if (smp[u].ok) {
+                        if (fa[u] < rows_smem) atomicAdd(&sh_hist[fa[u] * nb + smp[u].b], 1u);
+                        else atomicAdd(&gh[__ldg(a.rank_inv + fa[u]) * nb + smp[u].b], 1u);
+                    }
                 }
             }
         }
-        cnt0 = warp_sum(cnt0);
-        if (lane == 0 && cnt0) atomicAdd(gh, cnt0);
         __syncthreads();
-        // merge the CTA-private histogram into the transform's global histogram and re-zero it
-        for (int w = threadIdx.x; w < words; w += blockDim.x) {
-            const uint32_t v = sh_hist[w];
-            if (v) {
-                sh_hist[w] = 0u;
-                if (PACK16) {
-                    if (v & 0xFFFFu) atomicAdd(&gh[2 * w], v & 0xFFFFu);
-                    if (v >> 16) atomicAdd(&gh[2 * w + 1], v >> 16);
-                } else {
-                    atomicAdd(&gh[w], v);
+        // merge the CTA-private rows into the transform's global histogram (un-ranking the fixed
+        // bin) and re-zero them for the next item
+        for (int r = warp; r < rows_smem; r += nwarps) {
+            uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
+            for (int b = lane; b < nb; b += 32) {
+                const uint32_t v = sh_hist[r * nb + b];
+                if (v) {
+                    sh_hist[r * nb + b] = 0u;
+                    atomicAdd(&grow[b], v);
                 }
             }
         }
@@ -236,13 +333,10 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     }
 }
 
-template <int INTERP, bool PACK16, int UNROLL>
-static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, size_t smem_optin,
-                                     cudaStream_t s) {
-    const size_t nbins2 = (size_t)a.nb * a.nb;
-    const size_t smem = (PACK16 ? (nbins2 + 1) / 2 : nbins2) * sizeof(uint32_t);
-    if (smem > smem_optin) return cudaErrorInvalidConfiguration;
-    auto kern = resample_hist_kernel<INTERP, PACK16, UNROLL>;
+template <int INTERP, int UNROLL>
+static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStream_t s) {
+    const size_t smem = (size_t)a.rows_smem * a.nb * sizeof(uint32_t);
+    auto kern = resample_hist_kernel<INTERP, UNROLL>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long nitems = (long long)a.n_transforms * a.nslabs;
@@ -252,15 +346,17 @@ static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, size_t 
     return cudaGetLastError();
 }
 
-cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, size_t smem_optin,
-                                 cudaStream_t s) {
-    const bool pack16 = (size_t)a.nb * a.nb * sizeof(uint32_t) > 96 * 1024;
-    if (interp == MI_INTERP_NEAREST) {
-        return pack16 ? launch_resample_t<MI_INTERP_NEAREST, true, 4>(a, num_sms, smem_optin, s)
-                      : launch_resample_t<MI_INTERP_NEAREST, false, 4>(a, num_sms, smem_optin, s);
-    }
-    return pack16 ? launch_resample_t<MI_INTERP_TRILINEAR, true, 2>(a, num_sms, smem_optin, s)
-                  : launch_resample_t<MI_INTERP_TRILINEAR, false, 2>(a, num_sms, smem_optin, s);
+int hist_rows_in_smem(int nb, size_t smem_optin) {
+    const size_t reserve = 1024;  // static shared memory + alignment slack
+    size_t rows = (smem_optin > reserve ? smem_optin - reserve : 0) / ((size_t)nb * sizeof(uint32_t));
+    if (rows > (size_t)nb) rows = (size_t)nb;
+    return (int)rows;
+}
+
+cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s) {
+    if (a.rows_smem < 1) return cudaErrorInvalidConfiguration;
+    if (interp == MI_INTERP_NEAREST) return launch_resample_t<MI_INTERP_NEAREST, 4>(a, num_sms, s);
+    return launch_resample_t<MI_INTERP_TRILINEAR, 2>(a, num_sms, s);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -443,36 +539,31 @@ cudaError_t launch_map_assemble(const double* mi, int64_t n, int nch, double* ma
 }
 
 // ------------------------------------------------------------------------------------------------
-// Roofline probe: shared-memory atomicAdd rate on an nbins x nbins table
+// Roofline probe: shared-memory atomicAdd(u32) rate; result-less adds, four
+// independent updates per loop trip, index math kept to two instructions.
 // ------------------------------------------------------------------------------------------------
-template <bool PACK16>
 __global__ void __launch_bounds__(kHistThreads, 1)
-atomic_probe_kernel(int nbins2, int pattern, int iters, unsigned* __restrict__ sink) {
+atomic_probe_kernel(int words_log2, int pattern, int iters, unsigned* __restrict__ sink) {
     extern __shared__ __align__(16) uint32_t sh_tab[];
-    const int words = PACK16 ? (nbins2 + 1) / 2 : nbins2;
+    const int words = 1 << words_log2;
     for (int w = threadIdx.x; w < words; w += blockDim.x) sh_tab[w] = 0u;
     __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned mask = (unsigned)words - 1u;
     unsigned state = (blockIdx.x * 1024u + threadIdx.x) * 2654435761u + 12345u;
-    const unsigned mask_rows = (unsigned)(nbins2 / 32 > 0 ? nbins2 / 32 : 1);
-    for (int it = 0; it < iters; ++it) {
-        int idx;
-        if (pattern == 0) {
-            // lane-distinct banks: consecutive (packed: every other) bins of one 32-word row
-            const unsigned row = (warp * 7u + (unsigned)it * 13u) % (PACK16 ? mask_rows / 2 : mask_rows);
-            idx = PACK16 ? (int)(row * 64u + 2u * lane) : (int)(row * 32u + lane);
-        } else if (pattern == 1) {
-            state = state * 1664525u + 1013904223u;
-            idx = (int)(((unsigned long long)(state >> 8) * (unsigned)nbins2) >> 24);
-        } else {
-            idx = (int)(sink[0] & 1u) + 2;  // one address, not provably uniform at compile time
-        }
-        if (idx >= nbins2) idx = nbins2 - 1;
-        if (PACK16) {
-            const unsigned shift = (idx & 1) << 4;
-            const unsigned old = atomicAdd(&sh_tab[idx >> 1], 1u << shift);
-            if (((old >> shift) & 0xFFFFu) == 0x7FFFu) atomicSub(&sh_tab[idx >> 1], 0x8000u << shift);
-        } else {
+    const unsigned same = (sink[0] & 1u) + 2u;  // one address, not provably uniform at compile time
+    for (int it = 0; it < iters; it += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            unsigned idx;
+            if (pattern == 0) {
+                idx = (((warp * 37u + (unsigned)(it + u) * 11u) << 5) + lane) & mask;  // lane-distinct banks
+            } else if (pattern == 1) {
+                state = state * 1664525u + 1013904223u;
+                idx = (state >> 10) & mask;                                            // uniform random bins
+            } else {
+                idx = same;
+            }
             atomicAdd(&sh_tab[idx], 1u);
         }
     }
@@ -484,10 +575,12 @@ atomic_probe_kernel(int nbins2, int pattern, int iters, unsigned* __restrict__ s
 
 cudaError_t run_shared_atomic_probe(int nbins, int pattern, int iters, int num_sms, size_t smem_optin,
                                     double* updates_per_s) {
-    const int nbins2 = nbins * nbins;
-    const bool pack16 = (size_t)nbins2 * sizeof(uint32_t) > 96 * 1024;
-    const size_t smem = (pack16 ? (size_t)(nbins2 + 1) / 2 : (size_t)nbins2) * sizeof(uint32_t);
-    if (smem > smem_optin) return cudaErrorInvalidConfiguration;
+    // largest power-of-two table of u32 counters that is <= nbins^2 and fits in shared memory
+    int words_log2 = 5;
+    while ((1 << (words_log2 + 1)) <= nbins * nbins && ((size_t)4 << (words_log2 + 1)) <= smem_optin - 1024)
+        ++words_log2;
+    const size_t smem = (size_t)4 << words_log2;
+    iters = (iters + 3) & ~3;
     unsigned* sink = nullptr;
     cudaError_t e = cudaMalloc(&sink, 2 * sizeof(unsigned));
     if (e != cudaSuccess) return e;
@@ -496,21 +589,16 @@ cudaError_t run_shared_atomic_probe(int nbins, int pattern, int iters, int num_s
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
     float best_ms = 1e30f;
-    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {
+    cudaFuncSetAttribute(atomic_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    for (int rep = 0; rep < 6 && e == cudaSuccess; ++rep) {
         cudaEventRecord(e0, 0);
-        if (pack16) {
-            cudaFuncSetAttribute(atomic_probe_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            atomic_probe_kernel<true><<<num_sms, kHistThreads, smem, 0>>>(nbins2, pattern, iters, sink);
-        } else {
-            cudaFuncSetAttribute(atomic_probe_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            atomic_probe_kernel<false><<<num_sms, kHistThreads, smem, 0>>>(nbins2, pattern, iters, sink);
-        }
+        atomic_probe_kernel<<<num_sms, kHistThreads, smem, 0>>>(words_log2, pattern, iters, sink);
         cudaEventRecord(e1, 0);
         e = cudaEventSynchronize(e1);
         if (e == cudaSuccess) e = cudaGetLastError();
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
-        if (rep > 0 && ms < best_ms) best_ms = ms;
+        if (rep > 1 && ms < best_ms) best_ms = ms;
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
