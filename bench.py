@@ -312,7 +312,7 @@ def main():
     t_atom = evals_step / r_rand
     sm_hz = (clocks["sm_mhz"] or sm_max_mhz) * 1e6
     t_lsu = 32.0 * evals_step / (148 * 128.0 * sm_hz)
-    roofline = {"bound": "alu", "kernel": "resample_hist_kernel<TRILINEAR>",
+    roofline = {"bound": "alu", "kernel": "zhist_kernel<TRILINEAR> (separable path: x-pass, y-pass, z-lerp+histogram)",
                 "achieved": achieved / 1e9, "peak": r_rand / 1e9, "unit": "G shared-atomic updates/s",
                 "frac": achieved / r_rand, "traffic": None,
                 "peak_source": "mi_probe_shared_atomic_rate(pattern=uniform random bins) measured in this run",

@@ -5,6 +5,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -27,7 +28,21 @@ struct mi_ctx {
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
     int rows_smem = 0;
+    // separable path (diagonal-matrix families)
+    uint8_t* d_fb_pitched = nullptr;    // ranked fixed bins, [fnz][colpitch]
+    int colpitch = 0;                   // fny*fnx rounded up to a multiple of 4
+    int zrows_smem = 0;                 // shared-memory histogram rows of the z kernel (dump row included)
+    int zrows_real = 0;                 // fixed ranks counted in shared memory; ranks >= this are "rare"
+    uint2* d_rare = nullptr;            // rare voxels (col, iz | rank << 16)
+    unsigned n_rare = 0;
+    void* d_X = nullptr;        size_t cap_X = 0;      // bytes
+    void* d_XY = nullptr;       size_t cap_XY = 0;     // bytes
+    uint8_t* d_colvalid = nullptr; size_t cap_cv = 0;
+    float2* d_axis = nullptr;   size_t cap_axis = 0;   // 3 axes x nmax (scale, offset)
+    size_t xy_budget = (size_t)12 << 30;               // bytes of xy-plane scratch per batch
+    size_t sep_hist_budget = (size_t)3 << 30;          // bytes of histogram scratch per batch
     int tsallis_form = MI_TSALLIS_ADDITIVE;
+    bool use_separable = true;
     int num_sms = 148;
     size_t smem_optin = 48 * 1024;
     size_t hist_budget = (size_t)1 << 30;  // bytes of global histogram scratch per chunk
@@ -138,12 +153,145 @@ mi_status validate_q(mi_ctx* c, const double* q, int32_t nq) {
     return MI_OK;
 }
 
+// A map whose index-space matrices are all diagonal with per-axis parameters: transform
+// (k0,k1,k2) has c_x = fma(ax[k0].x, ix, ax[k0].y) and likewise for y (k1) and z (k2).
+struct SeparablePlan {
+    int n[3];
+    std::vector<float2> axis[3];
+};
+
+// Decide whether the grid of index-space matrices hM (p0 fastest) is separable and extract the
+// per-axis (scale, offset) tables.  Every transform is checked bit for bit against the tables.
+bool make_separable_plan(const std::vector<float>& hM, const int32_t n[3], SeparablePlan* plan) {
+    const int64_t N = (int64_t)n[0] * n[1] * n[2];
+    const int diag[3] = {0, 5, 10}, off[3] = {3, 7, 11};
+    for (int d = 0; d < 3; ++d) {
+        plan->n[d] = n[d];
+        plan->axis[d].resize(n[d]);
+    }
+    auto at = [&](int k0, int k1, int k2) { return hM.data() + (((int64_t)k2 * n[1] + k1) * n[0] + k0) * 12; };
+    for (int k = 0; k < n[0]; ++k) plan->axis[0][k] = make_float2(at(k, 0, 0)[diag[0]], at(k, 0, 0)[off[0]]);
+    for (int k = 0; k < n[1]; ++k) plan->axis[1][k] = make_float2(at(0, k, 0)[diag[1]], at(0, k, 0)[off[1]]);
+    for (int k = 0; k < n[2]; ++k) plan->axis[2][k] = make_float2(at(0, 0, k)[diag[2]], at(0, 0, k)[off[2]]);
+    // the z kernel walks the moving planes upwards: c_z must not decrease with iz
+    for (int k = 0; k < n[2]; ++k)
+        if (!(plan->axis[2][k].x >= 0.0f)) return false;
+    for (int64_t t = 0; t < N; ++t) {
+        const float* M = hM.data() + t * 12;
+        const int k[3] = {(int)(t % n[0]), (int)((t / n[0]) % n[1]), (int)(t / ((int64_t)n[0] * n[1]))};
+        if (M[1] != 0.f || M[2] != 0.f || M[4] != 0.f || M[6] != 0.f || M[8] != 0.f || M[9] != 0.f) return false;
+        for (int d = 0; d < 3; ++d) {
+            const float2 e = plan->axis[d][k[d]];
+            if (std::memcmp(&e.x, &M[diag[d]], 4) != 0 || std::memcmp(&e.y, &M[off[d]], 4) != 0) return false;
+        }
+    }
+    return true;
+}
+
+// Steps a3 + a4 of a separable map: for groups of p0 values run the x-pass, the y-pass for every
+// (p0,p1) pair of the group, then one z-lerp + histogram item per transform, then the entropy
+// kernel (a5) writing straight into map order.  Results land in c->d_mi / c->d_nvalid.
+mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int interp, EventTimer& timer) {
+    cudaStream_t s = c->stream;
+    const bool nn = interp == MI_INTERP_NEAREST;
+    const int n0 = sp.n[0], n1 = sp.n[1], n2 = sp.n[2];
+    const int nch = 1 + nq;
+    const size_t nbins2 = (size_t)c->nb * c->nb;
+    const int fnx = c->fd[0], cols = c->fd[0] * c->fd[1], fnz = c->fd[2];
+    const int planes = nn ? c->md[2] : c->md[2] + 2;
+    const int prows = nn ? c->md[1] : c->md[1] + 2;
+    const size_t elem = nn ? 1 : sizeof(float);
+    const size_t x_bytes_per_a = (size_t)planes * prows * fnx * elem;
+    const size_t xy_bytes_per_pair = (size_t)planes * c->colpitch * elem;
+    const size_t hist_bytes_per_pair = (size_t)n2 * nbins2 * sizeof(uint32_t);
+
+    // p0 values per batch: as many as the scratch budgets allow, chosen to minimise idle SM-waves
+    size_t max_pairs = c->xy_budget / xy_bytes_per_pair;
+    if (c->sep_hist_budget / hist_bytes_per_pair < max_pairs) max_pairs = c->sep_hist_budget / hist_bytes_per_pair;
+    if (max_pairs > 65535) max_pairs = 65535;  // gridDim.z of the y-pass
+    int ga_max = (int)(max_pairs / (size_t)n1);
+    if (ga_max > n0) ga_max = n0;
+    if (ga_max < 1) return fail(c, MI_ERR_OUT_OF_MEMORY, "separable map: one p0 slab exceeds the scratch budget");
+    int ga = 1;
+    long long best_waves = -1;
+    for (int g = 1; g <= ga_max; ++g) {
+        const long long per = ((long long)g * n1 * n2 + c->num_sms - 1) / c->num_sms;
+        const int rem = n0 % g;
+        long long waves = (long long)(n0 / g) * per;
+        if (rem) waves += ((long long)rem * n1 * n2 + c->num_sms - 1) / c->num_sms;
+        if (best_waves < 0 || waves <= best_waves) { best_waves = waves; ga = g; }
+    }
+
+    mi_status st;
+    const int nmax = n0 > n1 ? (n0 > n2 ? n0 : n2) : (n1 > n2 ? n1 : n2);
+    if ((st = grow(c, &c->d_axis, &c->cap_axis, (size_t)3 * nmax)) != MI_OK) return st;
+    if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_X), &c->cap_X, (size_t)ga * x_bytes_per_a)) != MI_OK) return st;
+    if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_XY), &c->cap_XY, (size_t)ga * n1 * xy_bytes_per_pair)) != MI_OK) return st;
+    if ((st = grow(c, &c->d_colvalid, &c->cap_cv, (size_t)ga * n1 * c->colpitch)) != MI_OK) return st;
+    if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist, (size_t)ga * n1 * hist_bytes_per_pair)) != MI_OK) return st;
+    for (int d = 0; d < 3; ++d)
+        MI_CUDA(c, cudaMemcpyAsync(c->d_axis + (size_t)d * nmax, sp.axis[d].data(), sp.axis[d].size() * sizeof(float2),
+                                   cudaMemcpyHostToDevice, s));
+    const float2* ax = c->d_axis;
+    const float2* ay = c->d_axis + nmax;
+    const float2* az = c->d_axis + 2 * (size_t)nmax;
+
+    for (int a0 = 0; a0 < n0; a0 += ga) {
+        const int na = (n0 - a0 < ga) ? (n0 - a0) : ga;
+        const int npairs = na * n1;
+        const long long items = (long long)npairs * n2;
+        timer.begin(1);
+        if (nn)
+            MI_CUDA(c, mi::launch_xpass(true, c->d_mbins, c->md[0], c->md[2] * c->md[1], c->md[0], ax, a0, na, fnx, c->d_X, s));
+        else
+            MI_CUDA(c, mi::launch_xpass(false, c->d_moving_pad, c->md[0] + 2, planes * prows, c->md[0], ax, a0, na, fnx, c->d_X, s));
+        MI_CUDA(c, mi::launch_ypass(nn, c->d_X, planes, prows, c->md[0], c->md[1], ax, ay, a0, n1, npairs, fnx, cols,
+                                    c->colpitch, c->d_XY, c->d_colvalid, s));
+        MI_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)items * nbins2 * sizeof(uint32_t), s));
+        mi::ZHistArgs z;
+        z.xy = c->d_XY;
+        z.colvalid = c->d_colvalid;
+        z.fb = c->d_fb_pitched;
+        z.rank_inv = c->d_rank_inv;
+        z.az = az;
+        z.hist = c->d_hist;
+        z.fnz = fnz;
+        z.colpitch = c->colpitch;
+        z.planes = planes;
+        z.mnz = c->md[2];
+        z.nb = c->nb;
+        z.rows_smem = c->zrows_smem;
+        z.rows_real = c->zrows_real;
+        z.rare = c->d_rare;
+        z.n_rare = c->n_rare;
+        z.mlo = c->mlo;
+        z.mscale = c->mscale;
+        z.n_pairs = npairs;
+        z.n2 = n2;
+        MI_CUDA(c, mi::launch_zhist(nn, z, c->num_sms, s));
+        c->last_launches[1] += 3;
+        timer.end();
+
+        timer.begin(2);
+        int q_off = 0;
+        do {
+            MI_CUDA(c, mi::launch_entropy(c->d_hist, c->nb, (int)items, c->d_q, nq, q_off, c->tsallis_form, c->d_mi,
+                                          c->d_nvalid, mi::OutMap{1, n0, n1, n2, a0}, s));
+            c->last_launches[2] += 1;
+            q_off += mi::kMaxQPerPass;
+        } while (q_off < nq);
+        timer.end();
+    }
+    (void)nch;
+    return MI_OK;
+}
+
 // The shared core of mi_eval_batch and mi_map.  hM: N x 12 index-space fp32 transforms in host
 // memory.  If map_out != NULL the result is assembled channel-major (step a6) instead of being
-// returned transform-major.
+// returned transform-major.  If sep != NULL the histograms are built by the separable path.
 mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const double* q, int32_t nq,
                     int interp, double* mi_out, uint32_t* hist_out, int64_t* nvalid_out,
-                    double* map_out, int64_t* argmax_out) {
+                    double* map_out, int64_t* argmax_out, const SeparablePlan* sep = nullptr) {
     const int nch = 1 + nq;
     const size_t nbins2 = (size_t)c->nb * c->nb;
     cudaStream_t s = c->stream;
@@ -175,14 +323,18 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * sizeof(uint32_t)));
     if (chunk < 1) chunk = 1;
     if (chunk > N) chunk = N;
-    if (!hist_to_user_dev) {
+    if (!hist_to_user_dev && sep == nullptr) {
         if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist,
                        (size_t)chunk * nbins2 * sizeof(uint32_t))) != MI_OK)
             return st;
     }
     const int rows_total = c->fd[1] * c->fd[2];
 
-    for (int64_t off = 0; off < N; off += chunk) {
+    if (sep != nullptr) {
+        st = run_separable(c, *sep, nq, interp, timer);
+        if (st != MI_OK) return st;
+    }
+    for (int64_t off = 0; sep == nullptr && off < N; off += chunk) {
         const int64_t cnt = (N - off < chunk) ? (N - off) : chunk;
         uint32_t* hist = hist_to_user_dev ? hist_out + (size_t)off * nbins2 : c->d_hist;
 
@@ -220,7 +372,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         int q_off = 0;
         do {
             MI_CUDA(c, mi::launch_entropy(hist, c->nb, (int)cnt, c->d_q, nq, q_off, c->tsallis_form,
-                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, s));
+                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, mi::OutMap{0, 0, 0, 0, 0}, s));
             c->last_launches[2] += 1;
             q_off += mi::kMaxQPerPass;
         } while (q_off < nq);
@@ -370,7 +522,15 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = cudaMalloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
         if ((e = cudaMalloc((void**)&d_mov, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
         if ((e = cudaMalloc((void**)&d_tmp, (size_t)nf * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
+        c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + 3) & ~3LL);
+        if ((e = cudaMalloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
+        c->zrows_smem = mi::zhist_rows_in_smem(nbins, fixed_dims[2], moving_dims[2] + 2, c->smem_optin);
         c->rows_smem = mi::hist_rows_in_smem(nbins, c->smem_optin);
+        // test knobs (tests/ shrink the scratch budgets to force several batches, or disable the path)
+        if (const char* v = std::getenv("MI_B200_SEPARABLE")) c->use_separable = std::atoi(v) != 0;
+        if (const char* v = std::getenv("MI_B200_XY_BUDGET_MB")) c->xy_budget = (size_t)std::atoll(v) << 20;
+        if (const char* v = std::getenv("MI_B200_SEP_HIST_BUDGET_MB")) c->sep_hist_budget = (size_t)std::atoll(v) << 20;
+        if (const char* v = std::getenv("MI_B200_ZROWS")) { const int r = std::atoi(v); if (r >= 2 && r < c->zrows_smem) c->zrows_smem = r; }
         if (c->rows_smem < 1) { st = fail(nullptr, MI_ERR_UNSUPPORTED, "device has too little shared memory"); break; }
         if ((e = cudaEventCreateWithFlags(&c->ev_staging, cudaEventDisableTiming)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaEventCreate"); break; }
         cudaStream_t s = c->stream;
@@ -379,6 +539,24 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
         if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
         if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
+        {
+            // the separable path keeps ranks < zrows_real in shared memory; if not every bin fits, the
+            // last shared row becomes a dump row and the voxels of the rare ranks go to a list
+            unsigned long long h_counts[256];
+            uint8_t h_rank[256];
+            if ((e = cudaMemcpyAsync(h_counts, d_counts, sizeof(h_counts), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy counts"); break; }
+            if ((e = cudaMemcpyAsync(h_rank, c->d_rank, sizeof(h_rank), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy ranks"); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync ranks"); break; }
+            c->zrows_real = c->zrows_smem > nbins ? nbins : c->zrows_smem - 1;   // one row is the dump row
+            unsigned long long n_rare = 0;
+            for (int a = 0; a < 256; ++a)
+                if ((int)h_rank[a] >= c->zrows_real) n_rare += h_counts[a];
+            c->n_rare = (unsigned)n_rare;
+            if ((e = cudaMalloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
+            if ((e = cudaMemsetAsync(d_counts, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
+            if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
+                                           c->d_fb_pitched, c->d_rare, reinterpret_cast<unsigned*>(d_counts), c->n_rare, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pitch fixed bins"); break; }
+        }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
@@ -399,7 +577,8 @@ void mi_destroy(mi_ctx* c) {
     if (guard.ok) {
         cudaStreamSynchronize(c->stream);
         cudaFree(c->d_fbins); cudaFree(c->d_fbins_ranked); cudaFree(c->d_rank); cudaFree(c->d_rank_inv);
-        cudaFree(c->d_moving_pad); cudaFree(c->d_mbins);
+        cudaFree(c->d_moving_pad); cudaFree(c->d_mbins); cudaFree(c->d_fb_pitched); cudaFree(c->d_rare);
+        cudaFree(c->d_X); cudaFree(c->d_XY); cudaFree(c->d_colvalid); cudaFree(c->d_axis);
         cudaFree(c->d_M); cudaFree(c->d_hist); cudaFree(c->d_mi); cudaFree(c->d_nvalid);
         cudaFree(c->d_q); cudaFree(c->d_map); cudaFree(c->d_argmax);
         if (c->h_M) cudaFreeHost(c->h_M);
@@ -483,7 +662,12 @@ mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double h
             }
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
-    return eval_core(c, hM, N, q, nq, (int)interp, nullptr, nullptr, nullptr, map_out, argmax_out);
+    // translation / scale maps have diagonal matrices: separable fast path (same arithmetic)
+    SeparablePlan plan;
+    const bool diag_family = family == MI_FAMILY_TRANSLATION || family == MI_FAMILY_SCALE || family == MI_FAMILY_SCALE_LOG;
+    const bool sep = diag_family && c->use_separable && c->zrows_smem >= 2 && c->fd[2] <= 65535 && make_separable_plan(hM, n, &plan);
+    return eval_core(c, hM, N, q, nq, (int)interp, nullptr, nullptr, nullptr, map_out, argmax_out,
+                     sep ? &plan : nullptr);
 }
 
 mi_status mi_get_bins(mi_ctx* c, int32_t which, uint8_t* out) {

@@ -45,9 +45,42 @@ cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long
                                    uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s);
 int hist_rows_in_smem(int nb, size_t smem_optin);
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s);
+// Where the entropy kernel writes the result of histogram `item`: transform-major position item
+// (enabled == 0) or, for the separable path whose items are ordered (p0, p1, p2) with p2 fastest,
+// the map's transform index (p2*n1 + p1)*n0 + p0.
+struct OutMap {
+    int enabled;
+    int n0, n1, n2, a0;
+};
 cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const double* q_dev, int nq,
                            int q_off, int form, double* mi_out /* n x (1+nq) */, int64_t* nvalid,
-                           cudaStream_t s);
+                           OutMap om, cudaStream_t s);
+
+// ---- separable path (mi_separable.cu) ----------------------------------------------------------
+struct ZHistArgs {
+    const void* xy;            // [n_pairs][planes][colpitch] float (trilinear) or uint8 (nearest)
+    const uint8_t* colvalid;   // [n_pairs][colpitch]: column (iy,ix) is inside the moving volume in x and y
+    const uint8_t* fb;         // ranked fixed bins, [fnz][colpitch]
+    const int* rank_inv;
+    const float2* az;          // n2 z-axis (scale, offset) pairs
+    uint32_t* hist;            // [n_pairs*n2][nb][nb], zero on entry
+    int fnz, colpitch, planes, mnz;
+    int nb, rows_smem;         // rows_smem: histogram rows in shared memory, dump row included
+    int rows_real;             // ranks below rows_real are counted in shared memory; the rest are "rare"
+    float mlo, mscale;
+    int n_pairs, n2;
+    const uint2* rare;         // rare voxels: (col, iz | rank << 16)
+    unsigned n_rare;
+};
+cudaError_t launch_pitch_bins(const uint8_t* in, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
+                              uint2* rare, unsigned* rare_count, unsigned rare_cap, cudaStream_t s);
+cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, const float2* ax, int a0,
+                         int na, int fnx, void* X, cudaStream_t s);
+cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
+                         const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
+                         void* XY, uint8_t* colvalid, cudaStream_t s);
+int zhist_rows_in_smem(int nb, int fnz, int planes, size_t smem_optin);
+cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t s);
 cudaError_t launch_map_assemble(const double* mi /* n x nch */, int64_t n, int nch, double* map_out,
                                 int64_t* argmax_out, cudaStream_t s);
 cudaError_t run_shared_atomic_probe(int nbins, int pattern, int iters, int num_sms, size_t smem_optin,

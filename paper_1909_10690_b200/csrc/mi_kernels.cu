@@ -374,7 +374,7 @@ __device__ __forceinline__ double warp_sum_d(double v) {
 __global__ void __launch_bounds__(kEntropyThreads)
 entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restrict__ q, int nq_total,
                int q_off, int nq_pass, int form, double* __restrict__ mi_out,
-               int64_t* __restrict__ nvalid) {
+               int64_t* __restrict__ nvalid, const OutMap om) {
     constexpr int NW = kEntropyThreads / 32;
     constexpr int NACC = 3 * (1 + kMaxQPerPass);
     __shared__ unsigned sh_pa[256], sh_pb[256];
@@ -458,8 +458,14 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
         }
         unsigned long long n = 0;
         for (int w = 0; w < NW; ++w) n += sh_n[w];
-        double* out = mi_out + (size_t)t * (1 + nq_total);
-        if (nvalid != nullptr) nvalid[t] = (int64_t)n;
+        size_t dst = (size_t)t;
+        if (om.enabled) {  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
+            const int c = t % om.n2, ab = t / om.n2;
+            const int b = ab % om.n1, al = ab / om.n1;
+            dst = ((size_t)c * om.n1 + b) * om.n0 + (size_t)(om.a0 + al);
+        }
+        double* out = mi_out + dst * (1 + nq_total);
+        if (nvalid != nullptr) nvalid[dst] = (int64_t)n;
         if (n == 0) {
             out[0] = 0.0;
             for (int k = 0; k < nq_pass; ++k) out[1 + q_off + k] = 0.0;
@@ -488,13 +494,13 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
 }
 
 cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const double* q_dev, int nq,
-                           int q_off, int form, double* mi_out, int64_t* nvalid, cudaStream_t s) {
+                           int q_off, int form, double* mi_out, int64_t* nvalid, OutMap om, cudaStream_t s) {
     if (n_transforms <= 0) return cudaSuccess;
     int nq_pass = nq - q_off;
     if (nq_pass > kMaxQPerPass) nq_pass = kMaxQPerPass;
     if (nq_pass < 0) nq_pass = 0;
     entropy_kernel<<<n_transforms, kEntropyThreads, 0, s>>>(hist, nb, q_dev, nq, q_off, nq_pass, form,
-                                                           mi_out, nvalid);
+                                                           mi_out, nvalid, om);
     return cudaGetLastError();
 }
 

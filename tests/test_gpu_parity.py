@@ -266,3 +266,79 @@ def test_c5_full_size_sampled_against_oracle(mi):
             else:
                 assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
             assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
+
+
+# ------------------------------------------------------------------------------------------------ separable path
+class env:
+    """Set MI_B200_* knobs (read by mi_create) for the duration of a with-block."""
+    def __init__(self, **kw):
+        self.kw = {k: str(v) for k, v in kw.items()}
+
+    def __enter__(self):
+        import os
+        self.old = {k: os.environ.get(k) for k in self.kw}
+        os.environ.update(self.kw)
+
+    def __exit__(self, *exc):
+        import os
+        for k, v in self.old.items():
+            if v is None:
+                os.environ.pop(k, None)
+            else:
+                os.environ[k] = v
+
+
+def gpu_map(mi, cfg, interp, **knobs):
+    with env(**knobs):
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins, cfg.ranges) as ctx:
+            return mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, interp)
+
+
+@pytest.mark.parametrize("name,kw", [("C1", {}), ("C5", dict(res=0.25, grid_n=5)), ("C4", dict(res=0.25, grid_n=4)),
+                                     ("C2", dict(size=48, grid_n=5, half_range=2.5))])
+def test_separable_path_equals_generic_path_bitwise(mi, name, kw):
+    """Translation / scale maps run through the separable x-, y-, z-pass kernels; the same map through
+    the generic kernel (whose histograms are checked bit for bit against the oracle above) must give
+    IDENTICAL doubles: the entropy kernel is deterministic, so equal maps <=> equal histograms."""
+    cfg = ph.get_config(name, **kw)
+    for interp in (0, 1):
+        ms, ams = gpu_map(mi, cfg, interp)
+        mg, amg = gpu_map(mi, cfg, interp, MI_B200_SEPARABLE=0)
+        assert np.array_equal(ms, mg), np.max(np.abs(ms - mg))
+        assert np.array_equal(ams, amg)
+
+
+def test_separable_batches_rare_rows_and_odd_grids(mi):
+    cfg = ph.get_config("C5", res=0.25, grid_n=5)
+    ref, _ = gpu_map(mi, cfg, 1, MI_B200_SEPARABLE=0)
+    # tiny scratch budgets: one p0 per batch, several batches
+    m, _ = gpu_map(mi, cfg, 1, MI_B200_XY_BUDGET_MB=8, MI_B200_SEP_HIST_BUDGET_MB=8)
+    assert np.array_equal(m, ref)
+    # only 40 of 256 fixed-bin rows in shared memory: most voxels go through the rare-voxel kernel
+    for interp in (0, 1):
+        ref, _ = gpu_map(mi, cfg, interp, MI_B200_SEPARABLE=0)
+        m, _ = gpu_map(mi, cfg, interp, MI_B200_ZROWS=40)
+        assert np.array_equal(m, ref)
+    # random volumes fill all 256 bins: the rare tail exists at the natural row count too; ragged
+    # non-cubic grid (n = 3 x 1 x 4), anisotropic spacing
+    fixed = ph.random_volume((37, 21, 13), 21)
+    moving = ph.random_volume((30, 25, 17), 22)
+    c = ph.Config("rnd", fixed, moving, (1.0, 1.2, 0.9), (1.1, 1.0, 1.3), 256, 0, (-3, 1, -2), (3, 1, 2), (3, 1, 4),
+                  (0.5,), (0, 0, 0))
+    for interp in (0, 1):
+        check_map(mi, c, interp)
+        ms, _ = gpu_map(mi, c, interp)
+        mg, _ = gpu_map(mi, c, interp, MI_B200_SEPARABLE=0)
+        assert np.array_equal(ms, mg)
+
+
+def test_scale_maps_with_plane_skips_and_negative_factors(mi):
+    """Scale factors > 1 in z skip moving planes between consecutive fixed slices; a factor of 0 maps
+    every slice to one plane; negative z factors fall back to the generic kernel."""
+    cfg = ph.get_config("C4", res=0.25, grid_n=4)
+    for lo, hi, n in [((0.6, 0.6, 0.6), (2.6, 2.6, 2.6), (3, 3, 5)), ((1.0, 1.0, 0.0), (1.0, 1.0, 0.0), (1, 1, 1)),
+                      ((0.9, 0.9, -1.2), (1.1, 1.1, 1.2), (2, 2, 3))]:
+        c = ph.Config("C4s", cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256, 3, lo, hi, n,
+                      (2.0,), cfg.truth)
+        for interp in (0, 1):
+            check_map(mi, c, interp)
