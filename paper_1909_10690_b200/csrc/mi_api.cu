@@ -30,7 +30,10 @@ struct mi_ctx {
     int rows_smem = 0;
     // separable path (diagonal-matrix families)
     uint8_t* d_fb_pitched = nullptr;    // ranked fixed bins, [fnz][colpitch]
-    int colpitch = 0;                   // fny*fnx rounded up to a multiple of 4
+    int colpitch = 0;                   // fny*fnx rounded up to a multiple of 8
+    int zpitch = 0;                     // words per shared histogram row of the z kernel
+    int zcols = 8;                      // adjacent columns per thread of the z kernel (4 or 8)
+    bool fast_bin = false;              // moving_lo == 0 and every moving voxel is finite and >= 0
     int zrows_smem = 0;                 // shared-memory histogram rows of the z kernel (dump row included)
     int zrows_real = 0;                 // fixed ranks counted in shared memory; ranks >= this are "rare"
     uint2* d_rare = nullptr;            // rare voxels (col, iz | rank << 16)
@@ -247,7 +250,6 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
             MI_CUDA(c, mi::launch_xpass(false, c->d_moving_pad, c->md[0] + 2, planes * prows, c->md[0], ax, a0, na, fnx, c->d_X, s));
         MI_CUDA(c, mi::launch_ypass(nn, c->d_X, planes, prows, c->md[0], c->md[1], ax, ay, a0, n1, npairs, fnx, cols,
                                     c->colpitch, c->d_XY, c->d_colvalid, s));
-        MI_CUDA(c, cudaMemsetAsync(c->d_hist, 0, (size_t)items * nbins2 * sizeof(uint32_t), s));
         mi::ZHistArgs z;
         z.xy = c->d_XY;
         z.colvalid = c->d_colvalid;
@@ -261,6 +263,9 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
         z.mnz = c->md[2];
         z.nb = c->nb;
         z.rows_smem = c->zrows_smem;
+        z.pitch = c->zpitch;
+        z.cols = c->zcols;
+        z.fast_bin = c->fast_bin ? 1 : 0;
         z.rows_real = c->zrows_real;
         z.rare = c->d_rare;
         z.n_rare = c->n_rare;
@@ -522,9 +527,14 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = cudaMalloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
         if ((e = cudaMalloc((void**)&d_mov, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
         if ((e = cudaMalloc((void**)&d_tmp, (size_t)nf * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
-        c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + 3) & ~3LL);
+        c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + 7) & ~7LL);
         if ((e = cudaMalloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
-        c->zrows_smem = mi::zhist_rows_in_smem(nbins, fixed_dims[2], moving_dims[2] + 2, c->smem_optin);
+        // bank of histogram word (a, b) = (a*pad + b) mod 32: an odd pad walks the rows over all banks
+        int zpad = 9;
+        if (const char* v = std::getenv("MI_B200_HIST_PAD")) { const int r = std::atoi(v); if (r >= 0 && r <= 64) zpad = r; }
+        if (const char* v = std::getenv("MI_B200_ZCOLS")) { const int r = std::atoi(v); if (r == 4 || r == 8) c->zcols = r; }
+        c->zpitch = nbins + zpad;
+        c->zrows_smem = mi::zhist_rows_in_smem(nbins, c->zpitch, fixed_dims[2], moving_dims[2] + 2, c->smem_optin);
         c->rows_smem = mi::hist_rows_in_smem(nbins, c->smem_optin);
         // test knobs (tests/ shrink the scratch budgets to force several batches, or disable the path)
         if (const char* v = std::getenv("MI_B200_SEPARABLE")) c->use_separable = std::atoi(v) != 0;
@@ -536,8 +546,16 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         cudaStream_t s = c->stream;
         if ((e = cudaMemcpyAsync(d_tmp, fixed, (size_t)nf * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy fixed"); break; }
         if ((e = cudaMemcpyAsync(d_mov, moving, (size_t)nm * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy moving"); break; }
-        if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
-        if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
+        if ((e = cudaMemsetAsync(d_counts, 0, 256 * sizeof(unsigned long long), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
+        if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, nullptr, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
+        if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, reinterpret_cast<unsigned*>(d_counts), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
+        {
+            unsigned h_flag = 1;
+            if ((e = cudaMemcpyAsync(&h_flag, d_counts, sizeof(unsigned), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy flag"); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync flag"); break; }
+            c->fast_bin = h_flag == 0 && c->mlo == 0.0f;
+            if (const char* v = std::getenv("MI_B200_FAST_BIN")) { if (std::atoi(v) == 0) c->fast_bin = false; }
+        }
         if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
         {
             // the separable path keeps ranks < zrows_real in shared memory; if not every bin fits, the

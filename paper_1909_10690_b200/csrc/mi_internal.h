@@ -38,8 +38,9 @@ struct ResampleArgs {
     int nslabs;              // CTAs cooperating on one transform (row slabs)
 };
 
+// flag (may be NULL): set to 1 if any voxel is negative or not finite
 cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, float scale, int nb,
-                          cudaStream_t s);
+                          unsigned* flag, cudaStream_t s);
 cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s);
 cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
                                    uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s);
@@ -66,6 +67,9 @@ struct ZHistArgs {
     uint32_t* hist;            // [n_pairs*n2][nb][nb], zero on entry
     int fnz, colpitch, planes, mnz;
     int nb, rows_smem;         // rows_smem: histogram rows in shared memory, dump row included
+    int pitch;                 // words per shared histogram row (>= nb; the pad spreads rows over banks)
+    int cols;                  // adjacent columns per thread: 4 or 8 (colpitch is a multiple of it)
+    int fast_bin;              // mlo == 0 and every moving voxel is finite and >= 0: t = v*mscale >= 0
     int rows_real;             // ranks below rows_real are counted in shared memory; the rest are "rare"
     float mlo, mscale;
     int n_pairs, n2;
@@ -79,7 +83,7 @@ cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, 
 cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
                          const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
                          void* XY, uint8_t* colvalid, cudaStream_t s);
-int zhist_rows_in_smem(int nb, int fnz, int planes, size_t smem_optin);
+int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin);
 cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t s);
 cudaError_t launch_map_assemble(const double* mi /* n x nch */, int64_t n, int nch, double* map_out,
                                 int64_t* argmax_out, cudaStream_t s);

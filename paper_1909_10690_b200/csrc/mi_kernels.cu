@@ -29,16 +29,24 @@ __device__ __forceinline__ int bin_index(float v, float lo, float scale, float t
 }
 
 // Each thread turns 16 consecutive floats (4 x 16-byte loads) into one 16-byte store.
+// `flag` (may be NULL) is set when a voxel is negative or not finite (the z-histogram kernel may
+// skip the lower clamp of CANON-5 when it stays 0 and lo == 0).
+__device__ __forceinline__ bool plain_nonneg(float v) { return v >= 0.0f && v <= 3.0e38f; }
+
 __global__ void __launch_bounds__(256) prebin_kernel(const float* __restrict__ vol,
                                                      uint8_t* __restrict__ bins, int64_t n, float lo,
-                                                     float scale, float top) {
+                                                     float scale, float top, unsigned* __restrict__ flag) {
     const int64_t nvec = n >> 4;
+    bool odd = false;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
         const float4* src = reinterpret_cast<const float4*>(vol) + i * 4;
         float4 v[4];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) v[k] = __ldcs(src + k);
+        for (int k = 0; k < 4; ++k) {
+            v[k] = __ldcs(src + k);
+            odd |= !(plain_nonneg(v[k].x) && plain_nonneg(v[k].y) && plain_nonneg(v[k].z) && plain_nonneg(v[k].w));
+        }
         uint32_t w[4];
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
@@ -52,17 +60,21 @@ __global__ void __launch_bounds__(256) prebin_kernel(const float* __restrict__ v
     // ragged tail (< 16 voxels), one thread each
     const int64_t tail0 = nvec << 4;
     const int64_t j = tail0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (j < n) bins[j] = (uint8_t)bin_index(vol[j], lo, scale, top);
+    if (j < n) {
+        bins[j] = (uint8_t)bin_index(vol[j], lo, scale, top);
+        odd |= !plain_nonneg(vol[j]);
+    }
+    if (flag != nullptr && __any_sync(0xffffffffu, odd) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
 }
 
 cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, float scale, int nb,
-                          cudaStream_t s) {
+                          unsigned* flag, cudaStream_t s) {
     if (n <= 0) return cudaSuccess;
     const int64_t nvec = n >> 4;
     int64_t blocks = (nvec + 255) / 256;
     if (blocks < 1) blocks = 1;
     if (blocks > 148 * 16) blocks = 148 * 16;
-    prebin_kernel<<<(unsigned)blocks, 256, 0, s>>>(vol, bins, n, lo, scale, (float)(nb - 1));
+    prebin_kernel<<<(unsigned)blocks, 256, 0, s>>>(vol, bins, n, lo, scale, (float)(nb - 1), flag);
     return cudaGetLastError();
 }
 

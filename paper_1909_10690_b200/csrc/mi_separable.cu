@@ -57,15 +57,15 @@ __device__ __forceinline__ AxisSample axis_sample(float c, int n) {
 }
 
 // ---- x-pass -------------------------------------------------------------------------------------
-// grid: (ceil(fnx/128), rows = planes*prows, na).  Trilinear: src = padded float volume, rows over
+// grid: (rows = planes*prows, ceil(fnx/128), na).  Trilinear: src = padded float volume, rows over
 // padded (z', y').  Nearest: src = moving bins, rows over (z, y).
 template <bool NN, typename VT>
 __global__ void __launch_bounds__(128) xpass_kernel(const VT* __restrict__ src, int snx, int mnx,
                                                     const float2* __restrict__ ax, int a0, int fnx,
                                                     VT* __restrict__ X) {
-    const int ix = blockIdx.x * 128 + threadIdx.x;
+    const int ix = blockIdx.y * 128 + threadIdx.x;
     if (ix >= fnx) return;
-    const int row = blockIdx.y;
+    const int row = blockIdx.x;          // up to 2^31-1 rows (gridDim.y/z stop at 65535)
     const int a = blockIdx.z;
     const float2 mo = ax[a0 + a];
     const AxisSample sx = axis_sample<NN>(__fmaf_rn(mo.x, (float)ix, mo.y), mnx);
@@ -75,97 +75,169 @@ __global__ void __launch_bounds__(128) xpass_kernel(const VT* __restrict__ src, 
         if (NN) out = r[sx.lower];
         else out = (VT)lerp_rn((float)r[sx.lower], (float)r[sx.lower + 1], sx.w);
     }
-    X[((size_t)a * gridDim.y + row) * fnx + ix] = out;
+    X[((size_t)a * gridDim.x + row) * fnx + ix] = out;
 }
 
 // ---- y-pass -------------------------------------------------------------------------------------
-// grid: (ceil(colpitch/256), planes, npairs).  pair = a_local*n1 + b.  Writes XY[pair][plane][col]
-// and (for plane 0) colvalid[pair][col].
+// grid: (ceil(colpitch/4 / 128), npairs).  pair = a_local*n1 + b.  Every thread owns 4 adjacent
+// columns of one pair, resolves their x/y samples once and then walks all planes (unrolled by 4 for
+// memory-level parallelism), writing XY[pair][plane][col..col+3] as one 16-byte store per plane, and
+// colvalid[pair][col..col+3].
 template <bool NN, typename VT>
-__global__ void __launch_bounds__(256) ypass_kernel(const VT* __restrict__ X, int prows, int mnx, int mny,
-                                                    const float2* __restrict__ ax, const float2* __restrict__ ay,
-                                                    int a0, int n1, int fnx, int cols, int colpitch,
-                                                    VT* __restrict__ XY, uint8_t* __restrict__ colvalid) {
-    const int col = blockIdx.x * 256 + threadIdx.x;
-    if (col >= colpitch) return;
-    const int plane = blockIdx.y, planes = gridDim.y;
-    const int pair = blockIdx.z;
+struct Quad;
+template <>
+struct Quad<false, float> {
+    float4 q;
+    __device__ __forceinline__ void set(int k, float v) { (&q.x)[k] = v; }
+    __device__ __forceinline__ void store(float* p) const { *reinterpret_cast<float4*>(p) = q; }
+};
+template <>
+struct Quad<true, uint8_t> {
+    uint32_t q = 0u;
+    __device__ __forceinline__ void set(int k, uint8_t v) { q |= (uint32_t)v << (8 * k); }
+    __device__ __forceinline__ void store(uint8_t* p) const { *reinterpret_cast<uint32_t*>(p) = q; }
+};
+
+template <bool NN, typename VT>
+__global__ void __launch_bounds__(128) ypass_kernel(const VT* __restrict__ X, int planes, int prows, int mnx,
+                                                    int mny, const float2* __restrict__ ax,
+                                                    const float2* __restrict__ ay, int a0, int n1, int fnx,
+                                                    int cols, int colpitch, VT* __restrict__ XY,
+                                                    uint8_t* __restrict__ colvalid) {
+    const int col0 = (blockIdx.x * 128 + threadIdx.x) * 4;
+    if (col0 >= colpitch) return;
+    const int pair = blockIdx.y;
     const int a = pair / n1, b = pair - a * n1;
-    const int iy = col / fnx, ix = col - iy * fnx;
-    VT out = VT(0);
-    bool ok = false;
-    if (col < cols) {
-        const float2 mx = ax[a0 + a], my = ay[b];
-        const AxisSample sx = axis_sample<NN>(__fmaf_rn(mx.x, (float)ix, mx.y), mnx);
-        const AxisSample sy = axis_sample<NN>(__fmaf_rn(my.x, (float)iy, my.y), mny);
-        ok = sx.ok && sy.ok;
-        if (ok) {
-            const VT* __restrict__ r = X + (((size_t)a * planes + plane) * prows + sy.lower) * fnx + ix;
-            if (NN) out = r[0];
-            else out = (VT)lerp_rn((float)r[0], (float)r[fnx], sy.w);
+    const float2 mx = ax[a0 + a], my = ay[b];
+    // per column: offset of X[a][plane 0][sy.lower][ix] (or -1 if the column is invalid) and the y weight
+    long long off[4];
+    float wy[4];
+    uint32_t cv = 0u;
+    int iy = col0 / fnx, ix = col0 - iy * fnx;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        off[k] = -1;
+        wy[k] = 0.0f;
+        if (col0 + k < cols) {
+            const AxisSample sx = axis_sample<NN>(__fmaf_rn(mx.x, (float)ix, mx.y), mnx);
+            const AxisSample sy = axis_sample<NN>(__fmaf_rn(my.x, (float)iy, my.y), mny);
+            if (sx.ok && sy.ok) {
+                off[k] = ((long long)a * planes * prows + sy.lower) * fnx + ix;
+                wy[k] = sy.w;
+                cv |= 1u << (8 * k);
+            }
         }
+        if (++ix == fnx) { ix = 0; ++iy; }
     }
-    XY[((size_t)pair * planes + plane) * colpitch + col] = out;
-    if (plane == 0) colvalid[(size_t)pair * colpitch + col] = ok ? 1 : 0;
+    *reinterpret_cast<uint32_t*>(colvalid + (size_t)pair * colpitch + col0) = cv;
+    const size_t pstride = (size_t)prows * fnx;
+    VT* __restrict__ out = XY + (size_t)pair * planes * colpitch + col0;
+#pragma unroll 4
+    for (int plane = 0; plane < planes; ++plane) {
+        Quad<NN, VT> q;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            VT v = VT(0);
+            if (off[k] >= 0) {
+                const VT* __restrict__ r = X + off[k] + plane * pstride;
+                if (NN) v = __ldg(r);
+                else v = (VT)lerp_rn((float)__ldg(r), (float)__ldg(r + fnx), wy[k]);
+            }
+            q.set(k, v);
+        }
+        q.store(out + (size_t)plane * colpitch);
+    }
 }
 
 // ---- z-lerp + joint histogram ---------------------------------------------------------------------
 __device__ __forceinline__ float4 ld4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 __device__ __forceinline__ uint32_t ld_u32(const uint8_t* p) { return __ldg(reinterpret_cast<const uint32_t*>(p)); }
 
-// Result-less shared-memory increment on a 32-bit shared address (SASS: ATOMS.POPC.INC / ATOMS.ADD).
+// Result-less shared-memory increment on a 32-bit shared address (SASS: ATOMS.POPC.INC, which
+// counts the lanes of a warp that hit the same address in one pass).
 __device__ __forceinline__ void red_shared_inc(unsigned addr) {
     asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
 }
 
-// CANON-5 on the integer side: PTX float->int conversions saturate to the destination range
-// (NaN -> 0), so cvt.rmi.u8 is clamp(floor(t), 0, 255) in one instruction; bins < 256 need one min.
-__device__ __forceinline__ unsigned bin_u8(float t, unsigned top) {
-    unsigned b;
-    asm("cvt.rmi.u8.f32 %0, %1;" : "=r"(b) : "f"(t));
-    return min(b, top);
-}
-
-// Words of shared memory in front of the histogram: ws[fnz] + run_lo[planes] + run_hi[planes],
-// rounded up to a multiple of 4 words.
+// Words of shared memory in front of the histogram: ws[fnz] + run_hi[planes], rounded up to a
+// multiple of 4 words.
 __host__ __device__ __forceinline__ int zhist_table_words(int fnz, int planes) {
-    return (fnz + 2 * planes + 3) & ~3;
+    return (fnz + planes + 3) & ~3;
 }
 
-// One CTA per (pair, p2) item at a time; every thread owns 4 adjacent columns (iy,ix) of the fixed
-// volume and walks them along z.  The walk is organised by moving plane: for lower plane p the fixed
-// slices iz with floor(c_z) = p form one contiguous run (c_z is non-decreasing in iz), during which
-// the two xy-lerped plane values stay in registers; the next plane is prefetched one step ahead and
-// the three float4 registers rotate by name (the plane loop is unrolled by 3), so a plane step costs
-// one 16-byte load and a pointer increment.
+template <int COLS>
+struct ColVec {                      // COLS adjacent columns of one plane / one fixed slice
+    float v[COLS];
+};
+template <int COLS>
+__device__ __forceinline__ void ld_cols(ColVec<COLS>& r, const float* p) {
+#pragma unroll
+    for (int j = 0; j < COLS / 4; ++j) {
+        const float4 q = ld4(p + 4 * j);
+        r.v[4 * j] = q.x; r.v[4 * j + 1] = q.y; r.v[4 * j + 2] = q.z; r.v[4 * j + 3] = q.w;
+    }
+}
+template <int COLS>
+struct BinVec {                      // COLS adjacent uint8 values
+    uint32_t w[COLS / 4];
+};
+template <int COLS>
+__device__ __forceinline__ void ld_bins(BinVec<COLS>& r, const uint8_t* p) {
+    if (COLS == 8) {
+        const uint2 q = __ldg(reinterpret_cast<const uint2*>(p));
+        r.w[0] = q.x; r.w[COLS / 4 - 1] = q.y;
+    } else {
+        r.w[0] = ld_u32(p);
+    }
+}
+__device__ __forceinline__ unsigned byte_of(uint32_t w, int k) { return __byte_perm(w, 0u, 0x4440u | (unsigned)k); }
+
+// One CTA per (pair, p2) item at a time; every thread owns COLS adjacent columns (iy,ix) of the
+// fixed volume and walks them along z.  The walk is organised by moving plane: for lower plane p the
+// fixed slices iz with floor(c_z) = p form one contiguous run (c_z is non-decreasing in iz), during
+// which the two xy-lerped plane values stay in registers; the next plane is prefetched one step
+// ahead and the three register sets rotate by name (the plane loop is unrolled by 3), so a plane step
+// costs one 16-byte load per 4 columns and a pointer increment.
 //
-// Shared memory: ws[fnz] z-weights | run_lo[planes], run_hi[planes] | histogram rows.
-template <bool NN>
+// Histogram update, trilinear (CANON-4 z-lerp, CANON-5 binning, one RED):
+//   v = fma(w, hi - lo, lo)              hi - lo is formed once per plane step
+//   t = (v - mlo) * mscale               FAST: mlo == 0 and every moving voxel >= 0, so v - 0 == v
+//   t = min(max(t, 0), nb - 1)           FAST: t >= 0 already; clamping before the floor == after it
+//   r = RD(t + (1.5*2^23 + a*pitch))     the low mantissa bits of r are a*pitch + floor(t) EXACTLY
+//                                        (ulp is 1 there and the second addend is an integer)
+//   RED [4*bits(r) + const]              const folds the shared base and -4*bits(1.5*2^23)
+// The shared histogram rows have a pitch of nb + pad words: bank = (a*pad + b) mod 32, so the rows
+// of the (many) background fixed bins do not all start on bank 0.
+//
+// Shared memory: ws[fnz] z-weights | run_hi[planes] | histogram rows (pitch words each).
+template <bool NN, int COLS, bool FAST>
 __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_constant__ ZHistArgs a) {
     extern __shared__ __align__(16) uint32_t sh_raw[];
     float* ws = reinterpret_cast<float*>(sh_raw);
-    int* run_lo = reinterpret_cast<int*>(sh_raw) + a.fnz;
-    int* run_hi = run_lo + a.planes;
+    int* run_hi = reinterpret_cast<int*>(sh_raw) + a.fnz;
     uint32_t* sh_hist = sh_raw + zhist_table_words(a.fnz, a.planes);
     __shared__ int s_lo, s_hi;
     const unsigned nb = (unsigned)a.nb;
+    const unsigned pitch = (unsigned)a.pitch;
     const int rows_smem = a.rows_smem;   // includes the dump row
-    const int words = rows_smem * a.nb;
+    const int words = rows_smem * a.pitch;
     for (int w = threadIdx.x; w < words; w += blockDim.x) sh_hist[w] = 0u;
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int colpitch = a.colpitch;
-    const unsigned top = (unsigned)(a.nb - 1);
-    const int ntiles = (colpitch + 4 * kHistThreads - 1) / (4 * kHistThreads);
+    const float topf = (float)(a.nb - 1);
+    const int ntiles = (colpitch + COLS * kHistThreads - 1) / (COLS * kHistThreads);
     const long long nitems = (long long)a.n_pairs * a.n2;
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
+    const unsigned cbase = sbase - 4u * (unsigned)kMagicBits;   // modulo 2^32
+    const float mlo = a.mlo, mscale = a.mscale;
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int pair = (int)(item / a.n2);
         const int c = (int)(item - (long long)pair * a.n2);
         const float2 mo = a.az[c];
         if (threadIdx.x == 0) { s_lo = 0x7FFFFFFF; s_hi = -1; }
-        for (int p = threadIdx.x; p < a.planes; p += blockDim.x) { run_lo[p] = 0x7FFFFFFF; run_hi[p] = 0; }
+        for (int p = threadIdx.x; p < a.planes; p += blockDim.x) run_hi[p] = 0;
         __syncthreads();
         for (int iz = threadIdx.x; iz < a.fnz; iz += blockDim.x) {
             const AxisSample sz = axis_sample<NN>(__fmaf_rn(mo.x, (float)iz, mo.y), a.mnz);
@@ -173,7 +245,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
             if (sz.ok) {
                 atomicMin(&s_lo, iz);
                 atomicMax(&s_hi, iz);
-                atomicMin(&run_lo[sz.lower], iz);
                 atomicMax(&run_hi[sz.lower], iz + 1);
             }
         }
@@ -191,15 +262,22 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                 p_hi = s1.lower;
             }
             for (int tile = 0; tile < ntiles; ++tile) {
-                const int col0 = (tile * kHistThreads + threadIdx.x) * 4;
+                const int col0 = (tile * kHistThreads + threadIdx.x) * COLS;
                 if (col0 >= colpitch) continue;
-                const uint32_t cv = ld_u32(a.colvalid + (size_t)pair * colpitch + col0);
-                if (cv == 0u) continue;
                 // columns outside the moving volume count into the dump row: (fa & keep) | dump
-                const uint32_t keep = cv * 0xFFu;                       // cv bytes are 0 or 1
-                const uint32_t dump = (~keep) & ((uint32_t)a.rows_real * 0x01010101u);
+                BinVec<COLS> cv, keep, dump;
+                ld_bins<COLS>(cv, a.colvalid + (size_t)pair * colpitch + col0);
+                uint32_t any = 0u;
+#pragma unroll
+                for (int j = 0; j < COLS / 4; ++j) {
+                    any |= cv.w[j];
+                    keep.w[j] = cv.w[j] * 0xFFu;                            // cv bytes are 0 or 1
+                    dump.w[j] = (~keep.w[j]) & ((uint32_t)a.rows_real * 0x01010101u);
+                }
+                if (any == 0u) continue;
                 const uint8_t* __restrict__ fbq = a.fb + (size_t)iz_lo * colpitch + col0;
-                uint32_t fa_next = ld_u32(fbq);
+                BinVec<COLS> fa_next;
+                ld_bins<COLS>(fa_next, fbq);
                 int iz = iz_lo;
                 if (NN) {
                     const uint8_t* __restrict__ pp = static_cast<const uint8_t*>(a.xy) +
@@ -207,42 +285,55 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                     for (int p = p_lo; p <= p_hi; ++p, pp += colpitch) {
                         const int hi = run_hi[p];
                         if (iz >= hi) continue;
-                        const uint32_t v = ld_u32(pp);
+                        BinVec<COLS> v;
+                        ld_bins<COLS>(v, pp);
                         for (; iz < hi; ++iz) {
-                            const uint32_t fa4 = (fa_next & keep) | dump;
+                            BinVec<COLS> fa;
+#pragma unroll
+                            for (int j = 0; j < COLS / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
                             fbq += colpitch;
-                            if (iz + 1 < iz_hi) fa_next = ld_u32(fbq);
-                            red_shared_inc(sbase + ((fa4 & 0xFF) * nb + (v & 0xFF)) * 4u);
-                            red_shared_inc(sbase + (((fa4 >> 8) & 0xFF) * nb + ((v >> 8) & 0xFF)) * 4u);
-                            red_shared_inc(sbase + (((fa4 >> 16) & 0xFF) * nb + ((v >> 16) & 0xFF)) * 4u);
-                            red_shared_inc(sbase + ((fa4 >> 24) * nb + (v >> 24)) * 4u);
+                            if (iz + 1 < iz_hi) ld_bins<COLS>(fa_next, fbq);
+#pragma unroll
+                            for (int k = 0; k < COLS; ++k)
+                                red_shared_inc(sbase + (byte_of(fa.w[k / 4], k & 3) * pitch + byte_of(v.w[k / 4], k & 3)) * 4u);
                         }
                     }
                 } else {
                     const float* __restrict__ pp = static_cast<const float*>(a.xy) +
                                                    ((size_t)pair * a.planes + p_lo) * colpitch + col0;
-                    float4 r0 = ld4(pp), r1 = ld4(pp + colpitch), r2 = r1;
+                    ColVec<COLS> r0, r1, r2;
+                    ld_cols<COLS>(r0, pp);
+                    ld_cols<COLS>(r1, pp + colpitch);
+                    r2 = r1;
                     pp += 2 * (size_t)colpitch;   // next plane to prefetch: p + 2
                     int p = p_lo;
                     // one plane step: prefetch plane p+2 into `pre`, run the slices of plane p on (lo, hi)
-                    auto step = [&](const float4& lo, const float4& hi, float4& pre) {
-                        if (p + 2 < a.planes) pre = ld4(pp);
+                    auto step = [&](const ColVec<COLS>& lo, const ColVec<COLS>& hi, ColVec<COLS>& pre) {
+                        if (p + 2 < a.planes) ld_cols<COLS>(pre, pp);
                         pp += colpitch;
                         const int end = run_hi[p];
-                        for (; iz < end; ++iz) {
-                            const float w = ws[iz];
-                            const uint32_t fa4 = (fa_next & keep) | dump;
-                            fbq += colpitch;
-                            if (iz + 1 < iz_hi) fa_next = ld_u32(fbq);
-                            // CANON-4 z-lerp, CANON-5 binning (floor and clamp by the saturating convert)
-                            const unsigned b0 = bin_u8(__fmul_rn(__fsub_rn(lerp_rn(lo.x, hi.x, w), a.mlo), a.mscale), top);
-                            const unsigned b1 = bin_u8(__fmul_rn(__fsub_rn(lerp_rn(lo.y, hi.y, w), a.mlo), a.mscale), top);
-                            const unsigned b2 = bin_u8(__fmul_rn(__fsub_rn(lerp_rn(lo.z, hi.z, w), a.mlo), a.mscale), top);
-                            const unsigned b3 = bin_u8(__fmul_rn(__fsub_rn(lerp_rn(lo.w, hi.w, w), a.mlo), a.mscale), top);
-                            red_shared_inc(sbase + ((fa4 & 0xFF) * nb + b0) * 4u);
-                            red_shared_inc(sbase + (((fa4 >> 8) & 0xFF) * nb + b1) * 4u);
-                            red_shared_inc(sbase + (((fa4 >> 16) & 0xFF) * nb + b2) * 4u);
-                            red_shared_inc(sbase + ((fa4 >> 24) * nb + b3) * 4u);
+                        if (iz < end) {
+                            float d[COLS];
+#pragma unroll
+                            for (int k = 0; k < COLS; ++k) d[k] = __fsub_rn(hi.v[k], lo.v[k]);
+                            for (; iz < end; ++iz) {
+                                const float w = ws[iz];
+                                BinVec<COLS> fa;
+#pragma unroll
+                                for (int j = 0; j < COLS / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
+                                fbq += colpitch;
+                                if (iz + 1 < iz_hi) ld_bins<COLS>(fa_next, fbq);
+#pragma unroll
+                                for (int k = 0; k < COLS; ++k) {
+                                    const float v = __fmaf_rn(w, d[k], lo.v[k]);
+                                    float t = FAST ? __fmul_rn(v, mscale) : __fmul_rn(__fsub_rn(v, mlo), mscale);
+                                    t = fminf(t, topf);
+                                    if (!FAST) t = fmaxf(t, 0.0f);
+                                    const unsigned mbits = byte_of(fa.w[k / 4], k & 3) * pitch + (unsigned)kMagicBits;
+                                    const float r = __fadd_rd(t, __uint_as_float(mbits));
+                                    red_shared_inc(__float_as_uint(r) * 4u + cbase);
+                                }
+                            }
                         }
                         ++p;
                     };
@@ -257,19 +348,23 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
             }
         }
         __syncthreads();
-        // merge the CTA-private rows into the item's global histogram (un-ranking the fixed bin);
-        // the dump row (rare fixed ranks, handled exactly by zrare_kernel) is only re-zeroed
-        for (int r = warp; r < rows_smem; r += nwarps) {
+        // write the item's whole global histogram (un-ranking the fixed bin): counted rows from shared
+        // memory (re-zeroed for the next item), rows of the rare ranks as zeros -- zrare_kernel adds
+        // their voxels afterwards.  No other CTA touches this histogram, so plain stores suffice.
+        for (int r = warp; r < (int)nb; r += nwarps) {
             uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
             const bool real = r < a.rows_real;
             for (unsigned b = lane; b < nb; b += 32) {
-                const uint32_t v = sh_hist[r * nb + b];
-                if (v) {
-                    sh_hist[r * nb + b] = 0u;
-                    if (real) atomicAdd(&grow[b], v);
+                uint32_t v = 0u;
+                if (real) {
+                    v = sh_hist[r * pitch + b];
+                    if (v) sh_hist[r * pitch + b] = 0u;
                 }
+                grow[b] = v;
             }
         }
+        if (a.rows_real < rows_smem)   // the dump row is only re-zeroed
+            for (unsigned b = threadIdx.x; b < nb; b += blockDim.x) sh_hist[a.rows_real * pitch + b] = 0u;
         __syncthreads();
     }
 }
@@ -291,6 +386,14 @@ __global__ void __launch_bounds__(256) pitch_bins_kernel(const uint8_t* __restri
         r = rows_real;
     }
     out[(size_t)iz * colpitch + col] = (uint8_t)r;
+}
+
+// CANON-5 on the integer side: PTX float->int conversions saturate to the destination range
+// (NaN -> 0), so cvt.rmi.u8 is clamp(floor(t), 0, 255) in one instruction; bins < 256 need one min.
+__device__ __forceinline__ unsigned bin_u8(float t, unsigned top) {
+    unsigned b;
+    asm("cvt.rmi.u8.f32 %0, %1;" : "=r"(b) : "f"(t));
+    return min(b, top);
 }
 
 // Exact handling of the rare fixed-bin rows: for every item (pair, p2) and every rare voxel, the same
@@ -335,7 +438,7 @@ cudaError_t launch_pitch_bins(const uint8_t* in, int cols, int colpitch, int fnz
 
 cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, const float2* ax, int a0,
                          int na, int fnx, void* X, cudaStream_t s) {
-    dim3 grid((fnx + 127) / 128, srows, na);
+    dim3 grid(srows, (fnx + 127) / 128, na);
     if (nn)
         xpass_kernel<true, uint8_t><<<grid, 128, 0, s>>>(static_cast<const uint8_t*>(src), snx, mnx, ax, a0, fnx,
                                                         static_cast<uint8_t*>(X));
@@ -348,40 +451,51 @@ cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, 
 cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
                          const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
                          void* XY, uint8_t* colvalid, cudaStream_t s) {
-    dim3 grid((colpitch + 255) / 256, planes, npairs);
+    dim3 grid((colpitch / 4 + 127) / 128, npairs);
     if (nn)
-        ypass_kernel<true, uint8_t><<<grid, 256, 0, s>>>(static_cast<const uint8_t*>(X), prows, mnx, mny, ax, ay, a0,
-                                                        n1, fnx, cols, colpitch, static_cast<uint8_t*>(XY), colvalid);
+        ypass_kernel<true, uint8_t><<<grid, 128, 0, s>>>(static_cast<const uint8_t*>(X), planes, prows, mnx, mny, ax,
+                                                        ay, a0, n1, fnx, cols, colpitch, static_cast<uint8_t*>(XY),
+                                                        colvalid);
     else
-        ypass_kernel<false, float><<<grid, 256, 0, s>>>(static_cast<const float*>(X), prows, mnx, mny, ax, ay, a0, n1,
-                                                       fnx, cols, colpitch, static_cast<float*>(XY), colvalid);
+        ypass_kernel<false, float><<<grid, 128, 0, s>>>(static_cast<const float*>(X), planes, prows, mnx, mny, ax, ay,
+                                                       a0, n1, fnx, cols, colpitch, static_cast<float*>(XY), colvalid);
     return cudaGetLastError();
 }
 
-// Histogram rows of the z kernel that fit in shared memory, the dump row included (at most nb + 1).
-int zhist_rows_in_smem(int nb, int fnz, int planes, size_t smem_optin) {
+// Histogram rows (of `pitch` words) of the z kernel that fit in shared memory, the dump row included
+// (at most nb + 1).
+int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin) {
     const size_t reserve = 1024 + 4 * (size_t)zhist_table_words(fnz, planes);
-    size_t rows = (smem_optin > reserve ? smem_optin - reserve : 0) / ((size_t)nb * sizeof(uint32_t));
+    size_t rows = (smem_optin > reserve ? smem_optin - reserve : 0) / ((size_t)pitch * sizeof(uint32_t));
     if (rows > (size_t)nb + 1) rows = (size_t)nb + 1;
     return (int)rows;
 }
 
+template <bool NN, int COLS, bool FAST>
+static cudaError_t launch_zhist_t(const ZHistArgs& a, unsigned grid, size_t smem, cudaStream_t s) {
+    auto kern = zhist_kernel<NN, COLS, FAST>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, kHistThreads, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t s) {
-    if (a.rows_smem < 1) return cudaErrorInvalidConfiguration;
-    const size_t smem = 4 * (size_t)zhist_table_words(a.fnz, a.planes) + (size_t)a.rows_smem * a.nb * sizeof(uint32_t);
+    if (a.rows_smem < 1 || a.pitch < a.nb || (a.colpitch % a.cols) != 0) return cudaErrorInvalidConfiguration;
+    const size_t smem = 4 * (size_t)zhist_table_words(a.fnz, a.planes) + (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
     const long long nitems = (long long)a.n_pairs * a.n2;
     long long grid = nitems < num_sms ? nitems : num_sms;
     if (grid < 1) return cudaSuccess;
     cudaError_t e;
+    const unsigned g = (unsigned)grid;
     if (nn) {
-        e = cudaFuncSetAttribute(zhist_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        zhist_kernel<true><<<(unsigned)grid, kHistThreads, smem, s>>>(a);
+        e = a.cols == 8 ? launch_zhist_t<true, 8, false>(a, g, smem, s) : launch_zhist_t<true, 4, false>(a, g, smem, s);
+    } else if (a.fast_bin) {
+        e = a.cols == 8 ? launch_zhist_t<false, 8, true>(a, g, smem, s) : launch_zhist_t<false, 4, true>(a, g, smem, s);
     } else {
-        e = cudaFuncSetAttribute(zhist_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        zhist_kernel<false><<<(unsigned)grid, kHistThreads, smem, s>>>(a);
+        e = a.cols == 8 ? launch_zhist_t<false, 8, false>(a, g, smem, s) : launch_zhist_t<false, 4, false>(a, g, smem, s);
     }
+    if (e != cudaSuccess) return e;
     if (a.n_rare > 0) {
         long long g2 = nitems < 8LL * num_sms ? nitems : 8LL * num_sms;
         if (nn) zrare_kernel<true><<<(unsigned)g2, 256, 0, s>>>(a);

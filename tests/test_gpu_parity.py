@@ -342,3 +342,14 @@ def test_scale_maps_with_plane_skips_and_negative_factors(mi):
                       (2.0,), cfg.truth)
         for interp in (0, 1):
             check_map(mi, c, interp)
+
+
+def test_separable_many_moving_rows_exceeds_grid_y_limit(mi):
+    """(mz+2)*(my+2) > 65535 moving rows (as at the full 260x311x260 size of C3/C4): the x-pass
+    indexes its rows through gridDim.x."""
+    fixed = ph.random_volume((6, 40, 30), 31)
+    moving = ph.random_volume((5, 300, 250), 32)
+    c = ph.Config("rows", fixed, moving, (1.0, 7.0, 8.0), (1.0, 1.0, 1.0), 32, 0, (-1, -3, -3), (1, 3, 3), (2, 2, 2),
+                  (2.0,), (0, 0, 0))
+    for interp in (0, 1):
+        check_map(mi, c, interp)
