@@ -1,0 +1,78 @@
+"""Multi-GPU plumbing for one exhaustive map: shard the parameter grid across ranks, gather the map.
+
+Every map voxel is a separate MI evaluation, so the path shards by TRANSFORMS with no
+exchange inside it: each rank owns a contiguous slab of the slowest grid axis (p2), holds both
+volumes (<= 105 MB, replicated) in its own context, maps its slab with `mi_map`, and the slabs are
+concatenated with one all-gather of doubles (<= 551 KB at C5).  This module holds host logic only
+(grid arithmetic + torch.distributed calls); it never touches the method's arithmetic, so it can be
+exercised with the gloo backend on CPU by passing any `map_fn`.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+
+def axis_values(lo: float, hi: float, n: int) -> np.ndarray:
+    """Grid values of include/mi.h: lo + k*(hi-lo)/(n-1) in double, n == 1 -> lo."""
+    if n == 1:
+        return np.array([lo], dtype=np.float64)
+    return np.array([lo + k * (hi - lo) / (n - 1) for k in range(n)], dtype=np.float64)
+
+
+def slab_bounds(n2: int, rank: int, world: int):
+    """Contiguous [k_begin, k_end) slab of the p2 axis for `rank`; sizes differ by at most one."""
+    if not (0 <= rank < world):
+        raise ValueError("rank %d outside world %d" % (rank, world))
+    base, rem = divmod(int(n2), int(world))
+    begin = rank * base + min(rank, rem)
+    return begin, begin + base + (1 if rank < rem else 0)
+
+
+def shard_grid(lo, hi, n, rank: int, world: int):
+    """Sub-grid (lo', hi', n') of the rank's p2 slab, or None if the slab is empty.
+
+    The slab's end points are taken from the FULL grid's axis values, so every rank evaluates
+    exactly the nodes the single-GPU map would (bit-identical parameters for k_begin and k_end-1;
+    interior nodes are re-derived by mi_map from (lo', hi', n') and agree to the last ulp or two of
+    the parameter -- callers that need bit-identical interior nodes use one p2 plane per call)."""
+    lo = [float(v) for v in lo]
+    hi = [float(v) for v in hi]
+    n = [int(v) for v in n]
+    b, e = slab_bounds(n[2], rank, world)
+    if e <= b:
+        return None
+    vals = axis_values(lo[2], hi[2], n[2])
+    return (lo[0], lo[1], float(vals[b])), (hi[0], hi[1], float(vals[e - 1])), (n[0], n[1], e - b)
+
+
+def map_sharded(map_fn, lo, hi, n, nch: int, rank: int, world: int, dist=None, device=None):
+    """Run `map_fn(lo', hi', n') -> array (nch, n2', n1, n0)` on this rank's slab and return the full
+    (nch, n2, n1, n0) float64 map on every rank plus the per-channel arg max (ties -> lowest index).
+
+    `dist` is `torch.distributed` (already initialised) or None for world == 1."""
+    import torch
+
+    n = [int(v) for v in n]
+    sub = shard_grid(lo, hi, n, rank, world)
+    plane = n[1] * n[0]
+    base = (n[2] + world - 1) // world           # padded slab depth so all_gather sees equal shapes
+    local = torch.zeros((nch, base, n[1], n[0]), dtype=torch.float64, device=device)
+    if sub is not None:
+        m = map_fn(*sub)
+        m = m if isinstance(m, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(m))
+        local[:, : sub[2][2]] = m.to(local.device).reshape(nch, sub[2][2], n[1], n[0])
+    if world == 1 or dist is None:
+        parts = [local]
+    else:
+        parts = [torch.empty_like(local) for _ in range(world)]
+        dist.all_gather(parts, local)
+    full = torch.empty((nch, n[2], n[1], n[0]), dtype=torch.float64, device=local.device)
+    for r in range(len(parts)):
+        b, e = slab_bounds(n[2], r, world)
+        if e > b:
+            full[:, b:e] = parts[r][:, : e - b]
+    flat = full.reshape(nch, n[2] * plane)
+    best = flat.max(dim=1, keepdim=True).values
+    idx = torch.arange(flat.shape[1], device=flat.device).expand_as(flat)
+    argmax = torch.where(flat == best, idx, torch.full_like(idx, flat.shape[1])).min(dim=1).values
+    return full, argmax

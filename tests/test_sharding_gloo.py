@@ -1,0 +1,86 @@
+"""N > 1 host logic on CPU: grid sharding + gloo all-gather of map slabs (world_size 2 and 3).
+The per-slab map function here is the ORACLE (allowed in tests); the GPU path plugs mi_map in."""
+import os
+import socket
+import sys
+
+import numpy as np
+import pytest
+import torch
+import torch.multiprocessing as mp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1909_10690_b200 import sharding as sh  # noqa: E402
+
+
+def test_slab_bounds_cover_the_axis_exactly():
+    for n2 in (1, 2, 5, 41):
+        for world in (1, 2, 3, 8):
+            seen = []
+            for r in range(world):
+                b, e = sh.slab_bounds(n2, r, world)
+                assert 0 <= b <= e <= n2
+                seen += list(range(b, e))
+            assert seen == list(range(n2))
+    with pytest.raises(ValueError):
+        sh.slab_bounds(4, 2, 2)
+
+
+def test_shard_grid_end_points_are_the_full_grids_nodes():
+    lo, hi, n = (-10, -10, -10), (10, 10, 10), (41, 41, 41)
+    vals = sh.axis_values(-10, 10, 41)
+    got = []
+    for r in range(4):
+        slo, shi, sn = sh.shard_grid(lo, hi, n, r, 4)
+        assert slo[:2] == (-10.0, -10.0) and shi[:2] == (10.0, 10.0) and sn[:2] == (41, 41)
+        b, e = sh.slab_bounds(41, r, 4)
+        assert slo[2] == vals[b] and shi[2] == vals[e - 1] and sn[2] == e - b
+        got += list(sh.axis_values(slo[2], shi[2], sn[2]))
+    assert np.allclose(got, vals, rtol=0, atol=1e-12)
+    assert sh.shard_grid(lo, hi, (3, 3, 1), 1, 2) is None          # more ranks than planes
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle as orc
+    from paper_1909_10690_b200 import phantoms as ph
+    cfg = ph.get_config("C1")
+
+    def map_fn(lo, hi, n):
+        return orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                          cfg.family, lo, hi, n, q=cfg.q)["map"]
+
+    full, am = sh.map_sharded(map_fn, cfg.lo, cfg.hi, cfg.n, 1 + len(cfg.q), rank, world, dist=dist)
+    np.save(os.path.join(out_dir, "map_%d.npy" % rank), full.numpy())
+    np.save(os.path.join(out_dir, "am_%d.npy" % rank), am.numpy())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sharded_map_equals_single_rank_map_gloo(world, tmp_path):
+    import oracle as orc
+    from paper_1909_10690_b200 import phantoms as ph
+    cfg = ph.get_config("C1")
+    ref = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                     cfg.family, cfg.lo, cfg.hi, cfg.n, q=cfg.q)
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    for r in range(world):
+        m = np.load(tmp_path / ("map_%d.npy" % r))
+        am = np.load(tmp_path / ("am_%d.npy" % r))
+        assert m.shape == ref["map"].shape
+        assert np.max(np.abs(m - ref["map"])) <= 1e-12       # integer-voxel C1 grid: identical nodes
+        assert np.array_equal(am, ref["argmax"])
