@@ -30,10 +30,10 @@ struct mi_ctx {
     int rows_smem = 0;
     // separable path (diagonal-matrix families)
     uint8_t* d_fb_pitched = nullptr;    // ranked fixed bins, [fnz][colpitch]
-    int colpitch = 0;                   // fny*fnx rounded up to a multiple of 8
+    int colpitch = 0;                   // fny*fnx rounded up to a multiple of kZColAlign
     int zpitch = 0;                     // words per shared histogram row of the z kernel
-    int zcols = 8;                      // adjacent columns per thread of the z kernel (4 or 8)
-    bool fast_bin = false;              // moving_lo == 0 and every moving voxel is finite and >= 0
+    int bin_mode = mi::kBinGeneral;     // moving-side binning variant of the z kernel (mi_internal.h)
+    bool fuse_entropy = true;           // step a5 as the z kernel's epilogue when possible
     int zrows_smem = 0;                 // shared-memory histogram rows of the z kernel (dump row included)
     int zrows_real = 0;                 // fixed ranks counted in shared memory; ranks >= this are "rare"
     uint2* d_rare = nullptr;            // rare voxels (col, iz | rank << 16)
@@ -206,7 +206,9 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
     const size_t elem = nn ? 1 : sizeof(float);
     const size_t x_bytes_per_a = (size_t)planes * prows * fnx * elem;
     const size_t xy_bytes_per_pair = (size_t)planes * c->colpitch * elem;
-    const size_t hist_bytes_per_pair = (size_t)n2 * nbins2 * sizeof(uint32_t);
+    // fused: step a5 runs as the z kernel's epilogue and no histogram leaves the SM
+    const bool fused = c->fuse_entropy && c->n_rare == 0 && nq <= mi::kMaxQPerPass;
+    const size_t hist_bytes_per_pair = fused ? 1 : (size_t)n2 * nbins2 * sizeof(uint32_t);
 
     // p0 values per batch: as many as the scratch budgets allow, chosen to minimise idle SM-waves
     size_t max_pairs = c->xy_budget / xy_bytes_per_pair;
@@ -231,7 +233,8 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
     if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_X), &c->cap_X, (size_t)ga * x_bytes_per_a)) != MI_OK) return st;
     if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_XY), &c->cap_XY, (size_t)ga * n1 * xy_bytes_per_pair)) != MI_OK) return st;
     if ((st = grow(c, &c->d_colvalid, &c->cap_cv, (size_t)ga * n1 * c->colpitch)) != MI_OK) return st;
-    if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist, (size_t)ga * n1 * hist_bytes_per_pair)) != MI_OK) return st;
+    if (!fused && (st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist, (size_t)ga * n1 * hist_bytes_per_pair)) != MI_OK) return st;
+    const float prescale = (!nn && c->bin_mode == mi::kBinFastPrescaled) ? c->mscale : 1.0f;
     for (int d = 0; d < 3; ++d)
         MI_CUDA(c, cudaMemcpyAsync(c->d_axis + (size_t)d * nmax, sp.axis[d].data(), sp.axis[d].size() * sizeof(float2),
                                    cudaMemcpyHostToDevice, s));
@@ -249,7 +252,7 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
         else
             MI_CUDA(c, mi::launch_xpass(false, c->d_moving_pad, c->md[0] + 2, planes * prows, c->md[0], ax, a0, na, fnx, c->d_X, s));
         MI_CUDA(c, mi::launch_ypass(nn, c->d_X, planes, prows, c->md[0], c->md[1], ax, ay, a0, n1, npairs, fnx, cols,
-                                    c->colpitch, c->d_XY, c->d_colvalid, s));
+                                    c->colpitch, prescale, c->d_XY, c->d_colvalid, s));
         mi::ZHistArgs z;
         z.xy = c->d_XY;
         z.colvalid = c->d_colvalid;
@@ -264,8 +267,7 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
         z.nb = c->nb;
         z.rows_smem = c->zrows_smem;
         z.pitch = c->zpitch;
-        z.cols = c->zcols;
-        z.fast_bin = c->fast_bin ? 1 : 0;
+        z.bin_mode = c->bin_mode;
         z.rows_real = c->zrows_real;
         z.rare = c->d_rare;
         z.n_rare = c->n_rare;
@@ -273,9 +275,18 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
         z.mscale = c->mscale;
         z.n_pairs = npairs;
         z.n2 = n2;
+        z.fused = fused ? 1 : 0;
+        z.q = c->d_q;
+        z.nq = nq;
+        z.nq_total = nq;
+        z.form = c->tsallis_form;
+        z.mi_out = c->d_mi;
+        z.nvalid = c->d_nvalid;
+        z.om = mi::OutMap{1, n0, n1, n2, a0};
         MI_CUDA(c, mi::launch_zhist(nn, z, c->num_sms, s));
-        c->last_launches[1] += 3;
+        c->last_launches[1] += 3 + (c->n_rare > 0 ? 1 : 0);
         timer.end();
+        if (fused) continue;
 
         timer.begin(2);
         int q_off = 0;
@@ -527,12 +538,12 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = cudaMalloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
         if ((e = cudaMalloc((void**)&d_mov, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
         if ((e = cudaMalloc((void**)&d_tmp, (size_t)nf * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
-        c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + 7) & ~7LL);
+        c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + mi::kZColAlign - 1) / mi::kZColAlign * mi::kZColAlign);
         if ((e = cudaMalloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
         // bank of histogram word (a, b) = (a*pad + b) mod 32: an odd pad walks the rows over all banks
         int zpad = 9;
-        if (const char* v = std::getenv("MI_B200_HIST_PAD")) { const int r = std::atoi(v); if (r >= 0 && r <= 64) zpad = r; }
-        if (const char* v = std::getenv("MI_B200_ZCOLS")) { const int r = std::atoi(v); if (r == 4 || r == 8) c->zcols = r; }
+        if (const char* v = std::getenv("MI_B200_HIST_PAD")) { const int r = std::atoi(v); if (r >= 1 && r <= 64) zpad = r; }
+        if (const char* v = std::getenv("MI_B200_FUSE_ENTROPY")) c->fuse_entropy = std::atoi(v) != 0;
         c->zpitch = nbins + zpad;
         c->zrows_smem = mi::zhist_rows_in_smem(nbins, c->zpitch, fixed_dims[2], moving_dims[2] + 2, c->smem_optin);
         c->rows_smem = mi::hist_rows_in_smem(nbins, c->smem_optin);
@@ -553,8 +564,12 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             unsigned h_flag = 1;
             if ((e = cudaMemcpyAsync(&h_flag, d_counts, sizeof(unsigned), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy flag"); break; }
             if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync flag"); break; }
-            c->fast_bin = h_flag == 0 && c->mlo == 0.0f;
-            if (const char* v = std::getenv("MI_B200_FAST_BIN")) { if (std::atoi(v) == 0) c->fast_bin = false; }
+            // kBinFast*: no clamps needed (mi_internal.h); prescaled when the bin scale is a power of two
+            // (so that scaling commutes with every rounding; 2^-100 < scale keeps products normal)
+            int ex = 0;
+            const bool pow2 = std::frexp(c->mscale, &ex) == 0.5f && ex > -100 && ex < 100;
+            c->bin_mode = (h_flag == 0 && c->mlo == 0.0f) ? (pow2 ? mi::kBinFastPrescaled : mi::kBinFast) : mi::kBinGeneral;
+            if (const char* v = std::getenv("MI_B200_BIN_MODE")) { const int r = std::atoi(v); if (r >= 0 && r < c->bin_mode) c->bin_mode = r; }
         }
         if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
         {

@@ -38,7 +38,7 @@ struct ResampleArgs {
     int nslabs;              // CTAs cooperating on one transform (row slabs)
 };
 
-// flag (may be NULL): set to 1 if any voxel is negative or not finite
+// flag (may be NULL): set to 1 if any voxel is negative, not finite or above the last bin edge
 cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, float scale, int nb,
                           unsigned* flag, cudaStream_t s);
 cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s);
@@ -67,22 +67,40 @@ struct ZHistArgs {
     uint32_t* hist;            // [n_pairs*n2][nb][nb], zero on entry
     int fnz, colpitch, planes, mnz;
     int nb, rows_smem;         // rows_smem: histogram rows in shared memory, dump row included
-    int pitch;                 // words per shared histogram row (>= nb; the pad spreads rows over banks)
-    int cols;                  // adjacent columns per thread: 4 or 8 (colpitch is a multiple of it)
-    int fast_bin;              // mlo == 0 and every moving voxel is finite and >= 0: t = v*mscale >= 0
+    int pitch;                 // words per shared histogram row (>= nb + 1; the pad spreads rows over banks)
+    int bin_mode;              // kBinGeneral / kBinFast / kBinFastPrescaled (see below)
     int rows_real;             // ranks below rows_real are counted in shared memory; the rest are "rare"
     float mlo, mscale;
     int n_pairs, n2;
     const uint2* rare;         // rare voxels: (col, iz | rank << 16)
     unsigned n_rare;
+    // fused entropy epilogue (step a5 straight from the shared histogram; needs n_rare == 0):
+    // hist is not written, the (1 + nq_total) values of item go to mi_out at its map position
+    int fused;
+    const double* q;           // device, nq_total orders; the first nq (<= kMaxQPerPass) are computed
+    int nq, nq_total, form;
+    double* mi_out;
+    int64_t* nvalid;
+    OutMap om;
 };
+// Moving-side binning variants of the z kernel (CANON-5, t = (v - mlo) * mscale, clamp, floor):
+//   kBinGeneral        the full sequence
+//   kBinFast           mlo == 0 and every moving voxel v is finite with 0 <= v and v*mscale <= nb:
+//                      every lerp result lies between its inputs, so t = v*mscale is in [0, nb]
+//                      without clamps; floor(t) == nb (v == hi) is counted in pad column nb of the
+//                      shared row and added to column nb-1 when the histogram is finished
+//   kBinFastPrescaled  kBinFast and mscale is a power of two: the y-pass stores v*mscale (exact),
+//                      and fma(w, s*hi - s*lo, s*lo) == s*fma(w, hi - lo, lo) bit for bit
+enum { kBinGeneral = 0, kBinFast = 1, kBinFastPrescaled = 2 };
+constexpr int kZCols = 8;            // columns per thread of the z kernel: 2 groups of 4
+constexpr int kZColAlign = 32 * kZCols;  // colpitch is a multiple of this (one warp's columns)
 cudaError_t launch_pitch_bins(const uint8_t* in, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
                               uint2* rare, unsigned* rare_count, unsigned rare_cap, cudaStream_t s);
 cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, const float2* ax, int a0,
                          int na, int fnx, void* X, cudaStream_t s);
 cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
                          const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
-                         void* XY, uint8_t* colvalid, cudaStream_t s);
+                         float prescale, void* XY, uint8_t* colvalid, cudaStream_t s);
 int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin);
 cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t s);
 cudaError_t launch_map_assemble(const double* mi /* n x nch */, int64_t n, int nch, double* map_out,

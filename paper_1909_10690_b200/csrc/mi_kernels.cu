@@ -29,9 +29,12 @@ __device__ __forceinline__ int bin_index(float v, float lo, float scale, float t
 }
 
 // Each thread turns 16 consecutive floats (4 x 16-byte loads) into one 16-byte store.
-// `flag` (may be NULL) is set when a voxel is negative or not finite (the z-histogram kernel may
-// skip the lower clamp of CANON-5 when it stays 0 and lo == 0).
-__device__ __forceinline__ bool plain_nonneg(float v) { return v >= 0.0f && v <= 3.0e38f; }
+// `flag` (may be NULL) is set when a voxel is negative, not finite, or lands above the last bin
+// edge ((v - lo)*scale > nb): while it stays 0 and lo == 0 the z-histogram kernel may skip both
+// clamps of CANON-5 (mi_internal.h, kBinFast).
+__device__ __forceinline__ bool plain_inrange(float v, float lo, float scale, float top) {
+    return v >= 0.0f && __fmul_rn(__fsub_rn(v, lo), scale) <= top + 1.0f;
+}
 
 __global__ void __launch_bounds__(256) prebin_kernel(const float* __restrict__ vol,
                                                      uint8_t* __restrict__ bins, int64_t n, float lo,
@@ -45,7 +48,8 @@ __global__ void __launch_bounds__(256) prebin_kernel(const float* __restrict__ v
 #pragma unroll
         for (int k = 0; k < 4; ++k) {
             v[k] = __ldcs(src + k);
-            odd |= !(plain_nonneg(v[k].x) && plain_nonneg(v[k].y) && plain_nonneg(v[k].z) && plain_nonneg(v[k].w));
+            odd |= !(plain_inrange(v[k].x, lo, scale, top) && plain_inrange(v[k].y, lo, scale, top) &&
+                     plain_inrange(v[k].z, lo, scale, top) && plain_inrange(v[k].w, lo, scale, top));
         }
         uint32_t w[4];
 #pragma unroll
@@ -62,7 +66,7 @@ __global__ void __launch_bounds__(256) prebin_kernel(const float* __restrict__ v
     const int64_t j = tail0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (j < n) {
         bins[j] = (uint8_t)bin_index(vol[j], lo, scale, top);
-        odd |= !plain_nonneg(vol[j]);
+        odd |= !plain_inrange(vol[j], lo, scale, top);
     }
     if (flag != nullptr && __any_sync(0xffffffffu, odd) && (threadIdx.x & 31) == 0) atomicOr(flag, 1u);
 }

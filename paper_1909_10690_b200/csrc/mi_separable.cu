@@ -82,7 +82,8 @@ __global__ void __launch_bounds__(128) xpass_kernel(const VT* __restrict__ src, 
 // grid: (ceil(colpitch/4 / 128), npairs).  pair = a_local*n1 + b.  Every thread owns 4 adjacent
 // columns of one pair, resolves their x/y samples once and then walks all planes (unrolled by 4 for
 // memory-level parallelism), writing XY[pair][plane][col..col+3] as one 16-byte store per plane, and
-// colvalid[pair][col..col+3].
+// colvalid[pair][col..col+3].  Trilinear values are stored times `prescale` (1, or the power-of-two
+// bin scale in kBinFastPrescaled mode -- an exact multiplication).
 template <bool NN, typename VT>
 struct Quad;
 template <>
@@ -102,8 +103,8 @@ template <bool NN, typename VT>
 __global__ void __launch_bounds__(128) ypass_kernel(const VT* __restrict__ X, int planes, int prows, int mnx,
                                                     int mny, const float2* __restrict__ ax,
                                                     const float2* __restrict__ ay, int a0, int n1, int fnx,
-                                                    int cols, int colpitch, VT* __restrict__ XY,
-                                                    uint8_t* __restrict__ colvalid) {
+                                                    int cols, int colpitch, float prescale,
+                                                    VT* __restrict__ XY, uint8_t* __restrict__ colvalid) {
     const int col0 = (blockIdx.x * 128 + threadIdx.x) * 4;
     if (col0 >= colpitch) return;
     const int pair = blockIdx.y;
@@ -141,7 +142,7 @@ __global__ void __launch_bounds__(128) ypass_kernel(const VT* __restrict__ X, in
             if (off[k] >= 0) {
                 const VT* __restrict__ r = X + off[k] + plane * pstride;
                 if (NN) v = __ldg(r);
-                else v = (VT)lerp_rn((float)__ldg(r), (float)__ldg(r + fnx), wy[k]);
+                else v = (VT)__fmul_rn(lerp_rn((float)__ldg(r), (float)__ldg(r + fnx), wy[k]), prescale);
             }
             q.set(k, v);
         }
@@ -149,7 +150,7 @@ __global__ void __launch_bounds__(128) ypass_kernel(const VT* __restrict__ X, in
     }
 }
 
-// ---- z-lerp + joint histogram ---------------------------------------------------------------------
+// ---- z-lerp + joint histogram (+ fused entropy epilogue) --------------------------------------------
 __device__ __forceinline__ float4 ld4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 __device__ __forceinline__ uint32_t ld_u32(const uint8_t* p) { return __ldg(reinterpret_cast<const uint32_t*>(p)); }
 
@@ -159,62 +160,203 @@ __device__ __forceinline__ void red_shared_inc(unsigned addr) {
     asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
 }
 
-// Words of shared memory in front of the histogram: ws[fnz] + run_hi[planes], rounded up to a
-// multiple of 4 words.
-__host__ __device__ __forceinline__ int zhist_table_words(int fnz, int planes) {
-    return (fnz + planes + 3) & ~3;
+__device__ __forceinline__ unsigned warp_sum_u(unsigned v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
 }
 
-template <int COLS>
-struct ColVec {                      // COLS adjacent columns of one plane / one fixed slice
-    float v[COLS];
-};
-template <int COLS>
-__device__ __forceinline__ void ld_cols(ColVec<COLS>& r, const float* p) {
-#pragma unroll
-    for (int j = 0; j < COLS / 4; ++j) {
-        const float4 q = ld4(p + 4 * j);
-        r.v[4 * j] = q.x; r.v[4 * j + 1] = q.y; r.v[4 * j + 2] = q.z; r.v[4 * j + 3] = q.w;
-    }
+// Shared-memory layout of the z kernel, in 32-bit words:
+//   ws[fnz] z-weights | run_hi[planes] | (pad to 4) | pb[kEntropyPb] | red[kEntropyRed] | histogram rows
+// pb / red are the fused entropy epilogue's scratch (moving marginal counts; per-warp partial sums).
+constexpr int kEntropyAcc = 1 + kMaxQPerPass;                     // sum c ln c, sum c^q_k
+constexpr int kEntropyPb = 272;                                   // 256 moving bins + 8 partial totals, multiple of 4
+constexpr int kEntropyRed = 2 * kEntropyAcc * (kHistThreads / 32 + 16);  // doubles as word pairs
+__host__ __device__ __forceinline__ int zhist_table_words(int fnz, int planes) {
+    return ((fnz + planes + 3) & ~3) + kEntropyPb + kEntropyRed;
 }
-template <int COLS>
-struct BinVec {                      // COLS adjacent uint8 values
-    uint32_t w[COLS / 4];
+
+struct Cols {                        // this thread's kZCols columns of one plane: 2 groups of 4
+    float4 g[kZCols / 4];
 };
-template <int COLS>
-__device__ __forceinline__ void ld_bins(BinVec<COLS>& r, const uint8_t* p) {
-    if (COLS == 8) {
-        const uint2 q = __ldg(reinterpret_cast<const uint2*>(p));
-        r.w[0] = q.x; r.w[COLS / 4 - 1] = q.y;
-    } else {
-        r.w[0] = ld_u32(p);
-    }
+__device__ __forceinline__ void ld_cols(Cols& r, const float* p) {
+#pragma unroll
+    for (int j = 0; j < kZCols / 4; ++j) r.g[j] = ld4(p + 128 * j);
+}
+__device__ __forceinline__ float col_of(const Cols& r, int k) { return (&r.g[k >> 2].x)[k & 3]; }
+struct Bins {                        // the same columns of a uint8 plane / fixed slice
+    uint32_t w[kZCols / 4];
+};
+__device__ __forceinline__ void ld_bins(Bins& r, const uint8_t* p) {
+#pragma unroll
+    for (int j = 0; j < kZCols / 4; ++j) r.w[j] = ld_u32(p + 128 * j);
 }
 __device__ __forceinline__ unsigned byte_of(uint32_t w, int k) { return __byte_perm(w, 0u, 0x4440u | (unsigned)k); }
 
-// One CTA per (pair, p2) item at a time; every thread owns COLS adjacent columns (iy,ix) of the
-// fixed volume and walks them along z.  The walk is organised by moving plane: for lower plane p the
-// fixed slices iz with floor(c_z) = p form one contiguous run (c_z is non-decreasing in iz), during
-// which the two xy-lerped plane values stay in registers; the next plane is prefetched one step
-// ahead and the three register sets rotate by name (the plane loop is unrolled by 3), so a plane step
-// costs one 16-byte load per 4 columns and a pointer increment.
+// Accumulate the entropy terms of one count c > 0 (CANON-7 on integer counts):
+//   acc[0] += c ln c,  acc[1+k] += c^q_k = exp(q_k ln c)
+template <int NQ>
+__device__ __forceinline__ void entropy_terms(double (&acc)[kEntropyAcc], unsigned c, const double (&qv)[kMaxQPerPass],
+                                              int nq) {
+    const double dv = (double)c;
+    const double lc = log(dv);
+    acc[0] += dv * lc;
+#pragma unroll
+    for (int k = 0; k < NQ; ++k)
+        if (k < nq) acc[1 + k] += exp(qv[k] * lc);
+}
+
+// Step a5 from the finished shared histogram of one item (all kHistThreads threads call this; the
+// CTA is synchronised on entry).  With c the integer counts and N their total (CANON-7):
+//   H = ln N - (sum c ln c)/N,   sum p^q = exp(-q ln N) * sum c^q.
+// Pass 1: every warp takes rows; each non-zero count adds its joint terms, is added to the moving
+// marginal pb[b] and re-zeroed; the row sum (fixed marginal) is parked in the row's first word.
+// Pass 2: threads 0..255 take the fixed marginal, threads 256..511 the moving marginal.
+// Per-warp partial sums meet in sh_red (fixed summation order -> reproducible values).
+__device__ __forceinline__ void zhist_entropy_epilogue(const ZHistArgs& a, long long item, uint32_t* sh_hist,
+                                                       uint32_t* sh_pb, double* sh_red) {
+    constexpr int nwarps = kHistThreads / 32;
+    constexpr int kSlots = nwarps + 16;          // joint warps | 8 fixed-marginal warps | 8 moving-marginal warps
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned nb = (unsigned)a.nb, pitch = (unsigned)a.pitch;
+    const int nq = a.nq;
+    double qv[kMaxQPerPass];
+#pragma unroll
+    for (int k = 0; k < kMaxQPerPass; ++k) qv[k] = k < nq ? __ldg(a.q + k) : 1.0;
+
+    double acc[kEntropyAcc];
+#pragma unroll
+    for (int i = 0; i < kEntropyAcc; ++i) acc[i] = 0.0;
+    for (int r = warp; r < a.rows_real; r += nwarps) {
+        uint32_t* row = sh_hist + r * pitch;
+        unsigned rowsum = 0u;
+        for (unsigned b = lane; b < nb; b += 32) {
+            const unsigned v = row[b];
+            if (v) {
+                row[b] = 0u;
+                rowsum += v;
+                atomicAdd(&sh_pb[b], v);
+                entropy_terms<kMaxQPerPass>(acc, v, qv, nq);
+            }
+        }
+        rowsum = warp_sum_u(rowsum);
+        if (lane == 0) row[0] = rowsum;
+    }
+#pragma unroll
+    for (int i = 0; i < kEntropyAcc; ++i) {
+        const double s = warp_sum_d(acc[i]);
+        if (lane == 0) sh_red[i * kSlots + warp] = s;
+        acc[i] = 0.0;
+    }
+    __syncthreads();
+
+    if (warp < 16) {
+        unsigned cnt = 0u;
+        if (warp < 8) {
+            const int r = threadIdx.x;
+            if (r < a.rows_real) {
+                cnt = sh_hist[r * pitch];
+                sh_hist[r * pitch] = 0u;
+            }
+        } else {
+            const unsigned b = threadIdx.x - 256u;
+            if (b < nb) {
+                cnt = sh_pb[b];
+                sh_pb[b] = 0u;
+            }
+        }
+        if (cnt) entropy_terms<kMaxQPerPass>(acc, cnt, qv, nq);
+#pragma unroll
+        for (int i = 0; i < kEntropyAcc; ++i) {
+            const double s = warp_sum_d(acc[i]);
+            if (lane == 0) sh_red[i * kSlots + nwarps + warp] = s;
+        }
+        const unsigned n = warp_sum_u(cnt);   // N_f < 2^31: the total fits
+        if (lane == 0 && warp < 8) sh_pb[256 + warp] = n;
+    }
+    __syncthreads();
+
+    if (threadIdx.x == 0) {
+        unsigned long long n = 0;
+        for (int w = 0; w < 8; ++w) n += sh_pb[256 + w];
+        size_t dst = (size_t)item;
+        if (a.om.enabled) {  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
+            const long long c = item % a.om.n2, ab = item / a.om.n2;
+            const long long b = ab % a.om.n1, al = ab / a.om.n1;
+            dst = ((size_t)c * a.om.n1 + (size_t)b) * a.om.n0 + (size_t)(a.om.a0 + al);
+        }
+        double* out = a.mi_out + dst * (size_t)(1 + a.nq_total);
+        if (a.nvalid != nullptr) a.nvalid[dst] = (int64_t)n;
+        if (n == 0) {
+            out[0] = 0.0;
+            for (int k = 0; k < nq; ++k) out[1 + k] = 0.0;
+        } else {
+            const double N = (double)n, lnN = log(N);
+            double tA[kEntropyAcc], tB[kEntropyAcc], tAB[kEntropyAcc];
+            for (int i = 0; i <= nq; ++i) {
+                double sab = 0.0, sa = 0.0, sb = 0.0;
+                for (int w = 0; w < nwarps; ++w) sab += sh_red[i * kSlots + w];
+                for (int w = 0; w < 8; ++w) sa += sh_red[i * kSlots + nwarps + w];
+                for (int w = 8; w < 16; ++w) sb += sh_red[i * kSlots + nwarps + w];
+                tA[i] = sa; tB[i] = sb; tAB[i] = sab;
+            }
+            const double HA = lnN - tA[0] / N, HB = lnN - tB[0] / N, HAB = lnN - tAB[0] / N;
+            const double I = HA + HB - HAB;  // eq. 2
+            out[0] = I;
+            for (int k = 0; k < nq; ++k) {
+                const double qq = qv[k];
+                double val;
+                if (qq == 1.0) {
+                    val = I;
+                } else {
+                    const double sc = exp(-qq * lnN);
+                    const double SA = (1.0 - tA[1 + k] * sc) / (qq - 1.0);
+                    const double SB = (1.0 - tB[1 + k] * sc) / (qq - 1.0);
+                    const double SAB = (1.0 - tAB[1 + k] * sc) / (qq - 1.0);
+                    val = SA + SB - SAB;
+                    if (a.form == MI_TSALLIS_PSEUDO_ADDITIVE) val += (1.0 - qq) * SA * SB;
+                }
+                out[1 + k] = val;
+            }
+        }
+    }
+}
+
+// One CTA per (pair, p2) item at a time; every thread owns kZCols columns (iy,ix) of the fixed volume
+// -- two groups of 4 adjacent columns, the groups of a warp interleaved so that each 16-byte load
+// instruction of a warp reads 512 contiguous bytes -- and walks them along z.  The walk is organised
+// by moving plane: for lower plane p the fixed slices iz with floor(c_z) = p form one contiguous run
+// (c_z is non-decreasing in iz), during which the two xy-lerped plane values stay in registers; the
+// next plane is prefetched one step ahead and the three register sets rotate by name (the plane loop
+// is unrolled by 3), so a plane step costs one 16-byte load per 4 columns and a pointer increment.
 //
 // Histogram update, trilinear (CANON-4 z-lerp, CANON-5 binning, one RED):
-//   v = fma(w, hi - lo, lo)              hi - lo is formed once per plane step
-//   t = (v - mlo) * mscale               FAST: mlo == 0 and every moving voxel >= 0, so v - 0 == v
-//   t = min(max(t, 0), nb - 1)           FAST: t >= 0 already; clamping before the floor == after it
+//   v = fma(w, hi - lo, lo)
+//   t = (v - mlo) * mscale               kBinFast: t = v*mscale; kBinFastPrescaled: t = v
+//   t = min(max(t, 0), nb - 1)           kBinFast*: not needed, t is in [0, nb] (mi_internal.h)
 //   r = RD(t + (1.5*2^23 + a*pitch))     the low mantissa bits of r are a*pitch + floor(t) EXACTLY
 //                                        (ulp is 1 there and the second addend is an integer)
 //   RED [4*bits(r) + const]              const folds the shared base and -4*bits(1.5*2^23)
 // The shared histogram rows have a pitch of nb + pad words: bank = (a*pad + b) mod 32, so the rows
-// of the (many) background fixed bins do not all start on bank 0.
+// of the (many) background fixed bins do not all start on bank 0; pad column nb takes v == hi.
 //
-// Shared memory: ws[fnz] z-weights | run_hi[planes] | histogram rows (pitch words each).
-template <bool NN, int COLS, bool FAST>
+// Epilogue: either the histogram is written to global memory (un-ranking the fixed bin), or -- fused
+// mode -- step a5 runs straight from shared memory: sum c ln c and sum c^q of the joint counts and
+// of both marginals in double, then eq. 2 and its Tsallis forms, written to the
+// item's position in the map.  Entropies do not depend on the order of the bins, so the ranked rows
+// are used as they are.
+template <bool NN, int MODE>
 __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_constant__ ZHistArgs a) {
     extern __shared__ __align__(16) uint32_t sh_raw[];
     float* ws = reinterpret_cast<float*>(sh_raw);
     int* run_hi = reinterpret_cast<int*>(sh_raw) + a.fnz;
+    uint32_t* sh_pb = sh_raw + ((a.fnz + a.planes + 3) & ~3);
+    double* sh_red = reinterpret_cast<double*>(sh_pb + kEntropyPb);
     uint32_t* sh_hist = sh_raw + zhist_table_words(a.fnz, a.planes);
     __shared__ int s_lo, s_hi;
     const unsigned nb = (unsigned)a.nb;
@@ -222,11 +364,13 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
     const int rows_smem = a.rows_smem;   // includes the dump row
     const int words = rows_smem * a.pitch;
     for (int w = threadIdx.x; w < words; w += blockDim.x) sh_hist[w] = 0u;
+    for (int w = threadIdx.x; w < kEntropyPb; w += blockDim.x) sh_pb[w] = 0u;
 
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int nwarps = kHistThreads / 32;
     const int colpitch = a.colpitch;
     const float topf = (float)(a.nb - 1);
-    const int ntiles = (colpitch + COLS * kHistThreads - 1) / (COLS * kHistThreads);
+    const int ntiles = (colpitch + kZCols * kHistThreads - 1) / (kZCols * kHistThreads);
     const long long nitems = (long long)a.n_pairs * a.n2;
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
     const unsigned cbase = sbase - 4u * (unsigned)kMagicBits;   // modulo 2^32
@@ -250,7 +394,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
         }
         __syncthreads();
         const int iz_lo = s_lo, iz_hi = s_hi + 1;   // valid z is one interval (c_z is monotone in iz)
-        uint32_t* gh = a.hist + (size_t)item * a.nb * a.nb;
 
         if (iz_lo < iz_hi) {
             // lower planes visited: p_lo .. p_hi (planes whose run is empty are stepped over)
@@ -262,22 +405,23 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                 p_hi = s1.lower;
             }
             for (int tile = 0; tile < ntiles; ++tile) {
-                const int col0 = (tile * kHistThreads + threadIdx.x) * COLS;
-                if (col0 >= colpitch) continue;
+                const int wcol = (tile * kHistThreads + warp * 32) * kZCols;   // first column of the warp
+                if (wcol >= colpitch) break;                                   // colpitch % kZColAlign == 0
+                const int col0 = wcol + lane * 4;                              // groups at col0, col0 + 128
                 // columns outside the moving volume count into the dump row: (fa & keep) | dump
-                BinVec<COLS> cv, keep, dump;
-                ld_bins<COLS>(cv, a.colvalid + (size_t)pair * colpitch + col0);
+                Bins cv, keep, dump;
+                ld_bins(cv, a.colvalid + (size_t)pair * colpitch + col0);
                 uint32_t any = 0u;
 #pragma unroll
-                for (int j = 0; j < COLS / 4; ++j) {
+                for (int j = 0; j < kZCols / 4; ++j) {
                     any |= cv.w[j];
                     keep.w[j] = cv.w[j] * 0xFFu;                            // cv bytes are 0 or 1
                     dump.w[j] = (~keep.w[j]) & ((uint32_t)a.rows_real * 0x01010101u);
                 }
                 if (any == 0u) continue;
                 const uint8_t* __restrict__ fbq = a.fb + (size_t)iz_lo * colpitch + col0;
-                BinVec<COLS> fa_next;
-                ld_bins<COLS>(fa_next, fbq);
+                Bins fa_next;
+                ld_bins(fa_next, fbq);
                 int iz = iz_lo;
                 if (NN) {
                     const uint8_t* __restrict__ pp = static_cast<const uint8_t*>(a.xy) +
@@ -285,54 +429,56 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                     for (int p = p_lo; p <= p_hi; ++p, pp += colpitch) {
                         const int hi = run_hi[p];
                         if (iz >= hi) continue;
-                        BinVec<COLS> v;
-                        ld_bins<COLS>(v, pp);
+                        Bins v;
+                        ld_bins(v, pp);
                         for (; iz < hi; ++iz) {
-                            BinVec<COLS> fa;
+                            Bins fa;
 #pragma unroll
-                            for (int j = 0; j < COLS / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
+                            for (int j = 0; j < kZCols / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
                             fbq += colpitch;
-                            if (iz + 1 < iz_hi) ld_bins<COLS>(fa_next, fbq);
+                            if (iz + 1 < iz_hi) ld_bins(fa_next, fbq);
 #pragma unroll
-                            for (int k = 0; k < COLS; ++k)
+                            for (int k = 0; k < kZCols; ++k)
                                 red_shared_inc(sbase + (byte_of(fa.w[k / 4], k & 3) * pitch + byte_of(v.w[k / 4], k & 3)) * 4u);
                         }
                     }
                 } else {
                     const float* __restrict__ pp = static_cast<const float*>(a.xy) +
                                                    ((size_t)pair * a.planes + p_lo) * colpitch + col0;
-                    ColVec<COLS> r0, r1, r2;
-                    ld_cols<COLS>(r0, pp);
-                    ld_cols<COLS>(r1, pp + colpitch);
+                    Cols r0, r1, r2;
+                    ld_cols(r0, pp);
+                    ld_cols(r1, pp + colpitch);
                     r2 = r1;
                     pp += 2 * (size_t)colpitch;   // next plane to prefetch: p + 2
                     int p = p_lo;
                     // one plane step: prefetch plane p+2 into `pre`, run the slices of plane p on (lo, hi)
-                    auto step = [&](const ColVec<COLS>& lo, const ColVec<COLS>& hi, ColVec<COLS>& pre) {
-                        if (p + 2 < a.planes) ld_cols<COLS>(pre, pp);
+                    auto step = [&](const Cols& lo, const Cols& hi, Cols& pre) {
+                        if (p + 2 < a.planes) ld_cols(pre, pp);
                         pp += colpitch;
                         const int end = run_hi[p];
-                        if (iz < end) {
-                            float d[COLS];
+                        for (; iz < end; ++iz) {
+                            const float w = ws[iz];
+                            Bins fa;
 #pragma unroll
-                            for (int k = 0; k < COLS; ++k) d[k] = __fsub_rn(hi.v[k], lo.v[k]);
-                            for (; iz < end; ++iz) {
-                                const float w = ws[iz];
-                                BinVec<COLS> fa;
+                            for (int j = 0; j < kZCols / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
+                            fbq += colpitch;
+                            if (iz + 1 < iz_hi) ld_bins(fa_next, fbq);
 #pragma unroll
-                                for (int j = 0; j < COLS / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
-                                fbq += colpitch;
-                                if (iz + 1 < iz_hi) ld_bins<COLS>(fa_next, fbq);
-#pragma unroll
-                                for (int k = 0; k < COLS; ++k) {
-                                    const float v = __fmaf_rn(w, d[k], lo.v[k]);
-                                    float t = FAST ? __fmul_rn(v, mscale) : __fmul_rn(__fsub_rn(v, mlo), mscale);
-                                    t = fminf(t, topf);
-                                    if (!FAST) t = fmaxf(t, 0.0f);
-                                    const unsigned mbits = byte_of(fa.w[k / 4], k & 3) * pitch + (unsigned)kMagicBits;
-                                    const float r = __fadd_rd(t, __uint_as_float(mbits));
-                                    red_shared_inc(__float_as_uint(r) * 4u + cbase);
+                            for (int k = 0; k < kZCols; ++k) {
+                                const float l = col_of(lo, k);
+                                const float v = __fmaf_rn(w, __fsub_rn(col_of(hi, k), l), l);
+                                float t;
+                                if (MODE == kBinFastPrescaled) {
+                                    t = v;
+                                } else if (MODE == kBinFast) {
+                                    t = __fmul_rn(v, mscale);
+                                } else {
+                                    t = __fmul_rn(__fsub_rn(v, mlo), mscale);
+                                    t = fmaxf(fminf(t, topf), 0.0f);   // clamping before the floor == after it
                                 }
+                                const unsigned mbits = byte_of(fa.w[k / 4], k & 3) * pitch + (unsigned)kMagicBits;
+                                const float r = __fadd_rd(t, __uint_as_float(mbits));
+                                red_shared_inc(__float_as_uint(r) * 4u + cbase);
                             }
                         }
                         ++p;
@@ -348,23 +494,39 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
             }
         }
         __syncthreads();
-        // write the item's whole global histogram (un-ranking the fixed bin): counted rows from shared
-        // memory (re-zeroed for the next item), rows of the rare ranks as zeros -- zrare_kernel adds
-        // their voxels afterwards.  No other CTA touches this histogram, so plain stores suffice.
-        for (int r = warp; r < (int)nb; r += nwarps) {
-            uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
-            const bool real = r < a.rows_real;
-            for (unsigned b = lane; b < nb; b += 32) {
-                uint32_t v = 0u;
-                if (real) {
-                    v = sh_hist[r * pitch + b];
-                    if (v) sh_hist[r * pitch + b] = 0u;
+        if (!NN && MODE != kBinGeneral) {   // pad column nb (v == moving_hi) belongs to the last bin
+            for (int r = threadIdx.x; r < rows_smem; r += blockDim.x) {
+                const uint32_t v = sh_hist[r * pitch + nb];
+                if (v) {
+                    sh_hist[r * pitch + nb] = 0u;
+                    sh_hist[r * pitch + nb - 1] += v;
                 }
-                grow[b] = v;
+            }
+            __syncthreads();
+        }
+        if (a.fused) {
+            zhist_entropy_epilogue(a, item, sh_hist, sh_pb, sh_red);
+        } else {
+            // write the item's whole global histogram (un-ranking the fixed bin): counted rows from
+            // shared memory (re-zeroed for the next item), rows of the rare ranks as zeros --
+            // zrare_kernel adds their voxels afterwards.  No other CTA touches this histogram, so
+            // plain stores suffice.
+            uint32_t* gh = a.hist + (size_t)item * a.nb * a.nb;
+            for (int r = warp; r < (int)nb; r += nwarps) {
+                uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
+                const bool real = r < a.rows_real;
+                for (unsigned b = lane; b < nb; b += 32) {
+                    uint32_t v = 0u;
+                    if (real) {
+                        v = sh_hist[r * pitch + b];
+                        if (v) sh_hist[r * pitch + b] = 0u;
+                    }
+                    grow[b] = v;
+                }
             }
         }
         if (a.rows_real < rows_smem)   // the dump row is only re-zeroed
-            for (unsigned b = threadIdx.x; b < nb; b += blockDim.x) sh_hist[a.rows_real * pitch + b] = 0u;
+            for (unsigned b = threadIdx.x; b <= nb; b += blockDim.x) sh_hist[a.rows_real * pitch + b] = 0u;
         __syncthreads();
     }
 }
@@ -420,7 +582,7 @@ __global__ void __launch_bounds__(256) zrare_kernel(const __grid_constant__ ZHis
             } else {
                 const float* xy = static_cast<const float*>(a.xy);
                 const float v = lerp_rn(xy[base], xy[base + a.colpitch], sz.w);
-                b = bin_u8(__fmul_rn(__fsub_rn(v, a.mlo), a.mscale), top);
+                b = bin_u8(a.bin_mode == kBinFastPrescaled ? v : __fmul_rn(__fsub_rn(v, a.mlo), a.mscale), top);
             }
             atomicAdd(&gh[(size_t)__ldg(a.rank_inv + rank) * a.nb + b], 1u);
         }
@@ -450,20 +612,21 @@ cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, 
 
 cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
                          const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
-                         void* XY, uint8_t* colvalid, cudaStream_t s) {
+                         float prescale, void* XY, uint8_t* colvalid, cudaStream_t s) {
     dim3 grid((colpitch / 4 + 127) / 128, npairs);
     if (nn)
         ypass_kernel<true, uint8_t><<<grid, 128, 0, s>>>(static_cast<const uint8_t*>(X), planes, prows, mnx, mny, ax,
-                                                        ay, a0, n1, fnx, cols, colpitch, static_cast<uint8_t*>(XY),
-                                                        colvalid);
+                                                        ay, a0, n1, fnx, cols, colpitch, 1.0f,
+                                                        static_cast<uint8_t*>(XY), colvalid);
     else
         ypass_kernel<false, float><<<grid, 128, 0, s>>>(static_cast<const float*>(X), planes, prows, mnx, mny, ax, ay,
-                                                       a0, n1, fnx, cols, colpitch, static_cast<float*>(XY), colvalid);
+                                                       a0, n1, fnx, cols, colpitch, prescale, static_cast<float*>(XY),
+                                                       colvalid);
     return cudaGetLastError();
 }
 
-// Histogram rows (of `pitch` words) of the z kernel that fit in shared memory, the dump row included
-// (at most nb + 1).
+// Histogram rows (of `pitch` words) of the z kernel that fit in shared memory beside its tables,
+// the dump row included (at most nb + 1).
 int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin) {
     const size_t reserve = 1024 + 4 * (size_t)zhist_table_words(fnz, planes);
     size_t rows = (smem_optin > reserve ? smem_optin - reserve : 0) / ((size_t)pitch * sizeof(uint32_t));
@@ -471,9 +634,9 @@ int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin
     return (int)rows;
 }
 
-template <bool NN, int COLS, bool FAST>
+template <bool NN, int MODE>
 static cudaError_t launch_zhist_t(const ZHistArgs& a, unsigned grid, size_t smem, cudaStream_t s) {
-    auto kern = zhist_kernel<NN, COLS, FAST>;
+    auto kern = zhist_kernel<NN, MODE>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kHistThreads, smem, s>>>(a);
@@ -481,20 +644,19 @@ static cudaError_t launch_zhist_t(const ZHistArgs& a, unsigned grid, size_t smem
 }
 
 cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t s) {
-    if (a.rows_smem < 1 || a.pitch < a.nb || (a.colpitch % a.cols) != 0) return cudaErrorInvalidConfiguration;
+    if (a.rows_smem < 1 || a.pitch < a.nb + 1 || (a.colpitch % kZColAlign) != 0 || a.nb > 256)
+        return cudaErrorInvalidConfiguration;
+    if (a.fused && (a.n_rare > 0 || a.nq > kMaxQPerPass || a.mi_out == nullptr)) return cudaErrorInvalidConfiguration;
     const size_t smem = 4 * (size_t)zhist_table_words(a.fnz, a.planes) + (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
     const long long nitems = (long long)a.n_pairs * a.n2;
     long long grid = nitems < num_sms ? nitems : num_sms;
     if (grid < 1) return cudaSuccess;
     cudaError_t e;
     const unsigned g = (unsigned)grid;
-    if (nn) {
-        e = a.cols == 8 ? launch_zhist_t<true, 8, false>(a, g, smem, s) : launch_zhist_t<true, 4, false>(a, g, smem, s);
-    } else if (a.fast_bin) {
-        e = a.cols == 8 ? launch_zhist_t<false, 8, true>(a, g, smem, s) : launch_zhist_t<false, 4, true>(a, g, smem, s);
-    } else {
-        e = a.cols == 8 ? launch_zhist_t<false, 8, false>(a, g, smem, s) : launch_zhist_t<false, 4, false>(a, g, smem, s);
-    }
+    if (nn) e = launch_zhist_t<true, kBinGeneral>(a, g, smem, s);
+    else if (a.bin_mode == kBinFastPrescaled) e = launch_zhist_t<false, kBinFastPrescaled>(a, g, smem, s);
+    else if (a.bin_mode == kBinFast) e = launch_zhist_t<false, kBinFast>(a, g, smem, s);
+    else e = launch_zhist_t<false, kBinGeneral>(a, g, smem, s);
     if (e != cudaSuccess) return e;
     if (a.n_rare > 0) {
         long long g2 = nitems < 8LL * num_sms ? nitems : 8LL * num_sms;

@@ -302,18 +302,27 @@ def test_separable_path_equals_generic_path_bitwise(mi, name, kw):
     IDENTICAL doubles: the entropy kernel is deterministic, so equal maps <=> equal histograms."""
     cfg = ph.get_config(name, **kw)
     for interp in (0, 1):
-        ms, ams = gpu_map(mi, cfg, interp)
         mg, amg = gpu_map(mi, cfg, interp, MI_B200_SEPARABLE=0)
-        assert np.array_equal(ms, mg), np.max(np.abs(ms - mg))
-        assert np.array_equal(ams, amg)
+        # histograms written out and reduced by the same entropy kernel as the generic path; every
+        # moving-side binning variant of the z kernel (general / no clamps / pre-scaled planes)
+        for mode in (0, 1, 2):
+            ms, ams = gpu_map(mi, cfg, interp, MI_B200_FUSE_ENTROPY=0, MI_B200_BIN_MODE=mode)
+            assert np.array_equal(ms, mg), (mode, np.max(np.abs(ms - mg)))
+            assert np.array_equal(ams, amg)
+        # default: entropies computed in the z kernel's epilogue (another summation order)
+        mf, amf = gpu_map(mi, cfg, interp)
+        assert np.max(np.abs(mf - mg)) <= 1e-9, np.max(np.abs(mf - mg))
+        assert np.array_equal(amf, amg)
 
 
 def test_separable_batches_rare_rows_and_odd_grids(mi):
     cfg = ph.get_config("C5", res=0.25, grid_n=5)
     ref, _ = gpu_map(mi, cfg, 1, MI_B200_SEPARABLE=0)
     # tiny scratch budgets: one p0 per batch, several batches
-    m, _ = gpu_map(mi, cfg, 1, MI_B200_XY_BUDGET_MB=8, MI_B200_SEP_HIST_BUDGET_MB=8)
+    m, _ = gpu_map(mi, cfg, 1, MI_B200_XY_BUDGET_MB=8, MI_B200_SEP_HIST_BUDGET_MB=8, MI_B200_FUSE_ENTROPY=0)
     assert np.array_equal(m, ref)
+    m, _ = gpu_map(mi, cfg, 1, MI_B200_XY_BUDGET_MB=8)
+    assert np.max(np.abs(m - ref)) <= 1e-9
     # only 40 of 256 fixed-bin rows in shared memory: most voxels go through the rare-voxel kernel
     for interp in (0, 1):
         ref, _ = gpu_map(mi, cfg, interp, MI_B200_SEPARABLE=0)
@@ -330,6 +339,30 @@ def test_separable_batches_rare_rows_and_odd_grids(mi):
         ms, _ = gpu_map(mi, c, interp)
         mg, _ = gpu_map(mi, c, interp, MI_B200_SEPARABLE=0)
         assert np.array_equal(ms, mg)
+
+
+def test_separable_binning_variants_and_range_edges(mi):
+    """The z kernel's moving-side binning variants against the oracle: power-of-two bin scale
+    (pre-scaled planes), other scales (no clamps), and the general sequence (moving_lo != 0 or voxels
+    outside the range).  Voxels exactly equal to moving_hi land in the last bin (pad column nb of the
+    clamp-free variants); more than kMaxQPerPass orders fall back to the separate entropy kernel."""
+    fixed = ph.random_volume((37, 21, 13), 41)
+    moving = ph.random_volume((30, 25, 17), 42).copy()
+    moving.reshape(-1)[::7] = 1.0
+    moving.reshape(-1)[3::11] = 0.0
+    cases = [(256, (0, 1, 0, 1), (0.5, 2.0)),            # scale 256: pre-scaled planes
+             (100, (0, 1, 0, 1), (0.5,)),                # scale 100: clamp-free, multiplied per sample
+             (64, (0, 1, 0.1, 0.9), (2.0,)),             # moving_lo != 0, voxels outside the range
+             (64, (0, 1, 0, 0.5), ()),                   # voxels above moving_hi
+             (128, (0, 1, 0, 1), (0.2, 0.5, 0.8, 0.9, 1.0, 1.1, 1.5, 2.0, 3.0))]   # nine orders: two entropy passes
+    for nb, ranges, q in cases:
+        c = ph.Config("edges", fixed, moving, (1.0, 1.2, 0.9), (1.1, 1.0, 1.3), nb, 0, (-2.5, 0.3, -1.7), (2.5, 0.3, 1.7),
+                      (3, 1, 3), q, (0, 0, 0), ranges)
+        for interp in (0, 1):
+            check_map(mi, c, interp)
+            ms, _ = gpu_map(mi, c, interp, MI_B200_FUSE_ENTROPY=0)
+            mg, _ = gpu_map(mi, c, interp, MI_B200_SEPARABLE=0)
+            assert np.array_equal(ms, mg)
 
 
 def test_scale_maps_with_plane_skips_and_negative_factors(mi):
