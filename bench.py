@@ -30,6 +30,9 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+# bytes per launch of the dominant kernel, from the committed ncu capture of the default command
+NCU_DRAM_BYTES_PER_LAUNCH = {}
+
 METRIC = "voxel-transform evaluations per second (MI map, 260x311x260 fixed, 256 bins)"
 UNIT = "evals/s"
 
@@ -245,17 +248,19 @@ def main():
     if rank == 0:
         sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    kern_ms = np.zeros(4)
+    kern_ms = np.zeros(5)
     launches = 0
+    hist_launches = 0
     wall0 = time.perf_counter()
     for k in range(args.steps):
         flush.fill_(k & 0xFF)
         ev[k][0].record()
         step()
         ev[k][1].record()
-        ms4, ln4 = mi.mi_last_timing(ctx)
-        kern_ms += ms4
-        launches += int(ln4.sum())
+        ms5, ln5 = mi.mi_last_timing(ctx)
+        kern_ms += ms5
+        launches += int(ln5[:4].sum())      # class 4 (the dominant kernel alone) is a subset of class 1
+        hist_launches += int(ln5[4])
     barrier()
     wall = time.perf_counter() - wall0
     clocks = sampler.stop() if rank == 0 else None
@@ -303,8 +308,12 @@ def main():
     # north_star: t_roof = max(t_HBM, t_atom); one shared-memory histogram update per evaluation.
     r_rand = mi.mi_probe_shared_atomic_rate(local, cfg.nbins, 1, 8192)
     r_free = mi.mi_probe_shared_atomic_rate(local, cfg.nbins, 0, 8192)
-    hist_ms = kern_ms[1] / args.steps
-    hist_launches = max(1, launches // args.steps) if launches else 1
+    # dominant kernel: the z-lerp+histogram kernel (separable maps) or the generic resample+histogram
+    # kernel, timed alone with CUDA events on the launching stream (mi_last_timing class 4); one step
+    # launches it hist_launches times and together the launches do every evaluation of the step once
+    separable = cfg.family in (0, 3, 4)
+    hist_ms = kern_ms[4] / args.steps
+    hist_launches = max(1, hist_launches // args.steps)
     achieved = evals_step / (hist_ms * 1e-3)                        # updates/s inside the kernel
     pass_bytes = cfg.fixed.size * 1 + cfg.moving.size * 4          # fixed bins + moving floats, read once
     t_hbm_b1 = cfg.n_transforms * pass_bytes / (hbm_gbs * 1e9)
@@ -312,13 +321,20 @@ def main():
     t_atom = evals_step / r_rand
     sm_hz = (clocks["sm_mhz"] or sm_max_mhz) * 1e6
     t_lsu = 32.0 * evals_step / (148 * 128.0 * sm_hz)
-    roofline = {"bound": "alu", "kernel": "zhist_kernel<TRILINEAR> (separable path: x-pass, y-pass, z-lerp+histogram)",
+    # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel in this exact
+    # command (ncu --set full, profiles/r1e_ncu_zhist_c5_full.md); other workloads: not captured
+    traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((cfg.name, tuple(cfg.n), interp))
+    roofline = {"bound": "alu",
+                "kernel": ("zhist_kernel (separable path: z-lerp + joint histogram + fused entropy epilogue)" if separable
+                           else "resample_hist_kernel (generic affine: 8 gathers + 7 lerps + joint histogram)"),
                 "achieved": achieved / 1e9, "peak": r_rand / 1e9, "unit": "G shared-atomic updates/s",
-                "frac": achieved / r_rand, "traffic": None,
+                "frac": achieved / r_rand, "traffic": traffic,
+                "all_a3_a4_kernels_ms_per_step": kern_ms[1] / args.steps,
                 "peak_source": "mi_probe_shared_atomic_rate(pattern=uniform random bins) measured in this run",
                 "peak_conflict_free": r_free / 1e9,
                 "t_atom_ms": t_atom * 1e3, "t_hbm_resident_ms": t_hbm_once * 1e3,
-                "t_hbm_if_every_transform_restreams_ms": t_hbm_b1 * 1e3, "t_lsu_gather_ms": t_lsu * 1e3,
+                "t_hbm_if_every_transform_restreams_ms": t_hbm_b1 * 1e3,
+                "t_lsu_gather_nominal_ms": None if separable else t_lsu * 1e3,
                 "kernel_ms_per_step": hist_ms, "kernel_launches_per_step": hist_launches,
                 "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": peak_src,
                 "step_frac_of_t_roof": max(t_atom, t_hbm_once) / (total_ms / args.steps * 1e-3)}
@@ -337,7 +353,8 @@ def main():
                     "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3},
             "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "kernel_ms_per_step": {"setup": kern_ms[0] / args.steps, "resample_hist": kern_ms[1] / args.steps,
-                                   "entropy": kern_ms[2] / args.steps, "map": kern_ms[3] / args.steps},
+                                   "entropy": kern_ms[2] / args.steps, "map": kern_ms[3] / args.steps,
+                                   "dominant_hist_kernel": kern_ms[4] / args.steps},
             "wall_s_timed_region": wall}
     print(json.dumps(line))
     mi.mi_destroy(ctx)

@@ -115,8 +115,14 @@ mi_status mi_map(mi_ctx *ctx, mi_family family, const double lo[3], const double
                  const int32_t n[3], const double *q, int32_t nq, mi_interp interp,
                  double *map_out, int64_t *argmax_out);
 
-/* Release the context and its device memory.  NULL is a no-op. */
+/* Release the context.  Its device memory goes back to a library-level stream-ordered pool (one per
+ * device) that keeps it cached for the next context -- the multi-GB scratch of a map is then not
+ * mapped and unmapped by the driver on every create/destroy cycle.  NULL is a no-op. */
 void mi_destroy(mi_ctx *ctx);
+
+/* Return the memory cached by destroyed contexts on `device` to the driver.  Live contexts are not
+ * affected.  MI_ERR_INVALID_ARG for a device that does not exist. */
+mi_status mi_release_cached_memory(int32_t device);
 
 /* Text of the last failure on this context (ctx != NULL) or of the last failed mi_create on this
  * thread (ctx == NULL).  The string is owned by the library and valid until the next call. */
@@ -140,8 +146,11 @@ mi_status mi_get_bins(mi_ctx *ctx, int32_t which, uint8_t *out);
 
 /* Device milliseconds (CUDA events on the context's stream) spent in the kernels of the last
  * mi_eval_batch / mi_map call: ms[0] transform upload + setup, ms[1] resample+histogram kernels,
- * ms[2] entropy kernels, ms[3] map assembly + arg max; launches[k] = kernels launched per class. */
-mi_status mi_last_timing(const mi_ctx *ctx, float ms[4], int64_t launches[4]);
+ * ms[2] entropy kernels (0 when step a5 ran as the histogram kernel's epilogue), ms[3] map assembly +
+ * arg max, ms[4] the dominant histogram kernel alone (z-lerp+histogram kernel of the separable path,
+ * or the generic resample+histogram kernel; a part of ms[1]); launches[k] = kernels launched per
+ * class (launches[4] is a subset of launches[1]). */
+mi_status mi_last_timing(const mi_ctx *ctx, float ms[5], int64_t launches[5]);
 
 /* Shared-memory atomic rate probe for the roofline: runs `iters` rounds of
  * atomicAdd(u32) into an nbins x nbins table in shared memory on every SM and reports

@@ -26,7 +26,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
            4: "MI_ERR_CUDA", 5: "MI_ERR_INTERNAL"}
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
-           "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing",
+           "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
            "mi_probe_shared_atomic_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
@@ -54,6 +54,8 @@ _lib.mi_index_affine.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp]
 _lib.mi_index_affine.restype = C.c_int
 _lib.mi_get_bins.argtypes = [_vp, C.c_int32, _vp]
 _lib.mi_get_bins.restype = C.c_int
+_lib.mi_release_cached_memory.argtypes = [C.c_int32]
+_lib.mi_release_cached_memory.restype = C.c_int
 _lib.mi_last_timing.argtypes = [_vp, _vp, _vp]
 _lib.mi_last_timing.restype = C.c_int
 _lib.mi_probe_shared_atomic_rate.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
@@ -241,11 +243,18 @@ def mi_get_bins(ctx, which: int) -> np.ndarray:
 
 
 def mi_last_timing(ctx):
-    """(ms[4], launches[4]) of the last eval/map call: setup, resample+hist, entropy, map assembly."""
-    ms = np.zeros(4, dtype=np.float32)
-    ln = np.zeros(4, dtype=np.int64)
+    """(ms[5], launches[5]) of the last eval/map call: setup, resample+hist, entropy, map assembly, and
+    the dominant histogram kernel alone (a part of resample+hist)."""
+    ms = np.zeros(5, dtype=np.float32)
+    ln = np.zeros(5, dtype=np.int64)
     _check(ctx, _lib.mi_last_timing(ctx.handle, _ptr(ms), _ptr(ln)))
     return ms, ln
+
+
+def mi_release_cached_memory(device=0) -> None:
+    st = _lib.mi_release_cached_memory(int(device))
+    if st != MI_OK:
+        raise MIError(st, "mi_release_cached_memory")
 
 
 def mi_probe_shared_atomic_rate(device=0, nbins=256, pattern=1, iters=4096) -> float:

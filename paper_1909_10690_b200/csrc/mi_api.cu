@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -27,7 +28,9 @@ struct mi_ctx {
     int* d_rank_inv = nullptr;          // 256: rank -> fixed bin
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
-    int rows_smem = 0;
+    int rows_smem = 0;                  // generic kernel: ranked fixed-bin rows in shared memory
+    int gpitch = 0;                     // generic kernel: words per shared histogram row
+    int ty_log2 = 3;                    // generic kernel: row tile = 8 (y) x 4 (z)
     // separable path (diagonal-matrix families)
     uint8_t* d_fb_pitched = nullptr;    // ranked fixed bins, [fnz][colpitch]
     int colpitch = 0;                   // fny*fnx rounded up to a multiple of kZColAlign
@@ -63,13 +66,52 @@ struct mi_ctx {
     bool staging_busy = false;
 
     std::string err;
-    float last_ms[4] = {0, 0, 0, 0};
-    int64_t last_launches[4] = {0, 0, 0, 0};
+    float last_ms[5] = {0, 0, 0, 0, 0};
+    int64_t last_launches[5] = {0, 0, 0, 0, 0};
 };
 
 namespace {
 
 thread_local std::string g_create_error;
+
+// Device memory comes from one library-level stream-ordered pool per device whose release threshold
+// is unbounded: what a destroyed context frees stays cached for the next one (the multi-GB scratch of
+// a map would otherwise be mapped and unmapped by the driver on every mi_create / mi_destroy cycle),
+// until mi_release_cached_memory() trims it.
+std::mutex g_pool_mutex;
+cudaMemPool_t g_pools[64] = {};
+
+cudaError_t device_pool(int dev, cudaMemPool_t* out) {
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pools[dev] == nullptr) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        cudaError_t e = cudaMemPoolCreate(&pool, &props);
+        if (e != cudaSuccess) return e;
+        unsigned long long keep = ~0ULL;
+        e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return e; }
+        g_pools[dev] = pool;
+    }
+    *out = g_pools[dev];
+    return cudaSuccess;
+}
+
+// Stream-ordered allocation on the context's stream (every use of the memory is ordered on it too).
+cudaError_t dev_alloc(void** p, size_t bytes, int dev, cudaStream_t s) {
+    cudaMemPool_t pool = nullptr;
+    cudaError_t e = device_pool(dev, &pool);
+    if (e != cudaSuccess) return e;
+    return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, s);
+}
+void dev_free(void* p, cudaStream_t s) {
+    if (p) cudaFreeAsync(p, s);
+}
 
 struct DeviceGuard {
     int prev = -1;
@@ -110,8 +152,8 @@ bool is_host_ptr(const void* p) {
 template <typename T>
 mi_status grow(mi_ctx* c, T** p, size_t* cap, size_t need) {
     if (need <= *cap) return MI_OK;
-    if (*p) { cudaFree(*p); *p = nullptr; *cap = 0; }
-    MI_CUDA(c, cudaMalloc(reinterpret_cast<void**>(p), need * sizeof(T)));
+    if (*p) { dev_free(*p, c->stream); *p = nullptr; *cap = 0; }
+    MI_CUDA(c, dev_alloc(reinterpret_cast<void**>(p), need * sizeof(T), c->device, c->stream));
     *cap = need;
     return MI_OK;
 }
@@ -122,6 +164,7 @@ struct EventTimer {
     // accumulates device time per class over a call; events are recorded on the context's stream
     struct Span { cudaEvent_t a, b; int cls; };
     std::vector<Span> spans;
+    std::vector<size_t> open;   // spans may nest (class 4 inside class 1)
     cudaStream_t s;
     explicit EventTimer(cudaStream_t st) : s(st) {}
     void begin(int cls) {
@@ -129,10 +172,14 @@ struct EventTimer {
         cudaEventCreate(&sp.a);
         cudaEventCreate(&sp.b);
         cudaEventRecord(sp.a, s);
+        open.push_back(spans.size());
         spans.push_back(sp);
     }
-    void end() { cudaEventRecord(spans.back().b, s); }
-    void collect(float ms[4]) {
+    void end() {
+        cudaEventRecord(spans[open.back()].b, s);
+        open.pop_back();
+    }
+    void collect(float ms[5]) {
         for (auto& sp : spans) {
             float t = 0.f;
             if (cudaEventSynchronize(sp.b) == cudaSuccess && cudaEventElapsedTime(&t, sp.a, sp.b) == cudaSuccess)
@@ -283,8 +330,11 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
         z.mi_out = c->d_mi;
         z.nvalid = c->d_nvalid;
         z.om = mi::OutMap{1, n0, n1, n2, a0};
+        timer.begin(4);
         MI_CUDA(c, mi::launch_zhist(nn, z, c->num_sms, s));
+        timer.end();
         c->last_launches[1] += 3 + (c->n_rare > 0 ? 1 : 0);
+        c->last_launches[4] += 1;
         timer.end();
         if (fused) continue;
 
@@ -311,7 +361,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     const int nch = 1 + nq;
     const size_t nbins2 = (size_t)c->nb * c->nb;
     cudaStream_t s = c->stream;
-    for (int k = 0; k < 4; ++k) { c->last_ms[k] = 0.f; c->last_launches[k] = 0; }
+    for (int k = 0; k < 5; ++k) { c->last_ms[k] = 0.f; c->last_launches[k] = 0; }
     EventTimer timer(s);
 
     // ---- setup: scratch + upload of transforms and q -------------------------------------------
@@ -362,6 +412,8 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.moving_pad = c->d_moving_pad;
         a.mbins = c->d_mbins;
         a.rows_smem = c->rows_smem;
+        a.pitch = c->gpitch;
+        a.ty_log2 = c->ty_log2;
         a.M = c->d_M + (size_t)off * 12;
         a.hist = hist;
         a.f = {c->fd[0], c->fd[1], c->fd[2]};
@@ -371,7 +423,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.mscale = c->mscale;
         a.n_transforms = (int)cnt;
         // CTAs per transform: one when there are many transforms; otherwise split the volume into
-        // row slabs so that about 16 waves of CTAs exist (each slab keeps >= 64 rows).
+        // slabs of 32-row tiles so that about 16 waves of CTAs exist (each slab keeps >= 2 tiles).
         int nslabs = 1;
         const int64_t want = 16LL * c->num_sms;
         if (cnt < want) {
@@ -380,8 +432,11 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             if (nslabs > cap) nslabs = cap;
         }
         a.nslabs = nslabs;
+        timer.begin(4);
         MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, s));
+        timer.end();
         c->last_launches[1] += 1;
+        c->last_launches[4] += 1;
         timer.end();
 
         timer.begin(2);
@@ -529,24 +584,32 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         c->fscale = mi::bin_scale(nbins, fixed_lo, fixed_hi);
         c->mscale = mi::bin_scale(nbins, moving_lo, moving_hi);
         // +16 bytes of slack so 16-byte vector stores of the last partial group stay inside
-        if ((e = cudaMalloc((void**)&c->d_fbins, (size_t)nf + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc fixed bins"); break; }
-        if ((e = cudaMalloc((void**)&c->d_mbins, (size_t)nm + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bins"); break; }
-        if ((e = cudaMalloc((void**)&c->d_fbins_ranked, (size_t)nf + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc ranked bins"); break; }
-        if ((e = cudaMalloc((void**)&c->d_rank, 256)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank"); break; }
-        if ((e = cudaMalloc((void**)&c->d_rank_inv, 256 * sizeof(int))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank_inv"); break; }
-        if ((e = cudaMalloc((void**)&d_counts, 256 * sizeof(unsigned long long))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc counts"); break; }
-        if ((e = cudaMalloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
-        if ((e = cudaMalloc((void**)&d_mov, (size_t)nm * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
-        if ((e = cudaMalloc((void**)&d_tmp, (size_t)nf * sizeof(float))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
+        if ((e = dev_alloc((void**)&c->d_fbins, (size_t)nf + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc fixed bins"); break; }
+        if ((e = dev_alloc((void**)&c->d_mbins, (size_t)nm + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bins"); break; }
+        if ((e = dev_alloc((void**)&c->d_fbins_ranked, (size_t)nf + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc ranked bins"); break; }
+        if ((e = dev_alloc((void**)&c->d_rank, 256, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank"); break; }
+        if ((e = dev_alloc((void**)&c->d_rank_inv, 256 * sizeof(int), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank_inv"); break; }
+        if ((e = dev_alloc((void**)&d_counts, 256 * sizeof(unsigned long long), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc counts"); break; }
+        if ((e = dev_alloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
+        if ((e = dev_alloc((void**)&d_mov, (size_t)nm * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
+        if ((e = dev_alloc((void**)&d_tmp, (size_t)nf * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
         c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + mi::kZColAlign - 1) / mi::kZColAlign * mi::kZColAlign);
-        if ((e = cudaMalloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
+        if ((e = dev_alloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
         // bank of histogram word (a, b) = (a*pad + b) mod 32: an odd pad walks the rows over all banks
         int zpad = 9;
         if (const char* v = std::getenv("MI_B200_HIST_PAD")) { const int r = std::atoi(v); if (r >= 1 && r <= 64) zpad = r; }
         if (const char* v = std::getenv("MI_B200_FUSE_ENTROPY")) c->fuse_entropy = std::atoi(v) != 0;
         c->zpitch = nbins + zpad;
         c->zrows_smem = mi::zhist_rows_in_smem(nbins, c->zpitch, fixed_dims[2], moving_dims[2] + 2, c->smem_optin);
-        c->rows_smem = mi::hist_rows_in_smem(nbins, c->smem_optin);
+        // generic kernel: the gathers live in L1, which is what the shared histogram leaves of the
+        // SM's 256 KB; above 196 KB of shared memory the next carve-out step leaves only 28 KB
+        int gpad = 5;
+        size_t gsmem = c->smem_optin < (size_t)196 * 1024 ? c->smem_optin : (size_t)196 * 1024;
+        if (const char* v = std::getenv("MI_B200_GENERIC_PAD")) { const int r = std::atoi(v); if (r >= 0 && r <= 64) gpad = r; }
+        if (const char* v = std::getenv("MI_B200_GENERIC_SMEM_KB")) { const size_t r = (size_t)std::atoll(v) << 10; if (r >= 8192 && r <= c->smem_optin) gsmem = r; }
+        if (const char* v = std::getenv("MI_B200_GENERIC_TY")) { const int r = std::atoi(v); if (r >= 0 && r <= 5) c->ty_log2 = r; }
+        c->gpitch = nbins + gpad;
+        c->rows_smem = mi::hist_rows_in_smem(nbins, c->gpitch, gsmem);
         // test knobs (tests/ shrink the scratch budgets to force several batches, or disable the path)
         if (const char* v = std::getenv("MI_B200_SEPARABLE")) c->use_separable = std::atoi(v) != 0;
         if (const char* v = std::getenv("MI_B200_XY_BUDGET_MB")) c->xy_budget = (size_t)std::atoll(v) << 20;
@@ -585,7 +648,7 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             for (int a = 0; a < 256; ++a)
                 if ((int)h_rank[a] >= c->zrows_real) n_rare += h_counts[a];
             c->n_rare = (unsigned)n_rare;
-            if ((e = cudaMalloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2))) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
+            if ((e = dev_alloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
             if ((e = cudaMemsetAsync(d_counts, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
             if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
                                            c->d_fb_pitched, c->d_rare, reinterpret_cast<unsigned*>(d_counts), c->n_rare, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pitch fixed bins"); break; }
@@ -593,9 +656,9 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
-    if (d_tmp) cudaFree(d_tmp);
-    if (d_mov) cudaFree(d_mov);
-    if (d_counts) cudaFree(d_counts);
+    dev_free(d_tmp, c->stream);
+    dev_free(d_mov, c->stream);
+    dev_free(d_counts, c->stream);
     if (st != MI_OK) {
         mi_destroy(c);
         return st;
@@ -608,17 +671,26 @@ void mi_destroy(mi_ctx* c) {
     if (!c) return;
     DeviceGuard guard(c->device);
     if (guard.ok) {
+        void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mbins,
+                        c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
+                        c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
+        for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);
-        cudaFree(c->d_fbins); cudaFree(c->d_fbins_ranked); cudaFree(c->d_rank); cudaFree(c->d_rank_inv);
-        cudaFree(c->d_moving_pad); cudaFree(c->d_mbins); cudaFree(c->d_fb_pitched); cudaFree(c->d_rare);
-        cudaFree(c->d_X); cudaFree(c->d_XY); cudaFree(c->d_colvalid); cudaFree(c->d_axis);
-        cudaFree(c->d_M); cudaFree(c->d_hist); cudaFree(c->d_mi); cudaFree(c->d_nvalid);
-        cudaFree(c->d_q); cudaFree(c->d_map); cudaFree(c->d_argmax);
         if (c->h_M) cudaFreeHost(c->h_M);
         if (c->ev_staging) cudaEventDestroy(c->ev_staging);
         cudaGetLastError();
     }
     delete c;
+}
+
+mi_status mi_release_cached_memory(int32_t device) {
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
+    if (device < 0 || device >= ndev || device >= 64) return MI_ERR_INVALID_ARG;
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
+    if (g_pools[device] == nullptr) return MI_OK;
+    if (cudaMemPoolTrimTo(g_pools[device], 0) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
+    return MI_OK;
 }
 
 mi_status mi_set_tsallis_form(mi_ctx* c, mi_tsallis_form form) {
@@ -715,9 +787,9 @@ mi_status mi_get_bins(mi_ctx* c, int32_t which, uint8_t* out) {
     return MI_OK;
 }
 
-mi_status mi_last_timing(const mi_ctx* c, float ms[4], int64_t launches[4]) {
+mi_status mi_last_timing(const mi_ctx* c, float ms[5], int64_t launches[5]) {
     if (!c) return MI_ERR_INVALID_ARG;
-    for (int k = 0; k < 4; ++k) {
+    for (int k = 0; k < 5; ++k) {
         if (ms) ms[k] = c->last_ms[k];
         if (launches) launches[k] = c->last_launches[k];
     }

@@ -31,11 +31,13 @@ struct ResampleArgs {
     const float* M;               // n_transforms x 12 index-space affines (device)
     uint32_t* hist;               // n_transforms x nb x nb (row = fixed bin), zero on entry
     int rows_smem;                // ranked fixed-bin rows kept in shared memory
+    int pitch;                    // words per shared histogram row (>= nb)
+    int ty_log2;                  // the CTA's 32 warps cover 2^ty_log2 (y) x 32/2^ty_log2 (z) fixed rows at a time
     VolumeDesc f, m;
     int nb;
     float mlo, mscale;       // moving binning (CANON-5)
     int n_transforms;
-    int nslabs;              // CTAs cooperating on one transform (row slabs)
+    int nslabs;              // CTAs cooperating on one transform (slabs of row tiles)
 };
 
 // flag (may be NULL): set to 1 if any voxel is negative, not finite or above the last bin edge
@@ -44,7 +46,7 @@ cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, 
 cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s);
 cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
                                    uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s);
-int hist_rows_in_smem(int nb, size_t smem_optin);
+int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes);
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s);
 // Where the entropy kernel writes the result of histogram `item`: transform-major position item
 // (enabled == 0) or, for the separable path whose items are ordered (p0, p1, p2) with p2 fastest,

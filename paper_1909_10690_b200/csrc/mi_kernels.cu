@@ -264,7 +264,8 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     const int nb = a.nb;
     const int nbins2 = nb * nb;
     const int rows_smem = a.rows_smem;
-    const int words = rows_smem * nb;
+    const int pitch = a.pitch;   // words per shared row; bank = (a*(pitch-nb) + b) mod 32
+    const int words = rows_smem * pitch;
     for (int w = threadIdx.x; w < words; w += blockDim.x) sh_hist[w] = 0u;
     __syncthreads();
 
@@ -272,7 +273,13 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     const int warp = threadIdx.x >> 5;
     const int nwarps = blockDim.x >> 5;
     const int fnx = a.f.nx;
-    const int rows_total = a.f.ny * a.f.nz;
+    // The 32 warps of the CTA take the rows of one (2^ty_log2 y) x (32 >> ty_log2 z) tile of fixed rows
+    // at a time, so that the 2x2x2 stencils of neighbouring rows in y AND z hit the same L1 sectors.
+    const int ty_log2 = a.ty_log2;
+    const int wy = warp & ((1 << ty_log2) - 1), wz = warp >> ty_log2;
+    const int tiles_y = (a.f.ny + (1 << ty_log2) - 1) >> ty_log2;
+    const int tz_rows = 32 >> ty_log2;
+    const int tiles_total = tiles_y * ((a.f.nz + tz_rows - 1) / tz_rows);
 
     MovingView mv;
     mv.pnx = a.m.nx + 2; mv.pny = a.m.ny + 2;
@@ -293,16 +300,19 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int t = (int)(item / a.nslabs);
         const int slab = (int)(item - (long long)t * a.nslabs);
-        const int row_lo = (int)((long long)rows_total * slab / a.nslabs);
-        const int row_hi = (int)((long long)rows_total * (slab + 1) / a.nslabs);
+        const int tile_lo = (int)((long long)tiles_total * slab / a.nslabs);
+        const int tile_hi = (int)((long long)tiles_total * (slab + 1) / a.nslabs);
         float m[12];
 #pragma unroll
         for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
         uint32_t* gh = a.hist + (size_t)t * nbins2;
 
-        for (int row = row_lo + warp; row < row_hi; row += nwarps) {
-            const int iz = row / a.f.ny;
-            const int iy = row - iz * a.f.ny;
+        for (int tile = tile_lo; tile < tile_hi; ++tile) {
+            const int tz = tile / tiles_y;
+            const int iy = ((tile - tz * tiles_y) << ty_log2) + wy;
+            const int iz = tz * tz_rows + wz;
+            if (iy >= a.f.ny || iz >= a.f.nz) continue;
+            const int row = iz * a.f.ny + iy;
             const float fy = (float)iy, fz = (float)iz;
             // CANON-2: row terms, then one fma per voxel and axis
             const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
@@ -326,7 +336,7 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
 #pragma unroll
                 for (int u = 0; u < UNROLL; ++u) {
                     if (smp[u].ok) {
-                        if (fa[u] < rows_smem) atomicAdd(&sh_hist[fa[u] * nb + smp[u].b], 1u);
+                        if (fa[u] < rows_smem) atomicAdd(&sh_hist[fa[u] * pitch + smp[u].b], 1u);
                         else atomicAdd(&gh[__ldg(a.rank_inv + fa[u]) * nb + smp[u].b], 1u);
                     }
                 }
@@ -338,9 +348,9 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
         for (int r = warp; r < rows_smem; r += nwarps) {
             uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
             for (int b = lane; b < nb; b += 32) {
-                const uint32_t v = sh_hist[r * nb + b];
+                const uint32_t v = sh_hist[r * pitch + b];
                 if (v) {
-                    sh_hist[r * nb + b] = 0u;
+                    sh_hist[r * pitch + b] = 0u;
                     atomicAdd(&grow[b], v);
                 }
             }
@@ -351,9 +361,16 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
 
 template <int INTERP, int UNROLL>
 static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStream_t s) {
-    const size_t smem = (size_t)a.rows_smem * a.nb * sizeof(uint32_t);
+    const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
     auto kern = resample_hist_kernel<INTERP, UNROLL>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    // leave the rest of the SM's 256 KB to L1 (the gathers live there)
+    // (a hint in percent of 228 KB, rounded down: the driver picks the smallest carve-out that still
+    // holds the CTA's shared memory + 1 KB)
+    int carve = (int)((smem + 1024) * 100 / (228 * 1024));
+    if (carve > 100) carve = 100;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
     if (e != cudaSuccess) return e;
     const long long nitems = (long long)a.n_transforms * a.nslabs;
     long long grid = nitems < num_sms ? nitems : num_sms;
@@ -362,15 +379,15 @@ static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStr
     return cudaGetLastError();
 }
 
-int hist_rows_in_smem(int nb, size_t smem_optin) {
+int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes) {
     const size_t reserve = 1024;  // static shared memory + alignment slack
-    size_t rows = (smem_optin > reserve ? smem_optin - reserve : 0) / ((size_t)nb * sizeof(uint32_t));
+    size_t rows = (smem_bytes > reserve ? smem_bytes - reserve : 0) / ((size_t)pitch * sizeof(uint32_t));
     if (rows > (size_t)nb) rows = (size_t)nb;
     return (int)rows;
 }
 
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s) {
-    if (a.rows_smem < 1) return cudaErrorInvalidConfiguration;
+    if (a.rows_smem < 1 || a.pitch < a.nb || a.ty_log2 < 0 || a.ty_log2 > 5) return cudaErrorInvalidConfiguration;
     if (interp == MI_INTERP_NEAREST) return launch_resample_t<MI_INTERP_NEAREST, 4>(a, num_sms, s);
     return launch_resample_t<MI_INTERP_TRILINEAR, 2>(a, num_sms, s);
 }

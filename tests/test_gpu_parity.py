@@ -268,6 +268,28 @@ def test_c5_full_size_sampled_against_oracle(mi):
             assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
 
 
+def test_context_cycles_reuse_the_pool_and_release(mi):
+    """Destroyed contexts hand their memory to the library's pool; results do not depend on what
+    an earlier context left in it, and mi_release_cached_memory gives it back."""
+    import torch
+    cfg = ph.get_config("C1")
+    first = None
+    for it in range(3):
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+            m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        first = m if first is None else first
+        assert np.array_equal(m, first)
+    free0, _ = torch.cuda.mem_get_info()
+    mi.mi_release_cached_memory(0)
+    free1, _ = torch.cuda.mem_get_info()
+    assert free1 >= free0
+    with pytest.raises(mi.MIError):
+        mi.mi_release_cached_memory(9999)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        m, _ = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+    assert np.array_equal(m, first)
+
+
 # ------------------------------------------------------------------------------------------------ separable path
 class env:
     """Set MI_B200_* knobs (read by mi_create) for the duration of a with-block."""
