@@ -30,8 +30,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-# bytes per launch of the dominant kernel, from the committed ncu capture of the default command
-NCU_DRAM_BYTES_PER_LAUNCH = {}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (4 of the 41 p0
+# slabs = 6724 transforms = 1.414e11 evaluations), from the committed ncu --set full capture of the
+# default command (profiles/r1e_ncu_zhist_resample.md); keyed by (config, grid, interpolation)
+NCU_DRAM_BYTES_PER_LAUNCH = {("C5", (41, 41, 41), 1): 16265455000 + 552631552}
 
 METRIC = "voxel-transform evaluations per second (MI map, 260x311x260 fixed, 256 bins)"
 UNIT = "evals/s"
@@ -321,8 +323,8 @@ def main():
     t_atom = evals_step / r_rand
     sm_hz = (clocks["sm_mhz"] or sm_max_mhz) * 1e6
     t_lsu = 32.0 * evals_step / (148 * 128.0 * sm_hz)
-    # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel in this exact
-    # command (ncu --set full, profiles/r1e_ncu_zhist_c5_full.md); other workloads: not captured
+    # measured DRAM bytes of one launch of the dominant kernel in this exact command; null for the
+    # workloads that have no committed capture
     traffic = NCU_DRAM_BYTES_PER_LAUNCH.get((cfg.name, tuple(cfg.n), interp))
     roofline = {"bound": "alu",
                 "kernel": ("zhist_kernel (separable path: z-lerp + joint histogram + fused entropy epilogue)" if separable
