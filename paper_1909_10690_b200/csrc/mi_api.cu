@@ -70,9 +70,7 @@ struct mi_ctx {
     int64_t last_launches[5] = {0, 0, 0, 0, 0};
 };
 
-namespace {
-
-thread_local std::string g_create_error;
+namespace mi {
 
 // Device memory comes from one library-level stream-ordered pool per device whose release threshold
 // is unbounded: what a destroyed context frees stays cached for the next one (the multi-GB scratch of
@@ -113,6 +111,24 @@ void dev_free(void* p, cudaStream_t s) {
     if (p) cudaFreeAsync(p, s);
 }
 
+thread_local std::string g_thread_error;
+void set_thread_error(const std::string& msg) { g_thread_error = msg; }
+bool is_host_pointer(const void* p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return true;
+    }
+    return !(at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
+}
+
+}  // namespace mi
+
+namespace {
+
+using mi::dev_alloc;
+using mi::dev_free;
+
 struct DeviceGuard {
     int prev = -1;
     bool ok = false;
@@ -126,7 +142,7 @@ struct DeviceGuard {
 };
 
 mi_status fail(mi_ctx* c, mi_status s, const std::string& msg) {
-    if (c) c->err = msg; else g_create_error = msg;
+    if (c) c->err = msg; else mi::set_thread_error(msg);
     return s;
 }
 mi_status cuda_fail(mi_ctx* c, cudaError_t e, const char* where) {
@@ -140,14 +156,7 @@ mi_status cuda_fail(mi_ctx* c, cudaError_t e, const char* where) {
         if (e__ != cudaSuccess) return cuda_fail((ctx), e__, #call); \
     } while (0)
 
-bool is_host_ptr(const void* p) {
-    cudaPointerAttributes at;
-    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
-        cudaGetLastError();
-        return true;
-    }
-    return !(at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged);
-}
+bool is_host_ptr(const void* p) { return mi::is_host_pointer(p); }
 
 template <typename T>
 mi_status grow(mi_ctx* c, T** p, size_t* cap, size_t need) {
@@ -502,7 +511,7 @@ extern "C" {
 
 const char* mi_version(void) { return "mi-b200 0.1 (sm_100a)"; }
 
-const char* mi_last_error(const mi_ctx* ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+const char* mi_last_error(const mi_ctx* ctx) { return ctx ? ctx->err.c_str() : mi::g_thread_error.c_str(); }
 
 mi_status mi_family_matrix(mi_family family, const double p[3], double T_out[12]) {
     if (p == nullptr || T_out == nullptr) return MI_ERR_INVALID_ARG;
@@ -687,9 +696,9 @@ mi_status mi_release_cached_memory(int32_t device) {
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
     if (device < 0 || device >= ndev || device >= 64) return MI_ERR_INVALID_ARG;
-    std::lock_guard<std::mutex> lock(g_pool_mutex);
-    if (g_pools[device] == nullptr) return MI_OK;
-    if (cudaMemPoolTrimTo(g_pools[device], 0) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
+    std::lock_guard<std::mutex> lock(mi::g_pool_mutex);
+    if (mi::g_pools[device] == nullptr) return MI_OK;
+    if (cudaMemPoolTrimTo(mi::g_pools[device], 0) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
     return MI_OK;
 }
 

@@ -4,9 +4,18 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <string>
+
 #include "mi.h"
 
 namespace mi {
+
+// ---- shared host runtime pieces (mi_api.cu) -----------------------------------------------------
+// stream-ordered allocation from the library's per-device pool / release back to it
+cudaError_t dev_alloc(void** p, size_t bytes, int dev, cudaStream_t s);
+void dev_free(void* p, cudaStream_t s);
+void set_thread_error(const std::string& msg);   // text behind mi_last_error(NULL)
+bool is_host_pointer(const void* p);
 
 constexpr int kMaxQPerPass = 8;      // Tsallis orders handled by one entropy-kernel pass
 constexpr int kHistThreads = 1024;   // resample+histogram CTA size
