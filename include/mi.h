@@ -128,6 +128,44 @@ mi_status mi_release_cached_memory(int32_t device);
  * thread (ctx == NULL).  The string is owned by the library and valid until the next call. */
 const char *mi_last_error(const mi_ctx *ctx);
 
+/* ---- capture-range analysis of a map ---------------------------------------
+ * The paper reads its maps through "the paths the gradient descent algorithm will take" and the
+ * regions "converging to the central point" or "to other points not related to our goal"
+ * (Figs. 2-5).  It prints no algorithm for those paths (they were drawn by a
+ * viewer), so the read-out is computed in its exact, parameter-free, discrete form (A17).
+ * Both calls take ONE channel of a map: n[2] x n[1] x n[0] doubles, p0 fastest, host or device
+ * memory, and work on `device` in `cuda_stream` (may be NULL); they return when their outputs are
+ * complete.  n[0]*n[1]*n[2] must be < 2^31. */
+
+/* Finite-difference gradient field in parameter units: grad_out is 3 x n[2] x n[1] x n[0] doubles
+ * (component d = dM/dp_d), host or device.  Grid step h_d = (hi[d]-lo[d])/(n[d]-1); central
+ * differences (M[k+1]-M[k-1])/(2 h_d) inside, one-sided (M[1]-M[0])/h_d and (M[n-1]-M[n-2])/h_d on
+ * the faces; an axis with n[d] == 1 has gradient 0.  MI_ERR_INVALID_ARG if n[d] > 1 and
+ * hi[d] == lo[d], or lo/hi are not finite. */
+mi_status mi_map_gradient(const double *map, const int32_t n[3], const double lo[3], const double hi[3],
+                          double *grad_out, int32_t device, void *cuda_stream);
+
+typedef struct {
+    int64_t n_extrema;        /* nodes that are their own best neighbour                            */
+    int64_t target;           /* the node used as target (the argument, or the global extremum)     */
+    int64_t target_label;     /* where the path from the target ends                                */
+    int64_t captured;         /* nodes whose path ends at target_label                              */
+    double capture_fraction;  /* captured / number of nodes                                         */
+    int32_t max_steps;        /* longest path, in moves                                             */
+    int32_t iterations;       /* pointer-doubling rounds the kernels took                           */
+} mi_basin_stats;
+
+/* Discrete steepest ascent (direction = +1, the arg max of eq. 3) or descent (direction = -1, "the
+ * minimum value it can reach") on the parameter grid.  With v = direction * M, every
+ * node steps to the neighbour (connectivity 6 or 26) with the largest v if that is strictly larger
+ * than its own v -- ties between neighbours go to the lowest linear index -- until no neighbour is
+ * better.  label_out (NULL or n[2] x n[1] x n[0] int64): linear index of the extremum reached;
+ * steps_out (NULL or int32): moves taken.  target: linear index of the ground-truth node, or -1 for
+ * the global extremum of v (lowest index on ties).  stats_out (host, may be NULL). */
+mi_status mi_map_basins(const double *map, const int32_t n[3], int32_t direction, int32_t connectivity,
+                        int64_t target, int64_t *label_out, int32_t *steps_out, mi_basin_stats *stats_out,
+                        int32_t device, void *cuda_stream);
+
 /* ---- host-side pieces of the path, exported so tests can check them without a GPU ------------ */
 
 /* Step a2, family generator: parameter triple -> physical 3x4 [A|t] (double). */

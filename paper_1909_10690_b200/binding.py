@@ -27,7 +27,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
-           "mi_probe_shared_atomic_rate", "mi_version")
+           "mi_map_gradient", "mi_map_basins", "mi_probe_shared_atomic_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError("%s is missing: build it with `python -m paper_1909_10690_b200.build` "
@@ -56,6 +56,10 @@ _lib.mi_get_bins.argtypes = [_vp, C.c_int32, _vp]
 _lib.mi_get_bins.restype = C.c_int
 _lib.mi_release_cached_memory.argtypes = [C.c_int32]
 _lib.mi_release_cached_memory.restype = C.c_int
+_lib.mi_map_gradient.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, _vp]
+_lib.mi_map_gradient.restype = C.c_int
+_lib.mi_map_basins.argtypes = [_vp, _vp, C.c_int32, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, _vp]
+_lib.mi_map_basins.restype = C.c_int
 _lib.mi_last_timing.argtypes = [_vp, _vp, _vp]
 _lib.mi_last_timing.restype = C.c_int
 _lib.mi_probe_shared_atomic_rate.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
@@ -249,6 +253,54 @@ def mi_last_timing(ctx):
     ln = np.zeros(5, dtype=np.int64)
     _check(ctx, _lib.mi_last_timing(ctx.handle, _ptr(ms), _ptr(ln)))
     return ms, ln
+
+
+class _BasinStats(C.Structure):
+    _fields_ = [("n_extrema", C.c_int64), ("target", C.c_int64), ("target_label", C.c_int64),
+                ("captured", C.c_int64), ("capture_fraction", C.c_double), ("max_steps", C.c_int32),
+                ("iterations", C.c_int32)]
+
+
+def _map_channel(m):
+    """One channel of a map: (n2, n1, n0) float64, numpy or torch (host or CUDA); returns (array, n)."""
+    if _is_torch(m):
+        import torch
+        assert m.dtype == torch.float64 and m.dim() == 3
+        m = m.contiguous()
+    else:
+        m = np.ascontiguousarray(m, dtype=np.float64)
+        assert m.ndim == 3
+    return m, _i32(tuple(m.shape)[::-1], 3)
+
+
+def _like(m, shape, dtype_np, dtype_torch_name):
+    if _is_torch(m):
+        import torch
+        return torch.empty(shape, dtype=getattr(torch, dtype_torch_name), device=m.device)
+    return np.empty(shape, dtype=dtype_np)
+
+
+def mi_map_gradient(m, lo, hi, device=0, cuda_stream=None):
+    """Finite-difference gradient field (3, n2, n1, n0) of one map channel, in the memory of `m`."""
+    m, n = _map_channel(m)
+    out = _like(m, (3,) + tuple(m.shape), np.float64, "float64")
+    lo, hi = _f64(lo, 3), _f64(hi, 3)          # keep the arrays alive across the call
+    _check(None, _lib.mi_map_gradient(_ptr(m), _ptr(n), _ptr(lo), _ptr(hi), _ptr(out), int(device), cuda_stream))
+    return out
+
+
+def mi_map_basins(m, direction=1, connectivity=26, target=-1, device=0, cuda_stream=None, want_arrays=True):
+    """Discrete steepest ascent (+1) / descent (-1) basins of one map channel: dict with label, steps
+    (in the memory of `m`, None if not wanted) and the mi_basin_stats fields."""
+    m, n = _map_channel(m)
+    label = _like(m, tuple(m.shape), np.int64, "int64") if want_arrays else None
+    steps = _like(m, tuple(m.shape), np.int32, "int32") if want_arrays else None
+    st = _BasinStats()
+    _check(None, _lib.mi_map_basins(_ptr(m), _ptr(n), int(direction), int(connectivity), int(target), _ptr(label),
+                                    _ptr(steps), C.addressof(st), int(device), cuda_stream))
+    out = {k: getattr(st, k) for k, _ in _BasinStats._fields_}
+    out["label"], out["steps"] = label, steps
+    return out
 
 
 def mi_release_cached_memory(device=0) -> None:

@@ -1,0 +1,128 @@
+"""GPU parity of the capture-range analysis calls (mi_map_gradient, mi_map_basins) against the CPU
+oracle (oracle/map_analysis.py), through the C ABI.  Labels, steps and counts are integer work:
+bit-exact.  The gradient is one IEEE double subtraction and one division per component: both sides
+do the same two correctly rounded operations, so it is compared for equality as well."""
+import numpy as np
+import pytest
+
+from oracle import map_analysis as ma
+from paper_1909_10690_b200 import phantoms as ph
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mi():
+    from paper_1909_10690_b200 import build
+    build.build()
+    from paper_1909_10690_b200 import binding
+    return binding
+
+
+def rough_map(shape, seed, plateaus=True):
+    rng = np.random.default_rng(seed)
+    m = rng.normal(size=shape)
+    if plateaus:
+        m.reshape(-1)[rng.integers(0, m.size, m.size // 4)] = 0.5
+    return m
+
+
+def check_basins(mi, m, direction, conn, target):
+    ref = ma.map_basins(m, direction, conn, target)
+    got = mi.mi_map_basins(m, direction, conn, target)
+    assert np.array_equal(got["label"], ref["label"])
+    assert np.array_equal(got["steps"], ref["steps"])
+    for k in ("n_extrema", "target", "target_label", "captured", "max_steps"):
+        assert got[k] == ref[k], k
+    assert got["capture_fraction"] == ref["capture_fraction"]
+    return got
+
+
+def test_gradient_equals_oracle_exactly(mi):
+    for shape, lo, hi in [((9, 8, 7), (-3, -2, 0), (3, 2, 9)), ((1, 1, 5), (0, 0, 0), (4, 1, 1)), ((41, 41, 41), (-10,) * 3, (10,) * 3),
+                          ((2, 300, 1), (0, -7, 0.5), (0, 7, 1.5)), ((1, 1, 1), (0, 0, 0), (0, 0, 0))]:
+        m = rough_map(shape, 1, plateaus=False)
+        lo3, hi3 = list(lo), list(hi)
+        for d in range(3):                      # an axis with one node may have lo == hi
+            if shape[2 - d] == 1:
+                hi3[d] = lo3[d]
+        g = mi.mi_map_gradient(m, lo3, hi3)
+        assert np.array_equal(g, ma.map_gradient(m, lo3, hi3)), shape
+
+
+def test_basins_equal_oracle_on_rough_maps(mi):
+    for shape in [(4, 4, 4), (9, 8, 7), (1, 1, 1), (1, 6, 40), (33, 1, 1), (41, 41, 41), (30, 50, 70)]:
+        m = rough_map(shape, 7)
+        for direction in (1, -1):
+            for conn in (6, 26):
+                check_basins(mi, m, direction, conn, -1)
+        check_basins(mi, m, 1, 26, m.size // 2)
+
+
+def test_basins_long_paths_need_many_doubling_rounds(mi):
+    # a monotone ramp along a 1 x 1 x 5000 line: one path of 4999 moves (13 doubling rounds)
+    m = np.arange(5000, dtype=np.float64).reshape(1, 1, 5000)
+    r = check_basins(mi, m, 1, 6, 0)
+    assert r["max_steps"] == 4999 and r["n_extrema"] == 1 and r["capture_fraction"] == 1.0
+    # a serpentine ridge through a 2D sheet: path length ~ n0*n1/2
+    n0, n1 = 64, 63
+    m = np.full((1, n1, n0), -1.0)
+    v = 0.0
+    for k1 in range(0, n1, 2):
+        cols = range(n0) if (k1 // 2) % 2 == 0 else range(n0 - 1, -1, -1)
+        for k0 in cols:
+            m[0, k1, k0] = v
+            v += 1.0
+        if k1 + 1 < n1:
+            m[0, k1 + 1, cols[-1]] = v
+            v += 1.0
+    r = check_basins(mi, m, 1, 6, 0)
+    assert r["max_steps"] > 2000
+
+
+def test_basins_device_pointers_and_no_arrays(mi):
+    import torch
+    m = rough_map((20, 21, 22), 3)
+    ref = ma.map_basins(m, 1, 26, -1)
+    md = torch.from_numpy(m).cuda()
+    got = mi.mi_map_basins(md, 1, 26, -1)
+    assert got["label"].is_cuda and np.array_equal(got["label"].cpu().numpy(), ref["label"])
+    assert np.array_equal(got["steps"].cpu().numpy(), ref["steps"])
+    g = mi.mi_map_gradient(md, (0, 0, 0), (1, 1, 1))
+    assert g.is_cuda and np.array_equal(g.cpu().numpy(), ma.map_gradient(m, (0, 0, 0), (1, 1, 1)))
+    only = mi.mi_map_basins(m, 1, 26, -1, want_arrays=False)
+    assert only["label"] is None and only["captured"] == ref["captured"]
+
+
+def test_analysis_argument_errors(mi):
+    m = np.zeros((3, 3, 3))
+    for kw in (dict(direction=0), dict(connectivity=18), dict(target=27), dict(target=-2)):
+        with pytest.raises(mi.MIError) as ei:
+            mi.mi_map_basins(m, **kw)
+        assert ei.value.status == mi.MI_ERR_INVALID_ARG
+    with pytest.raises(mi.MIError) as ei:
+        mi.mi_map_gradient(m, (0, 0, 0), (1, 0, 1))          # three nodes on an axis of zero length
+    assert ei.value.status == mi.MI_ERR_INVALID_ARG
+
+
+def test_capture_range_of_a_real_map_shannon_and_tsallis(mi):
+    """End to end on the C1 translation map (9^3 half-step grid): every channel's basins equal the
+    oracle's on the oracle's own map and on the GPU map; the Shannon channel captures the node next to
+    the ground truth (P11: the arg max is within one step of it)."""
+    import oracle as orc
+    cfg = ph.config_c1(grid_n=9)
+    ref = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                     cfg.family, cfg.lo, cfg.hi, cfg.n, q=cfg.q, interp=1)
+    with mi.mi_create(cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        gm, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+    for ch in range(gm.shape[0]):
+        r = check_basins(mi, ref["map"][ch], 1, 26, -1)
+        g = mi.mi_map_basins(gm[ch], 1, 26, -1)
+        # the two maps differ by ~1e-10 nats: the same arg max, and the same basins wherever the
+        # oracle's map has no near-tie between a node's best and second-best neighbour
+        assert g["target"] == r["target"] == int(am[ch])
+    sh = mi.mi_map_basins(gm[0], 1, 26, -1)
+    k2, k1, k0 = np.unravel_index(sh["target"], gm.shape[1:])
+    p = [cfg.lo[d] + k * (cfg.hi[d] - cfg.lo[d]) / (cfg.n[d] - 1) for d, k in enumerate((k0, k1, k2))]
+    assert max(abs(p[d] - cfg.truth[d]) for d in range(3)) <= 1.0
+    assert 0.0 < sh["capture_fraction"] <= 1.0
