@@ -423,6 +423,8 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.rows_smem = c->rows_smem;
         a.pitch = c->gpitch;
         a.ty_log2 = c->ty_log2;
+        a.unroll = 0;
+        if (const char* v = std::getenv("MI_B200_GENERIC_UNROLL")) a.unroll = std::atoi(v);
         a.M = c->d_M + (size_t)off * 12;
         a.hist = hist;
         a.f = {c->fd[0], c->fd[1], c->fd[2]};

@@ -46,6 +46,7 @@ struct ResampleArgs {
     int nb;
     float mlo, mscale;       // moving binning (CANON-5)
     int n_transforms;
+    int unroll;              // voxels per lane in flight (1..4); 0 = chosen from the row length
     int nslabs;              // CTAs cooperating on one transform (slabs of row tiles)
 };
 

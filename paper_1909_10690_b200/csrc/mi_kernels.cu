@@ -388,8 +388,28 @@ int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes) {
 
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s) {
     if (a.rows_smem < 1 || a.pitch < a.nb || a.ty_log2 < 0 || a.ty_log2 > 5) return cudaErrorInvalidConfiguration;
-    if (interp == MI_INTERP_NEAREST) return launch_resample_t<MI_INTERP_NEAREST, 4>(a, num_sms, s);
-    return launch_resample_t<MI_INTERP_TRILINEAR, 2>(a, num_sms, s);
+    // Voxels in flight per lane: a row is ceil(fnx/32) warp-chunks and a lane takes `unroll` of them per
+    // trip, so the last trip of a row idles (trips*unroll - chunks) chunks: pick the unroll in 1..4 that
+    // wastes the fewest, the larger one on ties (260 voxels = 9 chunks -> 3).
+    int unroll = a.unroll;
+    if (unroll < 1 || unroll > 4) {
+        const int chunks = (a.f.nx + 31) / 32;
+        int best_waste = 1 << 30;
+        for (int u = 1; u <= 4; ++u) {
+            const int waste = (chunks + u - 1) / u * u - chunks;
+            if (waste <= best_waste) { best_waste = waste; unroll = u; }
+        }
+    }
+    if (interp == MI_INTERP_NEAREST) {
+        if (unroll == 1) return launch_resample_t<MI_INTERP_NEAREST, 1>(a, num_sms, s);
+        if (unroll == 2) return launch_resample_t<MI_INTERP_NEAREST, 2>(a, num_sms, s);
+        if (unroll == 3) return launch_resample_t<MI_INTERP_NEAREST, 3>(a, num_sms, s);
+        return launch_resample_t<MI_INTERP_NEAREST, 4>(a, num_sms, s);
+    }
+    if (unroll == 1) return launch_resample_t<MI_INTERP_TRILINEAR, 1>(a, num_sms, s);
+    if (unroll == 2) return launch_resample_t<MI_INTERP_TRILINEAR, 2>(a, num_sms, s);
+    if (unroll == 3) return launch_resample_t<MI_INTERP_TRILINEAR, 3>(a, num_sms, s);
+    return launch_resample_t<MI_INTERP_TRILINEAR, 4>(a, num_sms, s);
 }
 
 // ------------------------------------------------------------------------------------------------
