@@ -266,6 +266,41 @@ def test_c5_full_size_sampled_against_oracle(mi):
             else:
                 assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
             assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
+        # the call bench.py times: the whole 41^3 map through the separable kernels with the entropy
+        # epilogue; its values at the sampled nodes against the oracle's trilinear Shannon values
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        for node, want in zip(nodes, ref["mi"][:, 0]):
+            assert abs(m[0, node[2], node[1], node[0]] - want) <= MI_TOL, node
+        assert m[0].reshape(-1)[am[0]] == m[0].max() and am[0] == int(np.argmax(m[0]))
+        k2, k1, k0 = np.unravel_index(am[0], m.shape[1:])
+        p = [-10 + k * step for k in (k0, k1, k2)]
+        assert max(abs(p[d] - cfg.truth[d]) for d in range(3)) <= step        # P11 at full size
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_c3_c4_full_size_maps_sampled_against_oracle(mi, name):
+    """The full-size rotation (generic kernel) and scale (separable kernels, five Tsallis orders) maps of
+    BASELINE.json; sampled grid nodes are checked one by one against the oracle."""
+    cfg = ph.get_config(name)
+    assert cfg.fixed.shape == (260, 311, 260)
+    n = cfg.n
+    nodes = [(0, 0, 0), (n[0] - 1, n[1] - 1, n[2] - 1), (n[0] // 2, n[1] // 2, n[2] // 2), (n[0] - 2, 1, n[2] // 3)]
+    par = lambda node: [cfg.lo[d] + node[d] * (cfg.hi[d] - cfg.lo[d]) / (n[d] - 1) for d in range(3)]
+    T = np.stack([orc.family_matrix(cfg.family, par(node)) for node in nodes])
+    fd, md = cfg.fixed.shape[::-1], cfg.moving.shape[::-1]
+    M = orc.physical_to_index(T, fd, cfg.fixed_spacing, md, cfg.moving_spacing)
+    ref = orc.eval_batch(cfg.fixed, cfg.moving, M, cfg.nbins, *cfg.ranges, 1, q=cfg.q)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+    for node, want in zip(nodes, ref["mi"]):
+        got = m[:, node[2], node[1], node[0]]
+        assert np.max(np.abs(got - want)) <= MI_TOL, (node, got, want)
+    for ch in range(m.shape[0]):
+        assert am[ch] == int(np.argmax(m[ch]))
+    k2, k1, k0 = np.unravel_index(am[0], m.shape[1:])
+    p = par((k0, k1, k2))
+    steps = [(cfg.hi[d] - cfg.lo[d]) / (n[d] - 1) for d in range(3)]
+    assert all(abs(p[d] - cfg.truth[d]) <= steps[d] * 1.0001 for d in range(3)), (p, cfg.truth)   # P11 (Shannon)
 
 
 def test_context_cycles_reuse_the_pool_and_release(mi):
