@@ -185,7 +185,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C5", choices=["C2", "C3", "C4", "C5"])
+    ap.add_argument("--config", default="C5", choices=["C2", "C3", "C4", "C5", "PAPER51"])
     ap.add_argument("--res", type=float, default=1.0, help="development only: reduced-resolution phantom")
     ap.add_argument("--grid", type=int, default=0, help="development only: grid nodes per axis")
     ap.add_argument("--interp", default="trilinear", choices=["trilinear", "nearest"])

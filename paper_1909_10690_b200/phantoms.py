@@ -255,11 +255,23 @@ def config_c5(res=1.0, grid_n=41, seed=303) -> Config:
     return Config("C5", fixed, moving, fsp, msp, 256, 0, (-10,) * 3, (10,) * 3, (grid_n,) * 3, (), d)
 
 
+def config_paper51(res=1.0, grid_n=51, seed=303) -> Config:
+    """Paper-shaped context run (not one of BASELINE.json's configs): the paper maps "the same image on
+    both fixed and moving" and gives 51 positions over +-25 mm per axis as its example
+    of a translation map: the T1-like head phantom against itself, 51^3 translations,
+    Shannon + Tsallis q = 0.5, 2.0 (the orders of Figs. 4-5)."""
+    dims = _head_dims(res)
+    sp = (0.7 / res,) * 3
+    fixed = render(head_phantom(seed), T1_TABLE, dims, sp, None, 0.02, seed, bias_amp=0.1)
+    return Config("PAPER51", fixed, fixed, sp, sp, 256, 0, (-25,) * 3, (25,) * 3, (grid_n,) * 3, (0.5, 2.0),
+                  (0.0, 0.0, 0.0))
+
+
 @lru_cache(maxsize=8)
 def get_config(name: str, **kw) -> Config:
     """Cached access: get_config('C5'), get_config('C3', res=0.25, grid_n=5) ..."""
     return {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4,
-            "C5": config_c5}[name](**kw)
+            "C5": config_c5, "PAPER51": config_paper51}[name](**kw)
 
 
 def ramp_volume(dims, coeffs) -> np.ndarray:
