@@ -133,6 +133,27 @@ __global__ void __launch_bounds__(128) ypass_kernel(const VT* __restrict__ X, in
     *reinterpret_cast<uint32_t*>(colvalid + (size_t)pair * colpitch + col0) = cv;
     const size_t pstride = (size_t)prows * fnx;
     VT* __restrict__ out = XY + (size_t)pair * planes * colpitch + col0;
+    // Common case (trilinear): the four columns are four adjacent, 16-byte aligned voxels of one moving
+    // row pair -- two 16-byte loads per plane instead of eight 4-byte ones (same values, same lerps).
+    bool vec = !NN && (fnx & 3) == 0 && off[0] >= 0;
+#pragma unroll
+    for (int k = 1; k < 4; ++k) vec = vec && off[k] == off[0] + k;
+    if (vec) {
+        const float w = wy[0];   // same iy for all four: same weight
+        const float* __restrict__ r = reinterpret_cast<const float*>(X) + off[0];
+#pragma unroll 4
+        for (int plane = 0; plane < planes; ++plane) {
+            const float4 lo = __ldg(reinterpret_cast<const float4*>(r + plane * pstride));
+            const float4 hi = __ldg(reinterpret_cast<const float4*>(r + plane * pstride + fnx));
+            float4 q;
+            q.x = __fmul_rn(lerp_rn(lo.x, hi.x, w), prescale);
+            q.y = __fmul_rn(lerp_rn(lo.y, hi.y, w), prescale);
+            q.z = __fmul_rn(lerp_rn(lo.z, hi.z, w), prescale);
+            q.w = __fmul_rn(lerp_rn(lo.w, hi.w, w), prescale);
+            *reinterpret_cast<float4*>(reinterpret_cast<float*>(out) + (size_t)plane * colpitch) = q;
+        }
+        return;
+    }
 #pragma unroll 4
     for (int plane = 0; plane < planes; ++plane) {
         Quad<NN, VT> q;
