@@ -46,7 +46,7 @@ typedef enum {
     MI_OK = 0,
     MI_ERR_INVALID_ARG = 1,   /* NULL pointer, dim < 1, grid n < 1, spacing <= 0 or non-finite, lo >= hi,
                                  nbins < 2, N < 0, q <= 0 or non-finite, non-finite matrix entry */
-    MI_ERR_UNSUPPORTED = 2,   /* nbins > 256; volume with more than 2^31-1 voxels */
+    MI_ERR_UNSUPPORTED = 2,   /* nbins > 4096; volume with more than 2^31-1 voxels */
     MI_ERR_OUT_OF_MEMORY = 3,
     MI_ERR_CUDA = 4,          /* any CUDA runtime failure, including "no device" */
     MI_ERR_INTERNAL = 5
@@ -77,7 +77,10 @@ typedef enum {
  *   fixed, moving  float32 volumes (host or device), finite values; copied -- the caller may free
  *                  them on return.
  *   *_dims         (nx, ny, nz), each >= 1;  *_spacing  mm, each > 0 and finite.
- *   nbins          2..256 bins per axis of the joint histogram.
+ *   nbins          2..4096 bins per axis of the joint histogram.  Up to 256 the histograms are built in
+ *                  shared memory (and translation / scale maps take the separable kernels); above, the
+ *                  "full histogram" of PAPER.md:212 for 12-bit data, they live in global memory
+ *                  (nbins*nbins*4 bytes per transform) and every transform takes the generic kernel.
  *   *_lo, *_hi     intensity range of each volume, lo < hi, finite.
  *   device         CUDA device ordinal.   cuda_stream  a cudaStream_t (may be NULL = default).
  * Blocks until the context is ready. */
@@ -179,8 +182,8 @@ mi_status mi_index_affine(const double T[12], const int32_t fixed_dims[3], const
 /* ---- introspection used by tests and the benchmark ------------------------------------------- */
 
 /* Copy the pre-binned volumes out of the context (step a1 parity): which = 0 fixed, 1 moving;
- * out receives nx*ny*nz uint8 (host or device). */
-mi_status mi_get_bins(mi_ctx *ctx, int32_t which, uint8_t *out);
+ * out receives nx*ny*nz bin indices (host or device): uint8 for nbins <= 256, uint16 above. */
+mi_status mi_get_bins(mi_ctx *ctx, int32_t which, void *out);
 
 /* Device milliseconds (CUDA events on the context's stream) spent in the kernels of the last
  * mi_eval_batch / mi_map call: ms[0] transform upload + setup, ms[1] resample+histogram kernels,

@@ -241,7 +241,7 @@ def mi_index_affine(T, fixed_dims, fixed_spacing, moving_dims, moving_spacing) -
 
 def mi_get_bins(ctx, which: int) -> np.ndarray:
     dims = ctx.fixed_dims if which == 0 else ctx.moving_dims
-    out = np.empty((dims[2], dims[1], dims[0]), dtype=np.uint8)
+    out = np.empty((dims[2], dims[1], dims[0]), dtype=np.uint8 if ctx.nbins <= 256 else np.uint16)
     _check(ctx, _lib.mi_get_bins(ctx.handle, int(which), _ptr(out)))
     return out
 

@@ -28,6 +28,9 @@ struct mi_ctx {
     int* d_rank_inv = nullptr;          // 256: rank -> fixed bin
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
+    bool wide = false;                  // nbins > 256: uint16 bins, global-memory histograms, generic kernel only
+    uint16_t* d_fbins16 = nullptr;
+    uint16_t* d_mbins16 = nullptr;
     int rows_smem = 0;                  // generic kernel: ranked fixed-bin rows in shared memory
     int gpitch = 0;                     // generic kernel: words per shared histogram row
     int ty_log2 = 3;                    // generic kernel: row tile = 8 (y) x 4 (z)
@@ -444,7 +447,24 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         }
         a.nslabs = nslabs;
         timer.begin(4);
-        MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, s));
+        if (c->wide) {
+            mi::WideArgs w;
+            w.fbins = c->d_fbins16;
+            w.mbins = c->d_mbins16;
+            w.moving_pad = c->d_moving_pad;
+            w.M = a.M;
+            w.hist = hist;
+            w.f = a.f;
+            w.m = a.m;
+            w.nb = c->nb;
+            w.mlo = c->mlo;
+            w.mscale = c->mscale;
+            w.n_transforms = (int)cnt;
+            w.nslabs = nslabs;
+            MI_CUDA(c, mi::launch_resample_hist_wide(w, interp, c->num_sms, s));
+        } else {
+            MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, s));
+        }
         timer.end();
         c->last_launches[1] += 1;
         c->last_launches[4] += 1;
@@ -560,7 +580,7 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
     const int64_t npad = ((int64_t)moving_dims[0] + 2) * ((int64_t)moving_dims[1] + 2) * ((int64_t)moving_dims[2] + 2);
     if (npad > 0x7FFFFFFFLL) return fail(nullptr, MI_ERR_UNSUPPORTED, "padded moving volume has more than 2^31-1 voxels");
     if (nbins < 2) return fail(nullptr, MI_ERR_INVALID_ARG, "nbins < 2");
-    if (nbins > 256) return fail(nullptr, MI_ERR_UNSUPPORTED, "nbins > 256 is not supported");
+    if (nbins > mi::kMaxBinsWide) return fail(nullptr, MI_ERR_UNSUPPORTED, "nbins > 4096 is not supported");
     if (!(std::isfinite(fixed_lo) && std::isfinite(fixed_hi) && fixed_lo < fixed_hi) ||
         !(std::isfinite(moving_lo) && std::isfinite(moving_hi) && moving_lo < moving_hi))
         return fail(nullptr, MI_ERR_INVALID_ARG, "intensity range must be finite with lo < hi");
@@ -632,37 +652,46 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = cudaMemcpyAsync(d_tmp, fixed, (size_t)nf * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy fixed"); break; }
         if ((e = cudaMemcpyAsync(d_mov, moving, (size_t)nm * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy moving"); break; }
         if ((e = cudaMemsetAsync(d_counts, 0, 256 * sizeof(unsigned long long), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
-        if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, nullptr, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
-        if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, reinterpret_cast<unsigned*>(d_counts), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
-        {
-            unsigned h_flag = 1;
-            if ((e = cudaMemcpyAsync(&h_flag, d_counts, sizeof(unsigned), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy flag"); break; }
-            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync flag"); break; }
-            // kBinFast*: no clamps needed (mi_internal.h); prescaled when the bin scale is a power of two
-            // (so that scaling commutes with every rounding; 2^-100 < scale keeps products normal)
-            int ex = 0;
-            const bool pow2 = std::frexp(c->mscale, &ex) == 0.5f && ex > -100 && ex < 100;
-            c->bin_mode = (h_flag == 0 && c->mlo == 0.0f) ? (pow2 ? mi::kBinFastPrescaled : mi::kBinFast) : mi::kBinGeneral;
-            if (const char* v = std::getenv("MI_B200_BIN_MODE")) { const int r = std::atoi(v); if (r >= 0 && r < c->bin_mode) c->bin_mode = r; }
-        }
-        if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
-        {
-            // the separable path keeps ranks < zrows_real in shared memory; if not every bin fits, the
-            // last shared row becomes a dump row and the voxels of the rare ranks go to a list
-            unsigned long long h_counts[256];
-            uint8_t h_rank[256];
-            if ((e = cudaMemcpyAsync(h_counts, d_counts, sizeof(h_counts), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy counts"); break; }
-            if ((e = cudaMemcpyAsync(h_rank, c->d_rank, sizeof(h_rank), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy ranks"); break; }
-            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync ranks"); break; }
-            c->zrows_real = c->zrows_smem > nbins ? nbins : c->zrows_smem - 1;   // one row is the dump row
-            unsigned long long n_rare = 0;
-            for (int a = 0; a < 256; ++a)
-                if ((int)h_rank[a] >= c->zrows_real) n_rare += h_counts[a];
-            c->n_rare = (unsigned)n_rare;
-            if ((e = dev_alloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
-            if ((e = cudaMemsetAsync(d_counts, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
-            if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
-                                           c->d_fb_pitched, c->d_rare, reinterpret_cast<unsigned*>(d_counts), c->n_rare, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pitch fixed bins"); break; }
+        c->wide = nbins > 256;
+        if (c->wide) {
+            c->use_separable = false;
+            if ((e = dev_alloc((void**)&c->d_fbins16, (size_t)nf * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide fixed bins"); break; }
+            if ((e = dev_alloc((void**)&c->d_mbins16, (size_t)nm * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide moving bins"); break; }
+            if ((e = mi::launch_prebin16(d_tmp, c->d_fbins16, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed (wide)"); break; }
+            if ((e = mi::launch_prebin16(d_mov, c->d_mbins16, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving (wide)"); break; }
+        } else {
+            if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, nullptr, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
+            if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, reinterpret_cast<unsigned*>(d_counts), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
+            {
+                unsigned h_flag = 1;
+                if ((e = cudaMemcpyAsync(&h_flag, d_counts, sizeof(unsigned), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy flag"); break; }
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync flag"); break; }
+                // kBinFast*: no clamps needed (mi_internal.h); prescaled when the bin scale is a power of two
+                // (so that scaling commutes with every rounding; 2^-100 < scale keeps products normal)
+                int ex = 0;
+                const bool pow2 = std::frexp(c->mscale, &ex) == 0.5f && ex > -100 && ex < 100;
+                c->bin_mode = (h_flag == 0 && c->mlo == 0.0f) ? (pow2 ? mi::kBinFastPrescaled : mi::kBinFast) : mi::kBinGeneral;
+                if (const char* v = std::getenv("MI_B200_BIN_MODE")) { const int r = std::atoi(v); if (r >= 0 && r < c->bin_mode) c->bin_mode = r; }
+            }
+            if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
+            {
+                // the separable path keeps ranks < zrows_real in shared memory; if not every bin fits, the
+                // last shared row becomes a dump row and the voxels of the rare ranks go to a list
+                unsigned long long h_counts[256];
+                uint8_t h_rank[256];
+                if ((e = cudaMemcpyAsync(h_counts, d_counts, sizeof(h_counts), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy counts"); break; }
+                if ((e = cudaMemcpyAsync(h_rank, c->d_rank, sizeof(h_rank), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy ranks"); break; }
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync ranks"); break; }
+                c->zrows_real = c->zrows_smem > nbins ? nbins : c->zrows_smem - 1;   // one row is the dump row
+                unsigned long long n_rare = 0;
+                for (int a = 0; a < 256; ++a)
+                    if ((int)h_rank[a] >= c->zrows_real) n_rare += h_counts[a];
+                c->n_rare = (unsigned)n_rare;
+                if ((e = dev_alloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
+                if ((e = cudaMemsetAsync(d_counts, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
+                if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
+                                               c->d_fb_pitched, c->d_rare, reinterpret_cast<unsigned*>(d_counts), c->n_rare, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pitch fixed bins"); break; }
+            }
         }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
@@ -682,7 +711,7 @@ void mi_destroy(mi_ctx* c) {
     if (!c) return;
     DeviceGuard guard(c->device);
     if (guard.ok) {
-        void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mbins,
+        void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_fbins16, c->d_mbins16, c->d_mbins,
                         c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
@@ -786,13 +815,19 @@ mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double h
                      sep ? &plan : nullptr);
 }
 
-mi_status mi_get_bins(mi_ctx* c, int32_t which, uint8_t* out) {
+mi_status mi_get_bins(mi_ctx* c, int32_t which, void* out) {
     if (!c || !out) return MI_ERR_INVALID_ARG;
     if (which != 0 && which != 1) return fail(c, MI_ERR_INVALID_ARG, "which must be 0 or 1");
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
-    const uint8_t* src = which == 0 ? c->d_fbins : c->d_mbins;
     const size_t n = (size_t)(which == 0 ? c->nf : c->nm);
+    if (c->wide) {   // two bytes per voxel
+        const uint16_t* src16 = which == 0 ? c->d_fbins16 : c->d_mbins16;
+        MI_CUDA(c, cudaMemcpyAsync(out, src16, n * sizeof(uint16_t), cudaMemcpyDefault, c->stream));
+        MI_CUDA(c, cudaStreamSynchronize(c->stream));
+        return MI_OK;
+    }
+    const uint8_t* src = which == 0 ? c->d_fbins : c->d_mbins;
     MI_CUDA(c, cudaMemcpyAsync(out, src, n, cudaMemcpyDefault, c->stream));
     MI_CUDA(c, cudaStreamSynchronize(c->stream));
     return MI_OK;

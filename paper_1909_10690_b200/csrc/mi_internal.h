@@ -20,6 +20,7 @@ bool is_host_pointer(const void* p);
 constexpr int kMaxQPerPass = 8;      // Tsallis orders handled by one entropy-kernel pass
 constexpr int kHistThreads = 1024;   // resample+histogram CTA size
 constexpr int kEntropyThreads = 256;
+constexpr int kMaxBinsWide = 4096;   // largest nbins (above 256: uint16 bins, global-memory histograms)
 
 // ---- host-side double math (mi_host.cpp; compiled with -ffp-contract=off) --------------------
 int family_matrix(int family, const double p[3], double T[12]);
@@ -57,6 +58,20 @@ cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, i
 cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
                                    uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s);
 int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes);
+// wide histograms (256 < nb <= kMaxBinsWide)
+struct WideArgs {
+    const uint16_t* fbins;        // fixed bins [fz][fy][fx]
+    const uint16_t* mbins;        // moving bins (nearest neighbour)
+    const float* moving_pad;      // replicate-padded moving float32
+    const float* M;               // n_transforms x 12 (device)
+    uint32_t* hist;               // n_transforms x nb x nb, zero on entry
+    VolumeDesc f, m;
+    int nb;
+    float mlo, mscale;
+    int n_transforms, nslabs;
+};
+cudaError_t launch_prebin16(const float* vol, uint16_t* bins, int64_t n, float lo, float scale, int nb, cudaStream_t s);
+cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s);
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s);
 // Where the entropy kernel writes the result of histogram `item`: transform-major position item
 // (enabled == 0) or, for the separable path whose items are ordered (p0, p1, p2) with p2 fastest,

@@ -421,16 +421,56 @@ __device__ __forceinline__ double warp_sum_d(double v) {
     return v;
 }
 
+// Last step of a5 for transform t from the three distributions' sums (tot[0..2] = sum c ln c of A, B, AB;
+// tot[3 + 3k + {0,1,2}] = sum c^q_k) and the sample count n: eq. 1-2 and the Tsallis forms.
+__device__ void entropy_finish(const double* tot, unsigned long long n, int t, const double* qv, int nq_pass,
+                               int q_off, int nq_total, int form, double* __restrict__ mi_out,
+                               int64_t* __restrict__ nvalid, const OutMap& om) {
+    size_t dst = (size_t)t;
+    if (om.enabled) {  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
+        const int c = t % om.n2, ab = t / om.n2;
+        const int b = ab % om.n1, al = ab / om.n1;
+        dst = ((size_t)c * om.n1 + b) * om.n0 + (size_t)(om.a0 + al);
+    }
+    double* out = mi_out + dst * (1 + nq_total);
+    if (nvalid != nullptr) nvalid[dst] = (int64_t)n;
+    if (n == 0) {
+        out[0] = 0.0;
+        for (int k = 0; k < nq_pass; ++k) out[1 + q_off + k] = 0.0;
+        return;
+    }
+    const double N = (double)n, lnN = log(N);
+    const double HA = lnN - tot[0] / N, HB = lnN - tot[1] / N, HAB = lnN - tot[2] / N;
+    const double I = HA + HB - HAB;  // eq. 2
+    out[0] = I;
+    for (int k = 0; k < nq_pass; ++k) {
+        const double qq = qv[k];
+        double val;
+        if (qq == 1.0) {
+            val = I;
+        } else {
+            const double sc = exp(-qq * lnN);
+            const double SA = (1.0 - tot[3 + 3 * k + 0] * sc) / (qq - 1.0);
+            const double SB = (1.0 - tot[3 + 3 * k + 1] * sc) / (qq - 1.0);
+            const double SAB = (1.0 - tot[3 + 3 * k + 2] * sc) / (qq - 1.0);
+            val = SA + SB - SAB;
+            if (form == MI_TSALLIS_PSEUDO_ADDITIVE) val += (1.0 - qq) * SA * SB;
+        }
+        out[1 + q_off + k] = val;
+    }
+}
+
 // One CTA per transform.  With c the integer counts and N their total:
 //   H = -sum (c/N) ln (c/N) = ln N - (sum c ln c)/N,      sum p^q = exp(-q ln N) * sum c^q.
 // Accumulators per distribution X in {A, B, AB}: L_X = sum c ln c and P_X[k] = sum c^q_k.
+template <int MAXB>
 __global__ void __launch_bounds__(kEntropyThreads)
 entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restrict__ q, int nq_total,
                int q_off, int nq_pass, int form, double* __restrict__ mi_out,
                int64_t* __restrict__ nvalid, const OutMap om) {
     constexpr int NW = kEntropyThreads / 32;
     constexpr int NACC = 3 * (1 + kMaxQPerPass);
-    __shared__ unsigned sh_pa[256], sh_pb[256];
+    __shared__ unsigned sh_pa[MAXB], sh_pb[MAXB];
     __shared__ double sh_red[NACC][NW];
     __shared__ unsigned long long sh_n[NW];
     const int t = blockIdx.x;
@@ -441,7 +481,7 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
 #pragma unroll
     for (int k = 0; k < kMaxQPerPass; ++k) qv[k] = k < nq_pass ? q[q_off + k] : 1.0;
 
-    for (int i = threadIdx.x; i < 256; i += kEntropyThreads) { sh_pa[i] = 0u; sh_pb[i] = 0u; }
+    for (int i = threadIdx.x; i < MAXB; i += kEntropyThreads) { sh_pa[i] = 0u; sh_pb[i] = 0u; }
     __syncthreads();
 
     double acc[NACC];
@@ -511,38 +551,128 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
         }
         unsigned long long n = 0;
         for (int w = 0; w < NW; ++w) n += sh_n[w];
-        size_t dst = (size_t)t;
-        if (om.enabled) {  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
-            const int c = t % om.n2, ab = t / om.n2;
-            const int b = ab % om.n1, al = ab / om.n1;
-            dst = ((size_t)c * om.n1 + b) * om.n0 + (size_t)(om.a0 + al);
-        }
-        double* out = mi_out + dst * (1 + nq_total);
-        if (nvalid != nullptr) nvalid[dst] = (int64_t)n;
-        if (n == 0) {
-            out[0] = 0.0;
-            for (int k = 0; k < nq_pass; ++k) out[1 + q_off + k] = 0.0;
-        } else {
-            const double N = (double)n, lnN = log(N);
-            const double HA = lnN - tot[0] / N, HB = lnN - tot[1] / N, HAB = lnN - tot[2] / N;
-            const double I = HA + HB - HAB;  // eq. 2
-            out[0] = I;
-            for (int k = 0; k < nq_pass; ++k) {
-                const double qq = qv[k];
-                double val;
-                if (qq == 1.0) {
-                    val = I;
-                } else {
-                    const double sc = exp(-qq * lnN);
-                    const double SA = (1.0 - tot[3 + 3 * k + 0] * sc) / (qq - 1.0);
-                    const double SB = (1.0 - tot[3 + 3 * k + 1] * sc) / (qq - 1.0);
-                    const double SAB = (1.0 - tot[3 + 3 * k + 2] * sc) / (qq - 1.0);
-                    val = SA + SB - SAB;
-                    if (form == MI_TSALLIS_PSEUDO_ADDITIVE) val += (1.0 - qq) * SA * SB;
+        entropy_finish(tot, n, t, qv, nq_pass, q_off, nq_total, form, mi_out, nvalid, om);
+    }
+}
+
+// Wide histograms (nb > 256) are tens of megabytes each: the rows of one histogram are split over
+// gridDim.x CTAs.  Pass 1: every CTA takes a row range of transform blockIdx.y -- joint terms into
+// per-CTA partial sums, row sums (fixed marginal) stored, column sums (moving marginal) added to pb
+// with integer atomics (order-free, so the result is reproducible).  Pass 2: one CTA per transform
+// adds the marginal terms and the partial sums in a fixed order and finishes.
+__global__ void __launch_bounds__(kEntropyThreads)
+entropy_wide_partial_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restrict__ q, int q_off,
+                            int nq_pass, unsigned* __restrict__ pa, unsigned* __restrict__ pb,
+                            double* __restrict__ partial /* [t][split][1 + kMaxQPerPass] */) {
+    constexpr int NW = kEntropyThreads / 32;
+    constexpr int NA = 1 + kMaxQPerPass;
+    __shared__ unsigned sh_pb[kMaxBinsWide];
+    __shared__ double sh_red[NA][NW];
+    const int t = blockIdx.y, split = blockIdx.x, nsplit = gridDim.x;
+    const int r0 = (int)((long long)nb * split / nsplit), r1 = (int)((long long)nb * (split + 1) / nsplit);
+    const uint32_t* __restrict__ h = hist + (size_t)t * nb * nb;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double qv[kMaxQPerPass];
+#pragma unroll
+    for (int k = 0; k < kMaxQPerPass; ++k) qv[k] = k < nq_pass ? q[q_off + k] : 1.0;
+    for (int i = threadIdx.x; i < nb; i += kEntropyThreads) sh_pb[i] = 0u;
+    __syncthreads();
+    double acc[NA];
+#pragma unroll
+    for (int i = 0; i < NA; ++i) acc[i] = 0.0;
+    for (int r = r0 + warp; r < r1; r += NW) {
+        const uint32_t* __restrict__ row = h + (size_t)r * nb;
+        unsigned rowsum = 0;
+        for (int c0 = lane; c0 < nb; c0 += 128) {          // four loads in flight per lane
+            unsigned v[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) v[u] = c0 + 32 * u < nb ? __ldg(row + c0 + 32 * u) : 0u;
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (v[u]) {
+                    rowsum += v[u];
+                    atomicAdd(&sh_pb[c0 + 32 * u], v[u]);
+                    const double dv = (double)v[u], lc = log(dv);
+                    acc[0] += dv * lc;
+#pragma unroll
+                    for (int k = 0; k < kMaxQPerPass; ++k)
+                        if (k < nq_pass) acc[1 + k] += exp(qv[k] * lc);
                 }
-                out[1 + q_off + k] = val;
-            }
         }
+        rowsum = warp_sum(rowsum);
+        if (lane == 0) pa[(size_t)t * nb + r] = rowsum;
+    }
+#pragma unroll
+    for (int i = 0; i < NA; ++i) {
+        const double sum = warp_sum_d(acc[i]);
+        if (lane == 0) sh_red[i][warp] = sum;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < nb; i += kEntropyThreads)
+        if (sh_pb[i]) atomicAdd(&pb[(size_t)t * nb + i], sh_pb[i]);
+    if (threadIdx.x < NA) {
+        double sum = 0.0;
+        for (int w = 0; w < NW; ++w) sum += sh_red[threadIdx.x][w];
+        partial[((size_t)t * nsplit + split) * NA + threadIdx.x] = sum;
+    }
+}
+
+__global__ void __launch_bounds__(kEntropyThreads)
+entropy_wide_final_kernel(int nb, const double* __restrict__ q, int nq_total, int q_off, int nq_pass, int form,
+                          const unsigned* __restrict__ pa, const unsigned* __restrict__ pb,
+                          const double* __restrict__ partial, int nsplit, double* __restrict__ mi_out,
+                          int64_t* __restrict__ nvalid, const OutMap om) {
+    constexpr int NW = kEntropyThreads / 32;
+    constexpr int NA = 1 + kMaxQPerPass;
+    constexpr int NACC = 3 * NA;
+    __shared__ double sh_red[2 * NA][NW];
+    __shared__ unsigned long long sh_n[NW];
+    const int t = blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double qv[kMaxQPerPass];
+#pragma unroll
+    for (int k = 0; k < kMaxQPerPass; ++k) qv[k] = k < nq_pass ? q[q_off + k] : 1.0;
+    double acc[2 * NA];      // [0..NA) fixed marginal, [NA..2NA) moving marginal: sum c ln c, sum c^q_k
+#pragma unroll
+    for (int i = 0; i < 2 * NA; ++i) acc[i] = 0.0;
+    unsigned long long n_local = 0;
+    for (int i = threadIdx.x; i < nb; i += kEntropyThreads) {
+        const unsigned cnt[2] = {pa[(size_t)t * nb + i], pb[(size_t)t * nb + i]};
+        n_local += cnt[0];
+#pragma unroll
+        for (int d = 0; d < 2; ++d)
+            if (cnt[d]) {
+                const double dv = (double)cnt[d], lc = log(dv);
+                acc[d * NA] += dv * lc;
+#pragma unroll
+                for (int k = 0; k < kMaxQPerPass; ++k)
+                    if (k < nq_pass) acc[d * NA + 1 + k] += exp(qv[k] * lc);
+            }
+    }
+#pragma unroll
+    for (int i = 0; i < 2 * NA; ++i) {
+        const double sum = warp_sum_d(acc[i]);
+        if (lane == 0) sh_red[i][warp] = sum;
+    }
+    {
+        unsigned lo = (unsigned)n_local, hi = (unsigned)(n_local >> 32);
+        lo = warp_sum(lo);
+        hi = warp_sum(hi);
+        if (lane == 0) sh_n[warp] = ((unsigned long long)hi << 32) + lo;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot[NACC];
+        for (int i = 0; i < NA; ++i) {
+            double sa = 0.0, sb = 0.0, sab = 0.0;
+            for (int w = 0; w < NW; ++w) { sa += sh_red[i][w]; sb += sh_red[NA + i][w]; }
+            for (int sp = 0; sp < nsplit; ++sp) sab += partial[((size_t)t * nsplit + sp) * NA + i];
+            const int base = i == 0 ? 0 : 3 + 3 * (i - 1);
+            tot[base + 0] = sa; tot[base + 1] = sb; tot[base + 2] = sab;
+        }
+        unsigned long long n = 0;
+        for (int w = 0; w < NW; ++w) n += sh_n[w];
+        entropy_finish(tot, n, t, qv, nq_pass, q_off, nq_total, form, mi_out, nvalid, om);
     }
 }
 
@@ -552,9 +682,41 @@ cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const
     int nq_pass = nq - q_off;
     if (nq_pass > kMaxQPerPass) nq_pass = kMaxQPerPass;
     if (nq_pass < 0) nq_pass = 0;
-    entropy_kernel<<<n_transforms, kEntropyThreads, 0, s>>>(hist, nb, q_dev, nq, q_off, nq_pass, form,
-                                                           mi_out, nvalid, om);
-    return cudaGetLastError();
+    if (nb <= 256) {
+        entropy_kernel<256><<<n_transforms, kEntropyThreads, 0, s>>>(hist, nb, q_dev, nq, q_off, nq_pass, form,
+                                                                    mi_out, nvalid, om);
+        return cudaGetLastError();
+    }
+    // wide: rows of every histogram split over about four waves of CTAs
+    int nsplit = (4 * 148 + n_transforms - 1) / n_transforms;
+    if (nsplit < 1) nsplit = 1;
+    if (nsplit > 64) nsplit = 64;
+    if (nsplit > nb) nsplit = nb;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    constexpr int NA = 1 + kMaxQPerPass;
+    unsigned* pab = nullptr;
+    double* partial = nullptr;
+    const size_t cnt_words = (size_t)n_transforms * nb * 2;
+    if ((e = dev_alloc((void**)&pab, cnt_words * sizeof(unsigned), dev, s)) != cudaSuccess) return e;
+    if ((e = dev_alloc((void**)&partial, (size_t)n_transforms * nsplit * NA * sizeof(double), dev, s)) != cudaSuccess) {
+        dev_free(pab, s);
+        return e;
+    }
+    unsigned* pa = pab;
+    unsigned* pb = pab + (size_t)n_transforms * nb;
+    e = cudaMemsetAsync(pab, 0, cnt_words * sizeof(unsigned), s);
+    if (e == cudaSuccess) {
+        entropy_wide_partial_kernel<<<dim3(nsplit, n_transforms), kEntropyThreads, 0, s>>>(hist, nb, q_dev, q_off, nq_pass,
+                                                                                         pa, pb, partial);
+        entropy_wide_final_kernel<<<n_transforms, kEntropyThreads, 0, s>>>(nb, q_dev, nq, q_off, nq_pass, form, pa, pb,
+                                                                          partial, nsplit, mi_out, nvalid, om);
+        e = cudaGetLastError();
+    }
+    dev_free(pab, s);
+    dev_free(partial, s);
+    return e;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -666,5 +828,97 @@ cudaError_t run_shared_atomic_probe(int nbins, int pattern, int iters, int num_s
     *updates_per_s = (double)iters * kHistThreads * num_sms / (best_ms * 1e-3);
     return cudaSuccess;
 }
+
+// ------------------------------------------------------------------------------------------------
+// Wide histograms, 256 < nbins <= kMaxBinsWide ("uses all the voxels and produces a
+// full histogram"): uint16 bin indices, the joint histogram (nb*nb*4 bytes: 64 MB at 4096
+// bins) lives in global memory and is updated with L2 reductions.  The lanes of a warp that hit the
+// same counter are merged first (__match_any_sync): the background bin alone takes a quarter of all
+// updates, and the L2 serialises updates of one address.  Same CANON-2..5 arithmetic as above.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) prebin16_kernel(const float* __restrict__ vol, uint16_t* __restrict__ bins,
+                                                       int64_t n, float lo, float scale, float top) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        bins[i] = (uint16_t)bin_index(__ldcs(vol + i), lo, scale, top);
+}
+
+cudaError_t launch_prebin16(const float* vol, uint16_t* bins, int64_t n, float lo, float scale, int nb, cudaStream_t s) {
+    if (n <= 0) return cudaSuccess;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    prebin16_kernel<<<(unsigned)blocks, 256, 0, s>>>(vol, bins, n, lo, scale, (float)(nb - 1));
+    return cudaGetLastError();
+}
+
+template <int INTERP>
+__global__ void __launch_bounds__(512) resample_hist_wide_kernel(const __grid_constant__ WideArgs a) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int fnx = a.f.nx, nb = a.nb;
+    const int rows_total = a.f.ny * a.f.nz;
+    const int pnx = a.m.nx + 2, pny = a.m.ny + 2;
+    const float fxm = (float)a.m.nx, fym = (float)a.m.ny, fzm = (float)a.m.nz;
+    const float hx = __fsub_rn(fxm, 0.5f), hy = __fsub_rn(fym, 0.5f), hz = __fsub_rn(fzm, 0.5f);
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int t = (int)(item / a.nslabs);
+        const int slab = (int)(item - (long long)t * a.nslabs);
+        const int row_lo = (int)((long long)rows_total * slab / a.nslabs);
+        const int row_hi = (int)((long long)rows_total * (slab + 1) / a.nslabs);
+        float m[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
+        uint32_t* gh = a.hist + (size_t)t * nb * nb;
+        for (int row = row_lo + warp; row < row_hi; row += nwarps) {
+            const int iz = row / a.f.ny, iy = row - iz * a.f.ny;
+            const float fy = (float)iy, fz = (float)iz;
+            const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
+            const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
+            const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
+            const uint16_t* __restrict__ frow = a.fbins + (size_t)row * fnx;
+            for (int ix0 = 0; ix0 < fnx; ix0 += 32) {          // the whole warp stays in the loop (match_any)
+                const int ix = ix0 + lane;
+                bool ok = ix < fnx;
+                unsigned key = 0xFFFFFFFFu;
+                if (ok) {
+                    const float fx = (float)ix;
+                    const float cx = __fmaf_rn(m[0], fx, rx), cy = __fmaf_rn(m[4], fx, ry), cz = __fmaf_rn(m[8], fx, rz);
+                    int b = 0;
+                    if (INTERP == MI_INTERP_NEAREST) {
+                        const float qx = floorf(__fadd_rn(cx, 0.5f)), qy = floorf(__fadd_rn(cy, 0.5f)), qz = floorf(__fadd_rn(cz, 0.5f));
+                        ok = qx >= 0.0f && qx < fxm && qy >= 0.0f && qy < fym && qz >= 0.0f && qz < fzm;
+                        if (ok) b = __ldg(a.mbins + ((size_t)(int)qz * a.m.ny + (int)qy) * a.m.nx + (int)qx);
+                    } else {
+                        ok = cx >= -0.5f && cx < hx && cy >= -0.5f && cy < hy && cz >= -0.5f && cz < hz;
+                        if (ok) {
+                            const float gx = floorf(cx), gy = floorf(cy), gz = floorf(cz);
+                            const float wx = __fsub_rn(cx, gx), wy = __fsub_rn(cy, gy), wz = __fsub_rn(cz, gz);
+                            const float* __restrict__ p = a.moving_pad + ((size_t)((int)gz + 1) * pny + ((int)gy + 1)) * pnx + ((int)gx + 1);
+                            const float* __restrict__ pz = p + (size_t)pnx * pny;
+                            const float v00 = lerp_rn(__ldg(p), __ldg(p + 1), wx), v10 = lerp_rn(__ldg(p + pnx), __ldg(p + pnx + 1), wx);
+                            const float v01 = lerp_rn(__ldg(pz), __ldg(pz + 1), wx), v11 = lerp_rn(__ldg(pz + pnx), __ldg(pz + pnx + 1), wx);
+                            const float v = lerp_rn(lerp_rn(v00, v10, wy), lerp_rn(v01, v11, wy), wz);
+                            const float tt = __fmul_rn(__fsub_rn(v, a.mlo), a.mscale);
+                            b = min(max(__float2int_rd(tt), 0), nb - 1);
+                        }
+                    }
+                    if (ok) key = (unsigned)__ldg(frow + ix) * (unsigned)nb + (unsigned)b;
+                }
+                // one reduction per distinct counter of the warp
+                const unsigned peers = __match_any_sync(0xffffffffu, key);
+                if (ok && lane == __ffs(peers) - 1) atomicAdd(&gh[key], (unsigned)__popc(peers));
+            }
+        }
+    }
+}
+
+cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s) {
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    long long grid = nitems < 4LL * num_sms ? nitems : 4LL * num_sms;
+    if (grid < 1) return cudaSuccess;
+    if (interp == MI_INTERP_NEAREST) resample_hist_wide_kernel<MI_INTERP_NEAREST><<<(unsigned)grid, 512, 0, s>>>(a);
+    else resample_hist_wide_kernel<MI_INTERP_TRILINEAR><<<(unsigned)grid, 512, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
 
 }  // namespace mi

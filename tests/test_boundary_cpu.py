@@ -95,7 +95,7 @@ def test_create_validates_arguments(lib):
             lib.mi_create(**args)
         assert ei.value.status == lib.MI_ERR_INVALID_ARG, kw
     with pytest.raises(lib.MIError) as ei:
-        lib.mi_create(v, v, sp, sp, 300)
+        lib.mi_create(v, v, sp, sp, 4097)
     assert ei.value.status == lib.MI_ERR_UNSUPPORTED
 
 

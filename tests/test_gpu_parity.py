@@ -303,6 +303,28 @@ def test_c3_c4_full_size_maps_sampled_against_oracle(mi, name):
     assert all(abs(p[d] - cfg.truth[d]) <= steps[d] * 1.0001 for d in range(3)), (p, cfg.truth)   # P11 (Shannon)
 
 
+def test_wide_histograms_above_256_bins(mi):
+    """nbins in (256, 4096]: uint16 bins, global-memory histograms, warp-aggregated updates; bins and
+    nearest-neighbour histograms bit-exact, trilinear within the flip allowance, MI within 1e-4."""
+    rng = np.random.default_rng(9)
+    fixed = ph.random_volume((37, 21, 13), 51)
+    moving = ph.random_volume((30, 25, 17), 52)
+    T = rand_physical(rng, 5)
+    for nb in (257, 1000, 4096):
+        with make_ctx(mi, fixed, moving, (1.0, 1.2, 0.9), (1.1, 1.0, 1.3), nb) as ctx:
+            b = mi.mi_get_bins(ctx, 0)
+            assert b.dtype == np.uint16 and np.array_equal(b, orc.prebin(fixed, nb, 0, 1))
+            assert np.array_equal(mi.mi_get_bins(ctx, 1), orc.prebin(moving, nb, 0, 1))
+        check_batch(mi, fixed, moving, (1.0, 1.2, 0.9), (1.1, 1.0, 1.3), nb, T, (0.5, 2.0))
+    # a head phantom pair (hot background bin: the warp aggregation path) and a translation map, which
+    # takes the generic kernel above 256 bins
+    cfg = ph.get_config("C5", res=0.25, grid_n=3)
+    c = ph.Config("wide", cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 1024, cfg.family, cfg.lo, cfg.hi,
+                  cfg.n, (0.5,), cfg.truth)
+    for interp in (0, 1):
+        check_map(mi, c, interp)
+
+
 def test_context_cycles_reuse_the_pool_and_release(mi):
     """Destroyed contexts hand their memory to the library's pool; results do not depend on what
     an earlier context left in it, and mi_release_cached_memory gives it back."""
