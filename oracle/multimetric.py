@@ -1,0 +1,64 @@
+"""CPU oracle for the multi-metric finite-difference gradient -- TEST INFRASTRUCTURE, not product code
+(same rules as oracle/__init__.py).
+
+The paper's strategy (section 4): "we can use the same histogram to produce the
+Shannon and Tsallis results [so] the reasonable strategy is to use multiple algorithms in the
+gradient descent.  In this way we can use the Tsallis in the translation gradients and Shannon in
+the rotation and scale gradients".  The paper gives no parameterisation of the combined transform
+and no difference rule; the readings taken (A18):
+
+* nine parameters p = (tx, ty, tz [mm], ax, ay, az [deg], sx, sy, sz [factors]); the transform is
+  y = R(a) S(s) x + t with R = Rz Ry Rx (the map family ROTATION_EULER_DEG), S = diag(s) (family
+  SCALE), both about the volume centre (the physical origin, CANON-1), translation last;
+* component k of the gradient is the central difference (F_k(p + d_k e_k) - F_k(p - d_k e_k)) / (2 d_k)
+  with F_k = the Tsallis MI of order q for the three translation parameters and the Shannon MI for
+  the six rotation and scale parameters; all 2*9 + 1 transforms are evaluated from one joint
+  histogram each, which yields both metrics (the "same histogram" of PAPER.md:199);
+* d_k <= 0 skips component k (gradient 0).
+
+Pins (tests/test_oracle_multimetric_pins.py): the composition against scipy's rotations and the map
+families; every gradient component against the central difference of an exhaustive map of the same
+family computed by oracle.mi_map + map_analysis.map_gradient (channel, sign, step and parameter
+order); the values at p.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle as _orc
+
+N_PARAMS = 9
+TRANSLATION_PARAMS = (0, 1, 2)          # use the Tsallis channel
+SHANNON_PARAMS = (3, 4, 5, 6, 7, 8)     # rotation and scale: use the Shannon channel
+
+
+def compose_matrix(p) -> np.ndarray:
+    """Physical 3x4 [A|t] of the nine parameters: A = R(ax,ay,az) diag(sx,sy,sz), t = (tx,ty,tz)."""
+    p = np.asarray(p, dtype=np.float64).reshape(N_PARAMS)
+    R = _orc.family_matrix(_orc.FAMILY_ROTATION_EULER_DEG, p[3:6])[:, :3]
+    A = R * p[6:9][None, :]              # column j scaled by s_j: one product per entry
+    return np.concatenate([A, p[0:3][:, None]], axis=1)
+
+
+def multimetric_gradient(fixed, fixed_spacing, moving, moving_spacing, nbins, ranges, p, delta, q,
+                         interp=_orc.INTERP_TRILINEAR, form=_orc.TSALLIS_ADDITIVE):
+    """Returns (grad[9], values[2] = (Shannon, Tsallis_q) at p)."""
+    p = np.asarray(p, dtype=np.float64).reshape(N_PARAMS)
+    delta = np.asarray(delta, dtype=np.float64).reshape(N_PARAMS)
+    Ts = [compose_matrix(p)]
+    for k in range(N_PARAMS):
+        for sgn in (+1.0, -1.0):
+            pk = p.copy()
+            pk[k] = p[k] + sgn * delta[k]
+            Ts.append(compose_matrix(pk))
+    T = np.stack(Ts)
+    fd, md = fixed.shape[::-1], moving.shape[::-1]
+    M = _orc.physical_to_index(T, fd, fixed_spacing, md, moving_spacing)
+    vals = _orc.eval_batch(fixed, moving, M, nbins, *ranges, interp, q=(float(q),), form=form)["mi"]
+    grad = np.zeros(N_PARAMS)
+    for k in range(N_PARAMS):
+        if delta[k] <= 0:
+            continue
+        ch = 1 if k in TRANSLATION_PARAMS else 0
+        grad[k] = (vals[1 + 2 * k, ch] - vals[2 + 2 * k, ch]) / (2.0 * delta[k])
+    return grad, vals[0].copy()

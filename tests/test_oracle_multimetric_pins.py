@@ -1,0 +1,66 @@
+"""Pins of the multi-metric gradient oracle (oracle/multimetric.py): no GPU, no CUDA library."""
+import numpy as np
+from scipy.spatial.transform import Rotation
+
+import oracle as orc
+from oracle import map_analysis as ma
+from oracle import multimetric as mm
+from paper_1909_10690_b200 import phantoms as ph
+
+
+def test_compose_matrix_against_scipy_and_the_map_families():
+    rng = np.random.default_rng(2)
+    for _ in range(5):
+        p = np.concatenate([rng.uniform(-9, 9, 3), rng.uniform(-25, 25, 3), rng.uniform(0.7, 1.3, 3)])
+        T = mm.compose_matrix(p)
+        # R = Rz(az) Ry(ay) Rx(ax): scipy's extrinsic "xyz" sequence
+        R = Rotation.from_euler("xyz", p[3:6], degrees=True).as_matrix()
+        assert np.allclose(T[:, :3], R @ np.diag(p[6:9]), atol=1e-14)
+        assert np.array_equal(T[:, 3], p[:3])
+        # y = R S x + t on a point
+        x = rng.normal(size=3)
+        assert np.allclose(T[:, :3] @ x + T[:, 3], R @ (p[6:9] * x) + p[:3], atol=1e-13)
+    ident = np.array([0, 0, 0, 0, 0, 0, 1, 1, 1.0])
+    assert np.array_equal(mm.compose_matrix(ident), np.eye(3, 4))
+    for fam, sl, p3 in ((0, slice(0, 3), (1.5, -2, 0.25)), (1, slice(3, 6), (4, -3, 2)), (3, slice(6, 9), (1.05, 0.97, 1.02))):
+        p = ident.copy()
+        p[sl] = p3
+        assert np.array_equal(mm.compose_matrix(p), orc.family_matrix(fam, p3))
+
+
+def test_gradient_components_equal_central_differences_of_the_family_maps():
+    """Each parameter group against an exhaustive 3x3x3 map of its own family around p (step = delta):
+    the centre node's central difference of the right channel -- Tsallis for translations, Shannon
+    for rotations and scales."""
+    cfg = ph.get_config("C1")
+    q = 0.5
+    p = np.array([0, 0, 0, 0, 0, 0, 1, 1, 1.0])
+    delta = np.array([1.0, 1.0, 0.5, 2.0, 3.0, 1.0, 0.02, 0.05, 0.03])
+    args = (cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, cfg.ranges)
+    grad, vals = mm.multimetric_gradient(*args, p, delta, q, interp=1)
+    for fam, sl, ch in ((0, slice(0, 3), 1), (1, slice(3, 6), 0), (3, slice(6, 9), 0)):
+        lo, hi = p[sl] - delta[sl], p[sl] + delta[sl]
+        r = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                       fam, lo, hi, (3, 3, 3), q=(q,), interp=1)
+        g = ma.map_gradient(r["map"][ch], lo, hi)[:, 1, 1, 1]
+        assert np.allclose(grad[sl], g, rtol=0, atol=1e-12), (fam, grad[sl], g)
+        assert np.allclose(vals, r["map"][:, 1, 1, 1], atol=1e-12)
+    # the translation components really come from the Tsallis channel: they differ from Shannon's
+    r = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                   0, p[:3] - delta[:3], p[:3] + delta[:3], (3, 3, 3), q=(q,), interp=1)
+    g_sh = ma.map_gradient(r["map"][0], p[:3] - delta[:3], p[:3] + delta[:3])[:, 1, 1, 1]
+    assert np.max(np.abs(grad[:3] - g_sh)) > 1e-3
+    # the Shannon translation gradient points towards the ground-truth shift (1.5, -2, 0.5)
+    assert np.dot(g_sh, cfg.truth) > 0
+
+
+def test_skipped_components_and_pseudo_additive_form():
+    cfg = ph.get_config("C1")
+    p = np.array([0.5, 0, 0, 1, 0, 0, 1, 1, 1.0])
+    delta = np.array([1, 0, 0, 0, 0, -1, 0.05, 0, 0.0])
+    args = (cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, cfg.ranges)
+    g0, v0 = mm.multimetric_gradient(*args, p, delta, 2.0, interp=0)
+    assert np.all(g0[[1, 2, 3, 4, 5, 7, 8]] == 0) and g0[0] != 0 and g0[6] != 0
+    g1, v1 = mm.multimetric_gradient(*args, p, delta, 2.0, interp=0, form=1)
+    assert v1[0] == v0[0] and v1[1] != v0[1]          # Shannon unchanged, Tsallis form changes
+    assert g1[6] == g0[6] and g1[0] != g0[0]
