@@ -131,6 +131,25 @@ mi_status mi_release_cached_memory(int32_t device);
  * thread (ctx == NULL).  The string is owned by the library and valid until the next call. */
 const char *mi_last_error(const mi_ctx *ctx);
 
+/* ---- multi-metric gradient ---------------------------------------------------
+ * "we can use the same histogram to produce the Shannon and Tsallis results [so] the reasonable
+ * strategy is to use multiple algorithms in the gradient descent ... the Tsallis in the translation
+ * gradients and Shannon in the rotation and scale gradients".  The paper fixes
+ * neither the parameterisation nor the difference rule; the reading (A18): nine parameters
+ * p = (tx, ty, tz [mm], ax, ay, az [deg], sx, sy, sz [factors]), transform y = R(a) S(s) x + t with
+ * R = Rz Ry Rx and S = diag(s) about the volume centre; component k is the central difference
+ * (F_k(p + d_k e_k) - F_k(p - d_k e_k)) / (2 d_k), F_k = Tsallis MI of order q (the context's Tsallis
+ * form) for k < 3 and Shannon MI for k >= 3.  All 2*9 + 1 transforms go through one mi_eval_batch,
+ * one joint histogram each. */
+
+/* Host side: physical 3x4 [A|t] of the nine parameters. */
+mi_status mi_compose_matrix(const double p[9], double T_out[12]);
+
+/* delta[k] <= 0 skips component k (grad_out[k] = 0).  grad_out: 9 doubles; value_out: NULL or 2
+ * doubles (Shannon, Tsallis_q at p).  Host pointers; q > 0 and finite. */
+mi_status mi_multimetric_gradient(mi_ctx *ctx, const double p[9], const double delta[9], double q,
+                                  mi_interp interp, double grad_out[9], double value_out[2]);
+
 /* ---- capture-range analysis of a map ---------------------------------------
  * The paper reads its maps through "the paths the gradient descent algorithm will take" and the
  * regions "converging to the central point" or "to other points not related to our goal"

@@ -27,7 +27,8 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
-           "mi_map_gradient", "mi_map_basins", "mi_probe_shared_atomic_rate", "mi_version")
+           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient",
+           "mi_probe_shared_atomic_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError("%s is missing: build it with `python -m paper_1909_10690_b200.build` "
@@ -56,6 +57,10 @@ _lib.mi_get_bins.argtypes = [_vp, C.c_int32, _vp]
 _lib.mi_get_bins.restype = C.c_int
 _lib.mi_release_cached_memory.argtypes = [C.c_int32]
 _lib.mi_release_cached_memory.restype = C.c_int
+_lib.mi_compose_matrix.argtypes = [_vp, _vp]
+_lib.mi_compose_matrix.restype = C.c_int
+_lib.mi_multimetric_gradient.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp]
+_lib.mi_multimetric_gradient.restype = C.c_int
 _lib.mi_map_gradient.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, _vp]
 _lib.mi_map_gradient.restype = C.c_int
 _lib.mi_map_basins.argtypes = [_vp, _vp, C.c_int32, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, _vp]
@@ -301,6 +306,24 @@ def mi_map_basins(m, direction=1, connectivity=26, target=-1, device=0, cuda_str
     out = {k: getattr(st, k) for k, _ in _BasinStats._fields_}
     out["label"], out["steps"] = label, steps
     return out
+
+
+def mi_compose_matrix(p) -> np.ndarray:
+    p = _f64(p, 9)
+    T = np.empty(12, dtype=np.float64)
+    st = _lib.mi_compose_matrix(_ptr(p), _ptr(T))
+    if st != MI_OK:
+        raise MIError(st, "mi_compose_matrix")
+    return T.reshape(3, 4)
+
+
+def mi_multimetric_gradient(ctx, p, delta, q, interp=MI_INTERP_TRILINEAR):
+    """(grad[9], values[2]) -- Tsallis_q differences for the translation parameters, Shannon for the rest."""
+    p, delta = _f64(p, 9), _f64(delta, 9)
+    grad, vals = np.empty(9, dtype=np.float64), np.empty(2, dtype=np.float64)
+    _check(ctx, _lib.mi_multimetric_gradient(ctx.handle, _ptr(p), _ptr(delta), float(q), int(interp), _ptr(grad),
+                                             _ptr(vals)))
+    return grad, vals
 
 
 def mi_release_cached_memory(device=0) -> None:

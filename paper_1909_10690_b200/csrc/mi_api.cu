@@ -769,6 +769,62 @@ mi_status mi_eval_batch(mi_ctx* c, const double* T, int64_t N, const double* q, 
     return eval_core(c, hM, N, q, nq, (int)interp, mi_out, hist_out, nvalid_out, nullptr, nullptr);
 }
 
+mi_status mi_compose_matrix(const double p[9], double T_out[12]) {
+    if (p == nullptr || T_out == nullptr) return MI_ERR_INVALID_ARG;
+    for (int i = 0; i < 9; ++i)
+        if (!std::isfinite(p[i])) return MI_ERR_INVALID_ARG;
+    mi::compose_matrix(p, T_out);
+    return MI_OK;
+}
+
+mi_status mi_multimetric_gradient(mi_ctx* c, const double p[9], const double delta[9], double q, mi_interp interp,
+                                  double grad_out[9], double value_out[2]) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (!p || !delta || !grad_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
+    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
+        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
+    mi_status st = validate_q(c, &q, 1);
+    if (st != MI_OK) return st;
+    for (int i = 0; i < 9; ++i)
+        if (!std::isfinite(p[i]) || !std::isfinite(delta[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite parameter");
+    // transform 0 = p; then p + d_k e_k, p - d_k e_k for every parameter with d_k > 0
+    int slot[9];
+    int64_t N = 1;
+    for (int k = 0; k < 9; ++k) {
+        slot[k] = delta[k] > 0.0 ? (int)N : -1;
+        if (delta[k] > 0.0) N += 2;
+    }
+    std::vector<float> hM((size_t)N * 12);
+    auto put = [&](int64_t t, const double pk[9]) {
+        double T[12];
+        mi::compose_matrix(pk, T);
+        mi::index_affine(T, c->fd, c->fs, c->md, c->ms, hM.data() + t * 12);
+    };
+    put(0, p);
+    for (int k = 0; k < 9; ++k) {
+        if (slot[k] < 0) continue;
+        double pk[9];
+        for (int i = 0; i < 9; ++i) pk[i] = p[i];
+        pk[k] = p[k] + delta[k];
+        put(slot[k], pk);
+        pk[k] = p[k] - delta[k];
+        put(slot[k] + 1, pk);
+    }
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    std::vector<double> vals((size_t)N * 2);
+    st = eval_core(c, hM, N, &q, 1, (int)interp, vals.data(), nullptr, nullptr, nullptr, nullptr);
+    if (st != MI_OK) return st;
+    for (int k = 0; k < 9; ++k) {
+        grad_out[k] = 0.0;
+        if (slot[k] < 0) continue;
+        const int ch = k < 3 ? 1 : 0;   // Tsallis for the translation parameters, Shannon for the rest
+        grad_out[k] = (vals[(size_t)slot[k] * 2 + ch] - vals[(size_t)(slot[k] + 1) * 2 + ch]) / (2.0 * delta[k]);
+    }
+    if (value_out) { value_out[0] = vals[0]; value_out[1] = vals[1]; }
+    return MI_OK;
+}
+
 mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
                  const double* q, int32_t nq, mi_interp interp, double* map_out, int64_t* argmax_out) {
     if (!c) return MI_ERR_INVALID_ARG;

@@ -28,6 +28,17 @@ static void matmul3(const double a[3][3], const double b[3][3], double c[3][3]) 
         }
 }
 
+// Nine-parameter transform of the multi-metric gradient (A18): y = R(a) S(s) x + t with
+// p = (tx,ty,tz mm, ax,ay,az deg, sx,sy,sz), R = Rz Ry Rx as in MI_FAMILY_ROTATION_EULER_DEG.
+int family_matrix(int family, const double p[3], double T[12]);
+void compose_matrix(const double p[9], double T[12]) {
+    family_matrix(MI_FAMILY_ROTATION_EULER_DEG, p + 3, T);
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j) T[i * 4 + j] = T[i * 4 + j] * p[6 + j];   // column j scaled by s_j
+        T[i * 4 + 3] = p[i];
+    }
+}
+
 // Transform families of the maps (translation 3.1, rotation 3.2, scale 3.3).
 int family_matrix(int family, const double p[3], double T[12]) {
     set_identity(T);

@@ -24,6 +24,7 @@ constexpr int kMaxBinsWide = 4096;   // largest nbins (above 256: uint16 bins, g
 
 // ---- host-side double math (mi_host.cpp; compiled with -ffp-contract=off) --------------------
 int family_matrix(int family, const double p[3], double T[12]);
+void compose_matrix(const double p[9], double T[12]);
 void index_affine(const double T[12], const int32_t fd[3], const double fs[3], const int32_t md[3],
                   const double ms[3], float out[12]);
 float bin_scale(int nbins, float lo, float hi);

@@ -82,6 +82,16 @@ def test_family_matrix_equals_oracle(lib):
         lib.mi_family_matrix(0, (np.nan, 0, 0))
 
 
+def test_compose_matrix_bit_for_bit_against_oracle(lib):
+    from oracle import multimetric as mm
+    rng = np.random.default_rng(4)
+    for _ in range(50):
+        p = np.concatenate([rng.uniform(-20, 20, 3), rng.uniform(-40, 40, 3), rng.uniform(0.5, 1.5, 3)])
+        assert np.array_equal(lib.mi_compose_matrix(p), mm.compose_matrix(p))
+    with pytest.raises(lib.MIError):
+        lib.mi_compose_matrix([0, 0, 0, 0, np.nan, 0, 1, 1, 1])
+
+
 def test_create_validates_arguments(lib):
     v = np.zeros((4, 4, 4), dtype=np.float32)
     sp = (1.0, 1.0, 1.0)

@@ -126,3 +126,26 @@ def test_capture_range_of_a_real_map_shannon_and_tsallis(mi):
     p = [cfg.lo[d] + k * (cfg.hi[d] - cfg.lo[d]) / (cfg.n[d] - 1) for d, k in enumerate((k0, k1, k2))]
     assert max(abs(p[d] - cfg.truth[d]) for d in range(3)) <= 1.0
     assert 0.0 < sh["capture_fraction"] <= 1.0
+
+
+def test_multimetric_gradient_equals_oracle(mi):
+    """mi_multimetric_gradient (one mi_eval_batch of 2*9 + 1 transforms) against oracle/multimetric.py: MI values
+    within 1e-4 nats, so each central difference within 1e-4 / delta_k; skipped components are exactly 0."""
+    from oracle import multimetric as mm
+    cfg = ph.get_config("C1")
+    args = (cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, cfg.ranges)
+    cases = [(np.array([0, 0, 0, 0, 0, 0, 1, 1, 1.0]), np.array([1.0, 1.0, 0.5, 2.0, 3.0, 1.0, 0.02, 0.05, 0.03]), 0.5, 0),
+             (np.array([1.2, -1.5, 0.4, 3, -2, 1, 1.03, 0.98, 1.01]), np.array([0.5, 0.5, 0.5, 1, 1, 1, 0.01, 0.01, 0.01]), 2.0, 0),
+             (np.array([0.5, 0, 0, 1, 0, 0, 1, 1, 1.0]), np.array([1, 0, 0, 0, 0, -1, 0.05, 0, 0.0]), 2.0, 1)]
+    with mi.mi_create(cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        for p, delta, q, form in cases:
+            mi.mi_set_tsallis_form(ctx, form)
+            for interp in (0, 1):
+                g_ref, v_ref = mm.multimetric_gradient(*args, p, delta, q, interp=interp, form=form)
+                g, v = mi.mi_multimetric_gradient(ctx, p, delta, q, interp)
+                assert np.max(np.abs(v - v_ref)) <= 1e-4
+                tol = np.where(delta > 0, 1e-4 / np.maximum(delta, 1e-300), 0.0)
+                assert np.all(np.abs(g - g_ref) <= tol), (g, g_ref)
+                assert np.all(g[delta <= 0] == 0)
+        with pytest.raises(mi.MIError):
+            mi.mi_multimetric_gradient(ctx, cases[0][0], cases[0][1], -1.0, 1)
