@@ -76,3 +76,56 @@ def map_sharded(map_fn, lo, hi, n, nch: int, rank: int, world: int, dist=None, d
     idx = torch.arange(flat.shape[1], device=flat.device).expand_as(flat)
     argmax = torch.where(flat == best, idx, torch.full_like(idx, flat.shape[1])).min(dim=1).values
     return full, argmax
+
+
+# ---- composite grids over all 12 affine degrees of freedom ---------------------------
+def affine12_count() -> int:
+    return 3 ** 12
+
+
+def affine12_grid(delta12, begin: int = 0, end: int | None = None) -> np.ndarray:
+    """The paper's 12-dimensional exhaustive idea: "Using 12 dimensions and only 3 individual parameter
+    (i.e. a minus parameter, a plus parameter and zero) in each dimension or direction we have
+    3^12 = 531441" measurements.  Read literally on the 12 entries of the physical 3x4
+    [A|t]: transform number i has entry k (row-major; k = 3, 7, 11 are the translations) equal to the
+    identity's entry plus (digit_k(i) - 1) * delta12[k], where digit_k is the k-th base-3 digit of i
+    (entry 0 fastest).  Returns transforms [begin, end) as an (end - begin, 3, 4) float64 array; the
+    identity is number (3^12 - 1) / 2.  Host logic only: the matrices go to mi_eval_batch."""
+    d = np.asarray(delta12, dtype=np.float64).reshape(12)
+    end = affine12_count() if end is None else int(end)
+    idx = np.arange(int(begin), end, dtype=np.int64)
+    T = np.tile(np.eye(3, 4).reshape(1, 12), (idx.size, 1))
+    for k in range(12):
+        digit = (idx // 3 ** k) % 3
+        T[:, k] += (digit - 1).astype(np.float64) * d[k]
+    return T.reshape(-1, 3, 4)
+
+
+def batch_bounds(n: int, rank: int, world: int):
+    """Contiguous [begin, end) share of n independent transforms for `rank` (sizes differ by at most one)."""
+    return slab_bounds(n, rank, world)
+
+
+def batch_sharded(eval_fn, n: int, nch: int, rank: int, world: int, dist=None, device=None):
+    """Evaluate transforms [0, n) split across ranks: `eval_fn(begin, end) -> (end - begin, nch)` values for
+    this rank's share; returns the (n, nch) float64 result on every rank (one all-gather of doubles)."""
+    import torch
+
+    b, e = batch_bounds(n, rank, world)
+    base = (int(n) + world - 1) // world
+    local = torch.zeros((base, nch), dtype=torch.float64, device=device)
+    if e > b:
+        v = eval_fn(b, e)
+        v = v if isinstance(v, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(v, dtype=np.float64))
+        local[: e - b] = v.to(local.device).reshape(e - b, nch)
+    if world == 1 or dist is None:
+        parts = [local]
+    else:
+        parts = [torch.empty_like(local) for _ in range(world)]
+        dist.all_gather(parts, local)
+    full = torch.empty((int(n), nch), dtype=torch.float64, device=local.device)
+    for r in range(len(parts)):
+        rb, re = batch_bounds(n, r, world)
+        if re > rb:
+            full[rb:re] = parts[r][: re - rb]
+    return full

@@ -325,6 +325,33 @@ def test_wide_histograms_above_256_bins(mi):
         check_map(mi, c, interp)
 
 
+def test_affine12_composite_grid_full_3_to_the_12(mi):
+    """The paper's 12-dimensional exhaustive idea: all 3^12 = 531441 combinations of a minus,
+    zero and plus step on the 12 entries of [A|t], evaluated in full on the C1 pair through
+    mi_eval_batch; sampled transforms against the oracle, the identity against the map's centre."""
+    from paper_1909_10690_b200 import sharding as sh
+    cfg = ph.get_config("C1")
+    d = np.array([0.03, 0.02, 0.02, 1.0, 0.02, 0.03, 0.02, 1.0, 0.02, 0.02, 0.03, 1.0])
+    n = sh.affine12_count()
+    vals = np.empty((n, 2))
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        for b in range(0, n, 65536):
+            e = min(n, b + 65536)
+            vals[b:e] = mi.mi_eval_batch(ctx, sh.affine12_grid(d, b, e), (0.5,), 1)[0]
+        centre = mi.mi_eval_batch(ctx, np.eye(3, 4)[None], (0.5,), 1)[0][0]
+    assert np.array_equal(vals[(n - 1) // 2], centre)
+    rng = np.random.default_rng(12)
+    pick = np.concatenate([[0, n - 1, (n - 1) // 2], rng.integers(0, n, 13)])
+    T = np.stack([sh.affine12_grid(d, int(i), int(i) + 1)[0] for i in pick])
+    M = orc.physical_to_index(T, (32,) * 3, cfg.fixed_spacing, (32,) * 3, cfg.moving_spacing)
+    ref = orc.eval_batch(cfg.fixed, cfg.moving, M, cfg.nbins, 0, 1, 0, 1, 1, q=(0.5,))["mi"]
+    assert np.max(np.abs(vals[pick] - ref)) <= MI_TOL
+    # the Shannon arg max moves the translation entries towards the ground truth (1.5, -2, 0.5)
+    best = int(np.argmax(vals[:, 0]))
+    digits = [(best // 3 ** k) % 3 - 1 for k in (3, 7, 11)]
+    assert digits[0] == 1 and digits[1] == -1
+
+
 def test_context_cycles_reuse_the_pool_and_release(mi):
     """Destroyed contexts hand their memory to the library's pool; results do not depend on what
     an earlier context left in it, and mi_release_cached_memory gives it back."""

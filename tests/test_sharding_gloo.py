@@ -84,3 +84,45 @@ def test_sharded_map_equals_single_rank_map_gloo(world, tmp_path):
         assert m.shape == ref["map"].shape
         assert np.max(np.abs(m - ref["map"])) <= 1e-12       # integer-voxel C1 grid: identical nodes
         assert np.array_equal(am, ref["argmax"])
+
+
+# ------------------------------------------------------------------------------------------------ 12-DOF composite grid
+def test_affine12_grid_is_the_3_to_the_12_product():
+    d = np.arange(1, 13) * 0.01
+    assert sh.affine12_count() == 531441
+    mid = (3 ** 12 - 1) // 2
+    assert np.array_equal(sh.affine12_grid(d, mid, mid + 1)[0], np.eye(3, 4))
+    first, last = sh.affine12_grid(d, 0, 1)[0], sh.affine12_grid(d, 3 ** 12 - 1, 3 ** 12)[0]
+    assert np.allclose(first, np.eye(3, 4) - d.reshape(3, 4)) and np.allclose(last, np.eye(3, 4) + d.reshape(3, 4))
+    # entry k moves with period 3^k; a chunk equals the same rows of a bigger chunk
+    T = sh.affine12_grid(d, 0, 3 ** 5)
+    for k in range(5):
+        col = T.reshape(-1, 12)[:, k] - np.eye(3, 4).reshape(12)[k]
+        want = ((np.arange(3 ** 5) // 3 ** k) % 3 - 1) * d[k]
+        assert np.allclose(col, want)
+    assert np.array_equal(sh.affine12_grid(d, 100, 140), sh.affine12_grid(d, 0, 200)[100:140])
+    assert len(np.unique(sh.affine12_grid(d, 0, 3 ** 6).reshape(-1, 12), axis=0)) == 3 ** 6
+
+
+def _batch_worker(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    import torch.distributed as dist
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    n = 83
+
+    def eval_fn(b, e):
+        i = np.arange(b, e, dtype=np.float64)
+        return np.stack([i * i, -i], axis=1)
+
+    full = sh.batch_sharded(eval_fn, n, 2, rank, world, dist=dist)
+    np.save(os.path.join(out_dir, "batch_%d.npy" % rank), full.numpy())
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_batch_sharded_gathers_every_share_gloo(world, tmp_path):
+    mp.spawn(_batch_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    i = np.arange(83, dtype=np.float64)
+    for r in range(world):
+        assert np.array_equal(np.load(tmp_path / ("batch_%d.npy" % r)), np.stack([i * i, -i], axis=1))
