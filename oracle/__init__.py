@@ -64,6 +64,14 @@ def lib():
                               C.c_float, C.c_float, C.c_float, C.c_int, _f64p, _f64p, _i32p, _f64p,
                               C.c_int, C.c_int, C.c_int, _f64p, _i64p]
         L.orc_map.restype = C.c_int
+        L.orc_eval_batch_masked.argtypes = [_f32p, _i32p, _f32p, _i32p, _f32p, C.c_int64, C.c_int,
+                                            C.c_float, C.c_float, C.c_float, C.c_float, C.c_int, _f64p,
+                                            C.c_int, C.c_int, _u8p, _f64p, _u32p, _i64p]
+        L.orc_eval_batch_masked.restype = C.c_int
+        L.orc_map_masked.argtypes = [_f32p, _i32p, _f64p, _f32p, _i32p, _f64p, C.c_int, C.c_float,
+                                     C.c_float, C.c_float, C.c_float, C.c_int, _f64p, _f64p, _i32p, _f64p,
+                                     C.c_int, C.c_int, C.c_int, _u8p, _f64p, _i64p]
+        L.orc_map_masked.restype = C.c_int
         L.orc_max_threads.argtypes = []
         L.orc_max_threads.restype = C.c_int
         _lib = L
@@ -167,9 +175,19 @@ def entropies(hist, q=None, form: int = TSALLIS_ADDITIVE, detail: bool = False):
     return (out, det) if detail else out
 
 
+def _mask(mask, fx):
+    """uint8 mask of the fixed volume's shape (non-zero = the voxel takes part), or None."""
+    if mask is None:
+        return None
+    m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.uint8)
+    assert m.shape == fx.shape
+    return m
+
+
 def eval_batch(fixed, moving, M, nb, flo, fhi, mlo, mhi, interp, q=None, form=TSALLIS_ADDITIVE,
-               want_hist: bool = False):
-    """M: (N, 3, 4) float32 index-space transforms -> dict(mi (N,1+nq), nvalid (N,), hist?, threads)."""
+               want_hist: bool = False, mask=None):
+    """M: (N, 3, 4) float32 index-space transforms -> dict(mi (N,1+nq), nvalid (N,), hist?, threads).
+    mask: optional subset of the fixed voxels that takes part (reading A19)."""
     fx, mv = _vol(fixed), _vol(moving)
     fd, md = _dims(fx), _dims(mv)
     M = np.ascontiguousarray(M, dtype=np.float32).reshape(-1, 12)
@@ -178,10 +196,12 @@ def eval_batch(fixed, moving, M, nb, flo, fhi, mlo, mhi, interp, q=None, form=TS
     mi = np.empty((N, 1 + nq), dtype=np.float64)
     nvalid = np.empty(N, dtype=np.int64)
     hist = np.empty((N, nb, nb), dtype=np.uint32) if want_hist else None
-    threads = lib().orc_eval_batch(_p(fx, _f32p), _p(fd, _i32p), _p(mv, _f32p), _p(md, _i32p),
-                                   _p(M, _f32p), N, int(nb), flo, fhi, mlo, mhi, int(interp),
-                                   _p(qa, _f64p), nq, int(form), _p(mi, _f64p),
-                                   _p(hist, _u32p) if want_hist else None, _p(nvalid, _i64p))
+    mk = _mask(mask, fx)
+    threads = lib().orc_eval_batch_masked(_p(fx, _f32p), _p(fd, _i32p), _p(mv, _f32p), _p(md, _i32p),
+                                          _p(M, _f32p), N, int(nb), flo, fhi, mlo, mhi, int(interp),
+                                          _p(qa, _f64p), nq, int(form),
+                                          _p(mk.reshape(-1), _u8p) if mk is not None else None, _p(mi, _f64p),
+                                          _p(hist, _u32p) if want_hist else None, _p(nvalid, _i64p))
     return {"mi": mi, "nvalid": nvalid, "hist": hist, "threads": int(threads)}
 
 
@@ -192,7 +212,7 @@ def physical_to_index(T, fixed_dims, fixed_spacing, moving_dims, moving_spacing)
 
 
 def mi_map(fixed, fixed_spacing, moving, moving_spacing, nb, flo, fhi, mlo, mhi, family, lo, hi, n,
-           q=None, form=TSALLIS_ADDITIVE, interp=INTERP_TRILINEAR):
+           q=None, form=TSALLIS_ADDITIVE, interp=INTERP_TRILINEAR, mask=None):
     """Exhaustive map: dict(map (1+nq, n2, n1, n0), argmax (1+nq,), threads)."""
     fx, mv = _vol(fixed), _vol(moving)
     fd, md = _dims(fx), _dims(mv)
@@ -204,8 +224,10 @@ def mi_map(fixed, fixed_spacing, moving, moving_spacing, nb, flo, fhi, mlo, mhi,
     qa, nq = _q(q)
     out = np.empty((1 + nq, int(n[2]), int(n[1]), int(n[0])), dtype=np.float64)
     am = np.empty(1 + nq, dtype=np.int64)
-    threads = lib().orc_map(_p(fx, _f32p), _p(fd, _i32p), _p(fs, _f64p), _p(mv, _f32p), _p(md, _i32p),
-                            _p(ms, _f64p), int(nb), flo, fhi, mlo, mhi, int(family), _p(lo, _f64p),
-                            _p(hi, _f64p), _p(n, _i32p), _p(qa, _f64p), nq, int(form), int(interp),
-                            _p(out, _f64p), _p(am, _i64p))
+    mk = _mask(mask, fx)
+    threads = lib().orc_map_masked(_p(fx, _f32p), _p(fd, _i32p), _p(fs, _f64p), _p(mv, _f32p), _p(md, _i32p),
+                                   _p(ms, _f64p), int(nb), flo, fhi, mlo, mhi, int(family), _p(lo, _f64p),
+                                   _p(hi, _f64p), _p(n, _i32p), _p(qa, _f64p), nq, int(form), int(interp),
+                                   _p(mk.reshape(-1), _u8p) if mk is not None else None,
+                                   _p(out, _f64p), _p(am, _i64p))
     return {"map": out, "argmax": am, "threads": int(threads)}

@@ -244,9 +244,11 @@ void orc_resample(const int32_t fd[3], const float* moving, const int32_t md[3],
 
 // CANON-6: joint histogram h[a*nb + b] of (bin u(x), bin v(T(x))) over every fixed voxel whose
 // sample is inside the moving volume (reading A5).  Returns the number of valid samples.
-int64_t orc_joint_hist(const float* fixed, const int32_t fd[3], const float* moving,
-                       const int32_t md[3], const float M[12], int nb, float flo, float fhi,
-                       float mlo, float mhi, int interp, uint32_t* hist) {
+// mask (may be NULL): one byte per fixed voxel; voxels with mask == 0 take no part (reading A19: the
+// random-sampling question of PAPER.md:212 -- the sampled subset is an INPUT, drawn by the harness).
+int64_t orc_joint_hist_masked(const float* fixed, const int32_t fd[3], const float* moving,
+                              const int32_t md[3], const float M[12], int nb, float flo, float fhi,
+                              float mlo, float mhi, int interp, const uint8_t* mask, uint32_t* hist) {
     std::memset(hist, 0, sizeof(uint32_t) * (size_t)nb * nb);
     const float fscale = bin_scale(nb, flo, fhi);
     const float mscale = bin_scale(nb, mlo, mhi);
@@ -255,16 +257,23 @@ int64_t orc_joint_hist(const float* fixed, const int32_t fd[3], const float* mov
         for (int iy = 0; iy < fd[1]; ++iy)
             for (int ix = 0; ix < fd[0]; ++ix) {
                 float c[3], v;
+                size_t i = ((size_t)iz * fd[1] + iy) * fd[0] + ix;
+                if (mask != nullptr && mask[i] == 0) continue;
                 coords(M, ix, iy, iz, c);
                 bool ok = interp ? sample_tri(moving, md, c, &v) : sample_nn(moving, md, c, &v);
                 if (!ok) continue;
-                size_t i = ((size_t)iz * fd[1] + iy) * fd[0] + ix;
                 int a = bin_of(fixed[i], flo, fscale, nb);
                 int b = bin_of(v, mlo, mscale, nb);
                 hist[(size_t)a * nb + b] += 1;
                 ++nvalid;
             }
     return nvalid;
+}
+
+int64_t orc_joint_hist(const float* fixed, const int32_t fd[3], const float* moving,
+                       const int32_t md[3], const float M[12], int nb, float flo, float fhi,
+                       float mlo, float mhi, int interp, uint32_t* hist) {
+    return orc_joint_hist_masked(fixed, fd, moving, md, M, nb, flo, fhi, mlo, mhi, interp, nullptr, hist);
 }
 
 // Pin P12: the same histogram with ALL geometry in fp64 (index-space matrix M64 given in double,
@@ -365,10 +374,10 @@ void orc_entropies(const uint32_t* hist, int nb, const double* q, int nq, int fo
 // N index-space transforms -> N x (1+nq) MI values (+ optional histograms and valid counts).
 // OpenMP over transforms, one private histogram per thread; this is the timed CPU baseline.
 // Returns the number of threads used.
-int orc_eval_batch(const float* fixed, const int32_t fd[3], const float* moving, const int32_t md[3],
-                   const float* M, int64_t N, int nb, float flo, float fhi, float mlo, float mhi,
-                   int interp, const double* q, int nq, int form, double* mi_out,
-                   uint32_t* hist_out, int64_t* nvalid_out) {
+int orc_eval_batch_masked(const float* fixed, const int32_t fd[3], const float* moving, const int32_t md[3],
+                          const float* M, int64_t N, int nb, float flo, float fhi, float mlo, float mhi,
+                          int interp, const double* q, int nq, int form, const uint8_t* mask, double* mi_out,
+                          uint32_t* hist_out, int64_t* nvalid_out) {
     int nthreads = 1;
 #ifdef _OPENMP
     nthreads = omp_get_max_threads();
@@ -378,8 +387,8 @@ int orc_eval_batch(const float* fixed, const int32_t fd[3], const float* moving,
         std::vector<uint32_t> h((size_t)nb * nb);
 #pragma omp for schedule(dynamic, 1)
         for (int64_t t = 0; t < N; ++t) {
-            int64_t nv = orc_joint_hist(fixed, fd, moving, md, M + t * 12, nb, flo, fhi, mlo, mhi,
-                                        interp, h.data());
+            int64_t nv = orc_joint_hist_masked(fixed, fd, moving, md, M + t * 12, nb, flo, fhi, mlo, mhi,
+                                               interp, mask, h.data());
             orc_entropies(h.data(), nb, q, nq, form, mi_out + t * (1 + nq), nullptr);
             if (hist_out) std::memcpy(hist_out + (size_t)t * nb * nb, h.data(), sizeof(uint32_t) * h.size());
             if (nvalid_out) nvalid_out[t] = nv;
@@ -388,13 +397,22 @@ int orc_eval_batch(const float* fixed, const int32_t fd[3], const float* moving,
     return nthreads;
 }
 
+int orc_eval_batch(const float* fixed, const int32_t fd[3], const float* moving, const int32_t md[3],
+                   const float* M, int64_t N, int nb, float flo, float fhi, float mlo, float mhi,
+                   int interp, const double* q, int nq, int form, double* mi_out,
+                   uint32_t* hist_out, int64_t* nvalid_out) {
+    return orc_eval_batch_masked(fixed, fd, moving, md, M, N, nb, flo, fhi, mlo, mhi, interp, q, nq, form, nullptr,
+                                 mi_out, hist_out, nvalid_out);
+}
+
 // Exhaustive map: grid value k on axis d is lo[d] + k (hi[d]-lo[d])/(n[d]-1);
 // map_out is (1+nq) x n[2] x n[1] x n[0], channel-major, p0 fastest; argmax per channel with ties
 // to the lowest linear index (eq. 3).  Returns the number of threads used.
-int orc_map(const float* fixed, const int32_t fd[3], const double fs[3], const float* moving,
-            const int32_t md[3], const double ms[3], int nb, float flo, float fhi, float mlo,
-            float mhi, int family, const double lo[3], const double hi[3], const int32_t n[3],
-            const double* q, int nq, int form, int interp, double* map_out, int64_t* argmax_out) {
+int orc_map_masked(const float* fixed, const int32_t fd[3], const double fs[3], const float* moving,
+                   const int32_t md[3], const double ms[3], int nb, float flo, float fhi, float mlo,
+                   float mhi, int family, const double lo[3], const double hi[3], const int32_t n[3],
+                   const double* q, int nq, int form, int interp, const uint8_t* mask, double* map_out,
+                   int64_t* argmax_out) {
     const int64_t NT = (int64_t)n[0] * n[1] * n[2];
     std::vector<float> M((size_t)NT * 12);
     for (int k2 = 0; k2 < n[2]; ++k2)
@@ -409,8 +427,8 @@ int orc_map(const float* fixed, const int32_t fd[3], const double fs[3], const f
                 orc_index_affine(T, fd, fs, md, ms, M.data() + t * 12);
             }
     std::vector<double> mi((size_t)NT * (1 + nq));
-    int nthreads = orc_eval_batch(fixed, fd, moving, md, M.data(), NT, nb, flo, fhi, mlo, mhi, interp,
-                                  q, nq, form, mi.data(), nullptr, nullptr);
+    int nthreads = orc_eval_batch_masked(fixed, fd, moving, md, M.data(), NT, nb, flo, fhi, mlo, mhi, interp,
+                                         q, nq, form, mask, mi.data(), nullptr, nullptr);
     for (int ch = 0; ch < 1 + nq; ++ch) {
         int64_t best = 0;
         for (int64_t t = 0; t < NT; ++t) {
@@ -421,6 +439,14 @@ int orc_map(const float* fixed, const int32_t fd[3], const double fs[3], const f
         if (argmax_out) argmax_out[ch] = best;
     }
     return nthreads;
+}
+
+int orc_map(const float* fixed, const int32_t fd[3], const double fs[3], const float* moving,
+            const int32_t md[3], const double ms[3], int nb, float flo, float fhi, float mlo,
+            float mhi, int family, const double lo[3], const double hi[3], const int32_t n[3],
+            const double* q, int nq, int form, int interp, double* map_out, int64_t* argmax_out) {
+    return orc_map_masked(fixed, fd, fs, moving, md, ms, nb, flo, fhi, mlo, mhi, family, lo, hi, n, q, nq, form,
+                          interp, nullptr, map_out, argmax_out);
 }
 
 int orc_max_threads(void) {
