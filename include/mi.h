@@ -118,6 +118,13 @@ mi_status mi_map(mi_ctx *ctx, mi_family family, const double lo[3], const double
                  const int32_t n[3], const double *q, int32_t nq, mi_interp interp,
                  double *map_out, int64_t *argmax_out);
 
+/* Restrict the metric to a subset of the fixed voxels (the random-sampling question of
+ * "ITK Mattes uses a random sampling of the image ... while MICUDA uses all the voxels";
+ * DESIGN.md A19).  mask: nx*ny*nz bytes in the fixed volume's layout, host or device, non-zero = the voxel
+ * takes part; NULL restores all voxels.  The subset is an input (the caller draws it); it applies to every
+ * later mi_eval_batch / mi_map / mi_multimetric_gradient of the context.  The mask is copied. */
+mi_status mi_set_fixed_mask(mi_ctx *ctx, const uint8_t *mask);
+
 /* Release the context.  Its device memory goes back to a library-level stream-ordered pool (one per
  * device) that keeps it cached for the next context -- the multi-GB scratch of a map is then not
  * mapped and unmapped by the driver on every create/destroy cycle.  NULL is a no-op. */

@@ -25,7 +25,7 @@ MI_TSALLIS_ADDITIVE, MI_TSALLIS_PSEUDO_ADDITIVE = 0, 1
 _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_ERR_OUT_OF_MEMORY",
            4: "MI_ERR_CUDA", 5: "MI_ERR_INTERNAL"}
 
-EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
+EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
            "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient",
            "mi_probe_shared_atomic_rate", "mi_version")
@@ -41,6 +41,8 @@ _lib.mi_create.argtypes = [C.POINTER(_vp), _vp, _vp, _vp, _vp, _vp, _vp, C.c_int
 _lib.mi_create.restype = C.c_int
 _lib.mi_set_tsallis_form.argtypes = [_vp, C.c_int]
 _lib.mi_set_tsallis_form.restype = C.c_int
+_lib.mi_set_fixed_mask.argtypes = [_vp, _vp]
+_lib.mi_set_fixed_mask.restype = C.c_int
 _lib.mi_eval_batch.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, C.c_int, _vp, _vp, _vp]
 _lib.mi_eval_batch.restype = C.c_int
 _lib.mi_map.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp]
@@ -306,6 +308,20 @@ def mi_map_basins(m, direction=1, connectivity=26, target=-1, device=0, cuda_str
     out = {k: getattr(st, k) for k, _ in _BasinStats._fields_}
     out["label"], out["steps"] = label, steps
     return out
+
+
+def mi_set_fixed_mask(ctx, mask) -> None:
+    """mask: None (all voxels) or an array / tensor of the fixed volume's shape, non-zero = voxel takes part."""
+    if mask is None:
+        _check(ctx, _lib.mi_set_fixed_mask(ctx.handle, None))
+        return
+    if _is_torch(mask):
+        import torch
+        m = (mask != 0).to(torch.uint8).contiguous()
+    else:
+        m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.uint8)
+    assert tuple(m.shape) == ctx.fixed_dims[::-1]
+    _check(ctx, _lib.mi_set_fixed_mask(ctx.handle, _ptr(m)))
 
 
 def mi_compose_matrix(p) -> np.ndarray:

@@ -28,6 +28,8 @@ struct mi_ctx {
     int* d_rank_inv = nullptr;          // 256: rank -> fixed bin
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
+    uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
+    unsigned rare_cap = 0;              // capacity of d_rare (entries)
     bool wide = false;                  // nbins > 256: uint16 bins, global-memory histograms, generic kernel only
     uint16_t* d_fbins16 = nullptr;
     uint16_t* d_mbins16 = nullptr;
@@ -421,6 +423,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         mi::ResampleArgs a;
         a.fbins_ranked = c->d_fbins_ranked;
         a.rank_inv = c->d_rank_inv;
+        a.mask_bits = c->d_mask_bits;
         a.moving_pad = c->d_moving_pad;
         a.mbins = c->d_mbins;
         a.rows_smem = c->rows_smem;
@@ -451,6 +454,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             mi::WideArgs w;
             w.fbins = c->d_fbins16;
             w.mbins = c->d_mbins16;
+            w.mask_bits = c->d_mask_bits;
             w.moving_pad = c->d_moving_pad;
             w.M = a.M;
             w.hist = hist;
@@ -687,9 +691,10 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
                 for (int a = 0; a < 256; ++a)
                     if ((int)h_rank[a] >= c->zrows_real) n_rare += h_counts[a];
                 c->n_rare = (unsigned)n_rare;
+                c->rare_cap = (unsigned)n_rare;
                 if ((e = dev_alloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
                 if ((e = cudaMemsetAsync(d_counts, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
-                if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
+                if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, nullptr, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
                                                c->d_fb_pitched, c->d_rare, reinterpret_cast<unsigned*>(d_counts), c->n_rare, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pitch fixed bins"); break; }
             }
         }
@@ -711,7 +716,7 @@ void mi_destroy(mi_ctx* c) {
     if (!c) return;
     DeviceGuard guard(c->device);
     if (guard.ok) {
-        void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_fbins16, c->d_mbins16, c->d_mbins,
+        void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mask_bits, c->d_fbins16, c->d_mbins16, c->d_mbins,
                         c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
@@ -731,6 +736,45 @@ mi_status mi_release_cached_memory(int32_t device) {
     if (mi::g_pools[device] == nullptr) return MI_OK;
     if (cudaMemPoolTrimTo(mi::g_pools[device], 0) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
     return MI_OK;
+}
+
+mi_status mi_set_fixed_mask(mi_ctx* c, const uint8_t* mask) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    cudaStream_t s = c->stream;
+    uint8_t* d_mask = nullptr;
+    unsigned* d_count = nullptr;
+    mi_status st = MI_OK;
+    do {
+        cudaError_t e;
+        if (mask != nullptr) {
+            if ((e = dev_alloc((void**)&d_mask, (size_t)c->nf, c->device, s)) != cudaSuccess) { st = cuda_fail(c, e, "cudaMalloc mask"); break; }
+            if ((e = cudaMemcpyAsync(d_mask, mask, (size_t)c->nf, cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(c, e, "copy mask"); break; }
+            if (c->d_mask_bits == nullptr &&
+                (e = dev_alloc((void**)&c->d_mask_bits, (size_t)((c->nf + 31) / 32) * sizeof(uint32_t), c->device, s)) != cudaSuccess) { st = cuda_fail(c, e, "cudaMalloc mask bits"); break; }
+            if ((e = mi::launch_mask_bits(d_mask, c->nf, c->d_mask_bits, s)) != cudaSuccess) { st = cuda_fail(c, e, "mask bits"); break; }
+        } else if (c->d_mask_bits != nullptr) {
+            dev_free(c->d_mask_bits, s);
+            c->d_mask_bits = nullptr;
+        }
+        if (!c->wide) {
+            // the separable path reads the mask through its pitched fixed bins: rebuild them (and the rare list)
+            unsigned h_count = 0;
+            if ((e = dev_alloc((void**)&d_count, sizeof(unsigned), c->device, s)) != cudaSuccess) { st = cuda_fail(c, e, "cudaMalloc counter"); break; }
+            if ((e = cudaMemsetAsync(d_count, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(c, e, "memset"); break; }
+            if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, d_mask, c->fd[0] * c->fd[1], c->colpitch, c->fd[2], c->zrows_real,
+                                           c->d_fb_pitched, c->d_rare, d_count, c->rare_cap, s)) != cudaSuccess) { st = cuda_fail(c, e, "pitch fixed bins"); break; }
+            if ((e = cudaMemcpyAsync(&h_count, d_count, sizeof(unsigned), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(c, e, "copy counter"); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(c, e, "sync"); break; }
+            c->n_rare = h_count < c->rare_cap ? h_count : c->rare_cap;
+        } else if ((e = cudaStreamSynchronize(s)) != cudaSuccess) {
+            st = cuda_fail(c, e, "sync");
+        }
+    } while (false);
+    dev_free(d_mask, s);
+    dev_free(d_count, s);
+    return st;
 }
 
 mi_status mi_set_tsallis_form(mi_ctx* c, mi_tsallis_form form) {

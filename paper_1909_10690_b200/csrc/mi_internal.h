@@ -37,6 +37,7 @@ struct VolumeDesc {
 struct ResampleArgs {
     const uint8_t* fbins_ranked;  // fixed bins replaced by their population rank, [fz][fy][fx]
     const int* rank_inv;          // rank -> fixed bin
+    const uint32_t* mask_bits;    // NULL, or one bit per fixed voxel (flat index): 0 = the voxel takes no part
     const float* moving_pad;      // replicate-padded moving float32, dims (mx+2, my+2, mz+2)
     const uint8_t* mbins;         // moving bin indices (nearest neighbour), unpadded
     const float* M;               // n_transforms x 12 index-space affines (device)
@@ -63,6 +64,7 @@ int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes);
 struct WideArgs {
     const uint16_t* fbins;        // fixed bins [fz][fy][fx]
     const uint16_t* mbins;        // moving bins (nearest neighbour)
+    const uint32_t* mask_bits;    // NULL, or one bit per fixed voxel
     const float* moving_pad;      // replicate-padded moving float32
     const float* M;               // n_transforms x 12 (device)
     uint32_t* hist;               // n_transforms x nb x nb, zero on entry
@@ -71,6 +73,7 @@ struct WideArgs {
     float mlo, mscale;
     int n_transforms, nslabs;
 };
+cudaError_t launch_mask_bits(const uint8_t* mask, int64_t n, uint32_t* bits, cudaStream_t s);
 cudaError_t launch_prebin16(const float* vol, uint16_t* bins, int64_t n, float lo, float scale, int nb, cudaStream_t s);
 cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s);
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s);
@@ -122,7 +125,7 @@ struct ZHistArgs {
 enum { kBinGeneral = 0, kBinFast = 1, kBinFastPrescaled = 2 };
 constexpr int kZCols = 8;            // columns per thread of the z kernel: 2 groups of 4
 constexpr int kZColAlign = 32 * kZCols;  // colpitch is a multiple of this (one warp's columns)
-cudaError_t launch_pitch_bins(const uint8_t* in, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
+cudaError_t launch_pitch_bins(const uint8_t* in, const uint8_t* mask, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
                               uint2* rare, unsigned* rare_count, unsigned rare_cap, cudaStream_t s);
 cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, const float2* ax, int a0,
                          int na, int fnx, void* X, cudaStream_t s);

@@ -110,6 +110,27 @@ cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, i
     return cudaGetLastError();
 }
 
+// One bit per voxel from a byte mask (bit i of word i/32 = mask[i] != 0).
+__global__ void __launch_bounds__(256) mask_bits_kernel(const uint8_t* __restrict__ mask, int64_t n,
+                                                        uint32_t* __restrict__ bits) {
+    const int64_t nwords = (n + 31) >> 5;
+    const int lane = threadIdx.x & 31;
+    for (int64_t w = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5; w < nwords;
+         w += ((int64_t)gridDim.x * blockDim.x) >> 5) {
+        const int64_t i = (w << 5) + lane;
+        const unsigned word = __ballot_sync(0xffffffffu, i < n && mask[i] != 0);
+        if (lane == 0) bits[w] = word;
+    }
+}
+
+cudaError_t launch_mask_bits(const uint8_t* mask, int64_t n, uint32_t* bits, cudaStream_t s) {
+    int64_t blocks = (n + 255) / 256;
+    if (blocks < 1) blocks = 1;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    mask_bits_kernel<<<(unsigned)blocks, 256, 0, s>>>(mask, n, bits);
+    return cudaGetLastError();
+}
+
 // 256-bin population count of a uint8 volume (CTA-private shared histogram, merged with atomics).
 __global__ void __launch_bounds__(256) bin_count_kernel(const uint8_t* __restrict__ bins, int64_t n,
                                                         unsigned long long* __restrict__ counts) {
@@ -331,6 +352,10 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
                     const float cz = __fmaf_rn(m[8], fx, rz);
                     smp[u] = sample_bin<INTERP>(mv, cx, cy, cz);
                     smp[u].ok = smp[u].ok && (ix0 + 32 * u < fnx);
+                    if (a.mask_bits != nullptr) {
+                        const unsigned vi = (unsigned)row * (unsigned)fnx + (unsigned)ix;
+                        smp[u].ok = smp[u].ok && ((__ldg(a.mask_bits + (vi >> 5)) >> (vi & 31u)) & 1u);
+                    }
                     fa[u] = __ldg(frow + ix);
                 }
 #pragma unroll
@@ -900,6 +925,10 @@ __global__ void __launch_bounds__(512) resample_hist_wide_kernel(const __grid_co
                             const float tt = __fmul_rn(__fsub_rn(v, a.mlo), a.mscale);
                             b = min(max(__float2int_rd(tt), 0), nb - 1);
                         }
+                    }
+                    if (ok && a.mask_bits != nullptr) {
+                        const unsigned vi = (unsigned)row * (unsigned)fnx + (unsigned)ix;
+                        ok = (__ldg(a.mask_bits + (vi >> 5)) >> (vi & 31u)) & 1u;
                     }
                     if (ok) key = (unsigned)__ldg(frow + ix) * (unsigned)nb + (unsigned)b;
                 }

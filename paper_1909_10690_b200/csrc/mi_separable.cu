@@ -554,8 +554,11 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
 
 // fixed ranked bins -> [fnz][colpitch] (plane pitch padded to a multiple of 4 so that four adjacent
 // columns are one aligned 32-bit load); pad columns are 0.  Ranks >= rows_real are clamped to the
-// dump row `rows_real` and the voxel is appended to the rare list as (col, iz | rank << 16).
-__global__ void __launch_bounds__(256) pitch_bins_kernel(const uint8_t* __restrict__ in, int cols,
+// dump row `rows_real` and the voxel is appended to the rare list as (col, iz | rank << 16).  Voxels
+// outside the optional fixed-voxel mask (mi_set_fixed_mask) become the dump row as well: the z kernel
+// then counts them where the entropy epilogue and the histogram write-out never look.
+__global__ void __launch_bounds__(256) pitch_bins_kernel(const uint8_t* __restrict__ in,
+                                                         const uint8_t* __restrict__ mask, int cols,
                                                          int colpitch, int rows_real,
                                                          uint8_t* __restrict__ out, uint2* __restrict__ rare,
                                                          unsigned* __restrict__ rare_count, unsigned rare_cap) {
@@ -563,6 +566,10 @@ __global__ void __launch_bounds__(256) pitch_bins_kernel(const uint8_t* __restri
     if (col >= colpitch) return;
     const int iz = blockIdx.y;
     int r = col < cols ? in[(size_t)iz * cols + col] : 0;
+    if (mask != nullptr && col < cols && mask[(size_t)iz * cols + col] == 0) {
+        out[(size_t)iz * colpitch + col] = (uint8_t)rows_real;   // masked-out voxel: counts into the dump row
+        return;
+    }
     if (r >= rows_real) {
         const unsigned slot = atomicAdd(rare_count, 1u);
         if (slot < rare_cap) rare[slot] = make_uint2((unsigned)col, (unsigned)iz | ((unsigned)r << 16));
@@ -612,10 +619,10 @@ __global__ void __launch_bounds__(256) zrare_kernel(const __grid_constant__ ZHis
 
 }  // namespace
 
-cudaError_t launch_pitch_bins(const uint8_t* in, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
+cudaError_t launch_pitch_bins(const uint8_t* in, const uint8_t* mask, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
                               uint2* rare, unsigned* rare_count, unsigned rare_cap, cudaStream_t s) {
     dim3 grid((colpitch + 255) / 256, fnz);
-    pitch_bins_kernel<<<grid, 256, 0, s>>>(in, cols, colpitch, rows_real, out, rare, rare_count, rare_cap);
+    pitch_bins_kernel<<<grid, 256, 0, s>>>(in, mask, cols, colpitch, rows_real, out, rare, rare_count, rare_cap);
     return cudaGetLastError();
 }
 

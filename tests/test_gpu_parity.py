@@ -352,6 +352,47 @@ def test_affine12_composite_grid_full_3_to_the_12(mi):
     assert digits[0] == 1 and digits[1] == -1
 
 
+def test_fixed_voxel_mask_all_paths(mi):
+    """mi_set_fixed_mask (a seeded 30 % subset of the fixed voxels, drawn by the harness) against the oracle
+    with the same mask: generic kernel (histograms, both interpolators), separable maps (fused epilogue,
+    rare rows), wide histograms; clearing the mask restores the full-volume results."""
+    import torch
+    cfg = ph.get_config("C5", res=0.25, grid_n=3)
+    mask = ph.keyed_uniform(91, np.arange(cfg.fixed.size, dtype=np.uint64)).reshape(cfg.fixed.shape) < 0.3
+    rng = np.random.default_rng(5)
+    T = rand_physical(rng, 4)
+    fd, md = cfg.fixed.shape[::-1], cfg.moving.shape[::-1]
+    M = orc.physical_to_index(T, fd, cfg.fixed_spacing, md, cfg.moving_spacing)
+    for nb in (256, 1000):
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, nb) as ctx:
+            full = mi.mi_eval_batch(ctx, T, (0.5,), 1)[0]
+            mi.mi_set_fixed_mask(ctx, mask if nb == 256 else torch.from_numpy(mask).cuda())
+            for interp in (0, 1):
+                ref = orc.eval_batch(cfg.fixed, cfg.moving, M, nb, 0, 1, 0, 1, interp, q=(0.5,), want_hist=True, mask=mask)
+                vals, hist, nvalid = mi.mi_eval_batch(ctx, T, (0.5,), interp, hist_out=True, nvalid_out=True)
+                if interp == 0:
+                    assert np.array_equal(hist, ref["hist"]) and np.array_equal(nvalid, ref["nvalid"])
+                else:
+                    moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
+                    assert np.all(moved <= FLIP_FRAC * cfg.fixed.size)
+                assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
+                # maps: separable kernels at 256 bins, the generic one above
+                rm = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, nb, 0, 1, 0, 1, cfg.family,
+                                cfg.lo, cfg.hi, cfg.n, q=(0.5,), interp=interp, mask=mask)
+                m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, (0.5,), interp)
+                assert np.max(np.abs(m - rm["map"])) <= MI_TOL and np.array_equal(am, rm["argmax"])
+            mi.mi_set_fixed_mask(ctx, None)
+            assert np.array_equal(mi.mi_eval_batch(ctx, T, (0.5,), 1)[0], full)
+    # few shared rows: masked voxels and rare-row voxels together
+    with env(MI_B200_ZROWS=40):
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
+            mi.mi_set_fixed_mask(ctx, mask)
+            rm = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, 256, 0, 1, 0, 1, cfg.family,
+                            cfg.lo, cfg.hi, cfg.n, q=(), interp=1, mask=mask)
+            m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, (), 1)
+            assert np.max(np.abs(m - rm["map"])) <= MI_TOL and np.array_equal(am, rm["argmax"])
+
+
 def test_context_cycles_reuse_the_pool_and_release(mi):
     """Destroyed contexts hand their memory to the library's pool; results do not depend on what
     an earlier context left in it, and mi_release_cached_memory gives it back."""
