@@ -193,13 +193,13 @@ __device__ __forceinline__ double warp_sum_d(double v) {
 }
 
 // Shared-memory layout of the z kernel, in 32-bit words:
-//   ws[fnz] z-weights | run_hi[planes] | (pad to 4) | pb[kEntropyPb] | red[kEntropyRed] | histogram rows
+//   run_hi[planes] | (pad to 4) | pb[kEntropyPb] | red[kEntropyRed] | histogram rows
 // pb / red are the fused entropy epilogue's scratch (moving marginal counts; per-warp partial sums).
 constexpr int kEntropyAcc = 1 + kMaxQPerPass;                     // sum c ln c, sum c^q_k
 constexpr int kEntropyPb = 272;                                   // 256 moving bins + 8 partial totals, multiple of 4
 constexpr int kEntropyRed = 2 * kEntropyAcc * (kHistThreads / 32 + 16);  // doubles as word pairs
-__host__ __device__ __forceinline__ int zhist_table_words(int fnz, int planes) {
-    return ((fnz + planes + 3) & ~3) + kEntropyPb + kEntropyRed;
+__host__ __device__ __forceinline__ int zhist_table_words(int planes) {
+    return ((planes + 3) & ~3) + kEntropyPb + kEntropyRed;
 }
 
 struct Cols {                        // this thread's kZCols columns of one plane: 2 groups of 4
@@ -374,11 +374,10 @@ __device__ __forceinline__ void zhist_entropy_epilogue(const ZHistArgs& a, long 
 template <bool NN, int MODE>
 __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_constant__ ZHistArgs a) {
     extern __shared__ __align__(16) uint32_t sh_raw[];
-    float* ws = reinterpret_cast<float*>(sh_raw);
-    int* run_hi = reinterpret_cast<int*>(sh_raw) + a.fnz;
-    uint32_t* sh_pb = sh_raw + ((a.fnz + a.planes + 3) & ~3);
+    int* run_hi = reinterpret_cast<int*>(sh_raw);
+    uint32_t* sh_pb = sh_raw + ((a.planes + 3) & ~3);
     double* sh_red = reinterpret_cast<double*>(sh_pb + kEntropyPb);
-    uint32_t* sh_hist = sh_raw + zhist_table_words(a.fnz, a.planes);
+    uint32_t* sh_hist = sh_raw + zhist_table_words(a.planes);
     __shared__ int s_lo, s_hi;
     const unsigned nb = (unsigned)a.nb;
     const unsigned pitch = (unsigned)a.pitch;
@@ -406,7 +405,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
         __syncthreads();
         for (int iz = threadIdx.x; iz < a.fnz; iz += blockDim.x) {
             const AxisSample sz = axis_sample<NN>(__fmaf_rn(mo.x, (float)iz, mo.y), a.mnz);
-            ws[iz] = sz.w;
             if (sz.ok) {
                 atomicMin(&s_lo, iz);
                 atomicMax(&s_hi, iz);
@@ -478,7 +476,12 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                         pp += colpitch;
                         const int end = run_hi[p];
                         for (; iz < end; ++iz) {
-                            const float w = ws[iz];
+                            // z weight c_z - floor(c_z) (CANON-4) recomputed per slice, 4 ALU instructions, rather
+                            // than read from a shared table: the LSU data pipe is this kernel's bottleneck, the
+                            // issue slots are not (658 -> 637 ms at C5; deriving the run ends the same way instead
+                            // of reading run_hi measured no further gain)
+                            const float czf = __fmaf_rn(mo.x, (float)iz, mo.y);
+                            const float w = __fsub_rn(czf, __fsub_rn(__fadd_rd(czf, kMagic), kMagic));
                             Bins fa;
 #pragma unroll
                             for (int j = 0; j < kZCols / 4; ++j) fa.w[j] = (fa_next.w[j] & keep.w[j]) | dump.w[j];
@@ -656,7 +659,8 @@ cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx,
 // Histogram rows (of `pitch` words) of the z kernel that fit in shared memory beside its tables,
 // the dump row included (at most nb + 1).
 int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin) {
-    const size_t reserve = 1024 + 4 * (size_t)zhist_table_words(fnz, planes);
+    (void)fnz;
+    const size_t reserve = 1024 + 4 * (size_t)zhist_table_words(planes);
     size_t rows = (smem_optin > reserve ? smem_optin - reserve : 0) / ((size_t)pitch * sizeof(uint32_t));
     if (rows > (size_t)nb + 1) rows = (size_t)nb + 1;
     return (int)rows;
@@ -675,7 +679,7 @@ cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t 
     if (a.rows_smem < 1 || a.pitch < a.nb + 1 || (a.colpitch % kZColAlign) != 0 || a.nb > 256)
         return cudaErrorInvalidConfiguration;
     if (a.fused && (a.n_rare > 0 || a.nq > kMaxQPerPass || a.mi_out == nullptr)) return cudaErrorInvalidConfiguration;
-    const size_t smem = 4 * (size_t)zhist_table_words(a.fnz, a.planes) + (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
+    const size_t smem = 4 * (size_t)zhist_table_words(a.planes) + (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
     const long long nitems = (long long)a.n_pairs * a.n2;
     long long grid = nitems < num_sms ? nitems : num_sms;
     if (grid < 1) return cudaSuccess;
