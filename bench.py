@@ -32,8 +32,8 @@ if ROOT not in sys.path:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (4 of the 41 p0
 # slabs = 6724 transforms = 1.414e11 evaluations), from the committed ncu --set full capture of the
-# default command (profiles/r1e_ncu_zhist_resample.md); keyed by (config, grid, interpolation)
-NCU_DRAM_BYTES_PER_LAUNCH = {("C5", (41, 41, 41), 1): 16265455000 + 552631552}
+# default command (profiles/r1k_ncu_zhist_final.md); keyed by (config, grid, interpolation)
+NCU_DRAM_BYTES_PER_LAUNCH = {("C5", (41, 41, 41), 1): 16264608000 + 553361408}
 
 METRIC = "voxel-transform evaluations per second (MI map, 260x311x260 fixed, 256 bins)"
 UNIT = "evals/s"
