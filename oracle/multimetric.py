@@ -62,3 +62,55 @@ def multimetric_gradient(fixed, fixed_spacing, moving, moving_spacing, nbins, ra
         ch = 1 if k in TRANSLATION_PARAMS else 0
         grad[k] = (vals[1 + 2 * k, ch] - vals[2 + 2 * k, ch]) / (2.0 * delta[k])
     return grad, vals[0].copy()
+
+
+GROUPS = ((0, 1, 2), (3, 4, 5), (6, 7, 8))      # translation [mm], rotation [deg], scale [factor]
+
+
+def register(fixed, fixed_spacing, moving, moving_spacing, nbins, ranges, p0, delta, step0, step_min, max_iter, q,
+             interp=_orc.INTERP_TRILINEAR, form=_orc.TSALLIS_ADDITIVE):
+    """The loop of the paper's Fig. 1 (Transform -> Metric -> Optimizer) driven by the
+    multi-metric gradient of section 4.  The paper names "gradient descent" and the multi-metric strategy
+    but prints no step rule; the rule taken (A20) is regular-step gradient ASCENT (+MI is
+    maximised, reading A2) applied to each parameter group with its own step length:
+
+        g = multimetric_gradient(p)                      (Tsallis for translations, Shannon otherwise)
+        for each group G with step L_G >= step_min[G]:
+            d = g_G / |g_G|                              (skipped when |g_G| == 0)
+            if d . d_prev_G < 0:  L_G = L_G / 2          (the direction turned back: halve the step)
+            if L_G >= step_min[G]:  p_G = p_G + L_G * d
+        stop when no group moved, or after max_iter iterations.
+
+    Returns dict(p (9,), iterations, trace (iterations + 1, 9) of the visited p, steps (3,) final step lengths,
+    values (2,) = (Shannon, Tsallis) at the last gradient evaluation)."""
+    p = np.asarray(p0, dtype=np.float64).reshape(N_PARAMS).copy()
+    delta = np.asarray(delta, dtype=np.float64).reshape(N_PARAMS)
+    L = np.asarray(step0, dtype=np.float64).reshape(3).copy()
+    Lmin = np.asarray(step_min, dtype=np.float64).reshape(3)
+    prev = [None, None, None]
+    trace = [p.copy()]
+    vals = np.zeros(2)
+    it = 0
+    while it < int(max_iter):
+        g, vals = multimetric_gradient(fixed, fixed_spacing, moving, moving_spacing, nbins, ranges, p, delta, q,
+                                       interp=interp, form=form)
+        moved = False
+        for gi, idx in enumerate(GROUPS):
+            if not (L[gi] >= Lmin[gi] and L[gi] > 0):
+                continue
+            gg = g[list(idx)]
+            norm = float(np.sqrt(gg[0] * gg[0] + gg[1] * gg[1] + gg[2] * gg[2]))
+            if norm == 0.0:
+                continue
+            d = gg / norm
+            if prev[gi] is not None and (d[0] * prev[gi][0] + d[1] * prev[gi][1] + d[2] * prev[gi][2]) < 0.0:
+                L[gi] = L[gi] / 2.0
+            prev[gi] = d
+            if L[gi] >= Lmin[gi]:
+                p[list(idx)] = p[list(idx)] + L[gi] * d
+                moved = True
+        it += 1
+        trace.append(p.copy())
+        if not moved:
+            break
+    return {"p": p, "iterations": it, "trace": np.stack(trace), "steps": L, "values": vals}

@@ -64,3 +64,39 @@ def test_skipped_components_and_pseudo_additive_form():
     g1, v1 = mm.multimetric_gradient(*args, p, delta, 2.0, interp=0, form=1)
     assert v1[0] == v0[0] and v1[1] != v0[1]          # Shannon unchanged, Tsallis form changes
     assert g1[6] == g0[6] and g1[0] != g0[0]
+
+
+def test_register_follows_its_rule_and_reaches_the_map_maximum():
+    """The driver on the C1 pair, translations only: every move has the current step length, a halving
+    happens exactly when the direction turns back, and the end point sits next to the maximum of the
+    Tsallis q = 0.5 translation map (the metric its translation group ascends), which the exhaustive
+    oracle map locates independently."""
+    cfg = ph.get_config("C1")
+    args = (cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, cfg.ranges)
+    p0 = np.array([0, 0, 0, 0, 0, 0, 1, 1, 1.0])
+    delta = np.array([0.5, 0.5, 0.5, 0, 0, 0, 0, 0, 0.0])
+    r = mm.register(*args, p0, delta, (1.0, 0, 0), (0.1, 1, 1), 40, 0.5, interp=1)
+    tr = r["trace"]
+    assert r["iterations"] == len(tr) - 1 and np.array_equal(tr[0], p0)
+    assert np.all(tr[:, 3:] == p0[3:])                       # rotation and scale never move (step 0)
+    moves = np.linalg.norm(np.diff(tr[:, :3], axis=0), axis=1)
+    L = 1.0
+    for k in range(len(moves)):
+        if moves[k] == 0:
+            assert k == len(moves) - 1                       # the last iteration may not move
+            continue
+        assert np.isclose(moves[k], L) or np.isclose(moves[k], L / 2)
+        if np.isclose(moves[k], L / 2) and not np.isclose(moves[k], L):
+            d0, d1 = np.diff(tr[:, :3], axis=0)[k - 1], np.diff(tr[:, :3], axis=0)[k]
+            assert np.dot(d0, d1) < 0                        # halved exactly where the direction turned back
+            L = L / 2
+    assert r["steps"][0] < 0.1 * 2 and r["iterations"] < 40  # stopped on the step length, not the cap
+    # independent check of where it ends: the exhaustive Tsallis map at 0.5-voxel resolution
+    m = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges, 0, (-1, -4, -2), (4, 1, 3),
+                   (11, 11, 11), q=(0.5,), interp=1)
+    k2, k1, k0 = np.unravel_index(int(m["argmax"][1]), (11, 11, 11))
+    peak = np.array([-1 + 0.5 * k0, -4 + 0.5 * k1, -2 + 0.5 * k2])
+    assert np.max(np.abs(r["p"][:3] - peak)) <= 0.75, (r["p"][:3], peak)
+    # and it climbed: the Tsallis value at the end exceeds the one at the start
+    _, v0 = mm.multimetric_gradient(*args, p0, delta, 0.5, interp=1)
+    assert r["values"][1] > v0[1]
