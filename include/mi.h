@@ -157,6 +157,24 @@ mi_status mi_compose_matrix(const double p[9], double T_out[12]);
 mi_status mi_multimetric_gradient(mi_ctx *ctx, const double p[9], const double delta[9], double q,
                                   mi_interp interp, double grad_out[9], double value_out[2]);
 
+/* The loop of the paper's Fig. 1 (Transform -> Metric -> Optimizer) around the
+ * multi-metric gradient.  The paper names "gradient descent" and the strategy but prints no step rule;
+ * the rule taken (A20) is regular-step gradient ascent per parameter group G (translation,
+ * rotation, scale) with its own step length L_G (mm, degrees, factor):
+ *     g = mi_multimetric_gradient(p);  d = g_G / |g_G|  (skipped when |g_G| == 0)
+ *     if d . d_prev_G < 0: L_G = L_G / 2;   if L_G >= step_min[G]: p_G = p_G + L_G d
+ * A group with step0[G] < step_min[G] (e.g. 0) never moves.  Stops when no group moved or after
+ * max_iter iterations.  p_out: 9 doubles; trace_out: NULL or (max_iter + 1) x 9 doubles (the visited
+ * p, row 0 = p0; rows beyond info.iterations are not written); info_out may be NULL.  Host pointers. */
+typedef struct {
+    int32_t iterations;       /* gradient evaluations made                                          */
+    double steps[3];          /* final step lengths                                                 */
+    double values[2];         /* (Shannon, Tsallis_q) at the last gradient evaluation               */
+} mi_register_info;
+mi_status mi_register(mi_ctx *ctx, const double p0[9], const double delta[9], const double step0[3],
+                      const double step_min[3], int32_t max_iter, double q, mi_interp interp,
+                      double p_out[9], double *trace_out, mi_register_info *info_out);
+
 /* ---- capture-range analysis of a map ---------------------------------------
  * The paper reads its maps through "the paths the gradient descent algorithm will take" and the
  * regions "converging to the central point" or "to other points not related to our goal"

@@ -16,6 +16,10 @@ and no difference rule; the readings taken (A18):
   histogram each, which yields both metrics (the "same histogram" of PAPER.md:199);
 * d_k <= 0 skips component k (gradient 0).
 
+`register` (reading A20) is the loop of Fig. 1 around that gradient; its step rule is this build's --
+the paper prints none -- so against the paper it is "parity unpinned"; it is pinned on its own rule and
+against the exhaustive map's maximum.
+
 Pins (tests/test_oracle_multimetric_pins.py): the composition against scipy's rotations and the map
 families; every gradient component against the central difference of an exhaustive map of the same
 family computed by oracle.mi_map + map_analysis.map_gradient (channel, sign, step and parameter

@@ -27,7 +27,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
-           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient",
+           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient", "mi_register",
            "mi_probe_shared_atomic_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
@@ -63,6 +63,8 @@ _lib.mi_compose_matrix.argtypes = [_vp, _vp]
 _lib.mi_compose_matrix.restype = C.c_int
 _lib.mi_multimetric_gradient.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp]
 _lib.mi_multimetric_gradient.restype = C.c_int
+_lib.mi_register.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_double, C.c_int, _vp, _vp, _vp]
+_lib.mi_register.restype = C.c_int
 _lib.mi_map_gradient.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, _vp]
 _lib.mi_map_gradient.restype = C.c_int
 _lib.mi_map_basins.argtypes = [_vp, _vp, C.c_int32, C.c_int32, C.c_int64, _vp, _vp, _vp, C.c_int32, _vp]
@@ -340,6 +342,22 @@ def mi_multimetric_gradient(ctx, p, delta, q, interp=MI_INTERP_TRILINEAR):
     _check(ctx, _lib.mi_multimetric_gradient(ctx.handle, _ptr(p), _ptr(delta), float(q), int(interp), _ptr(grad),
                                              _ptr(vals)))
     return grad, vals
+
+
+class _RegisterInfo(C.Structure):
+    _fields_ = [("iterations", C.c_int32), ("steps", C.c_double * 3), ("values", C.c_double * 2)]
+
+
+def mi_register(ctx, p0, delta, step0, step_min, max_iter, q, interp=MI_INTERP_TRILINEAR):
+    """Regular-step multi-metric ascent: dict(p, iterations, trace (iterations + 1, 9), steps, values)."""
+    p0, delta, step0, step_min = _f64(p0, 9), _f64(delta, 9), _f64(step0, 3), _f64(step_min, 3)
+    p = np.empty(9, dtype=np.float64)
+    trace = np.zeros((int(max_iter) + 1, 9), dtype=np.float64)
+    info = _RegisterInfo()
+    _check(ctx, _lib.mi_register(ctx.handle, _ptr(p0), _ptr(delta), _ptr(step0), _ptr(step_min), int(max_iter), float(q),
+                                 int(interp), _ptr(p), _ptr(trace), C.addressof(info)))
+    return {"p": p, "iterations": int(info.iterations), "trace": trace[: info.iterations + 1].copy(),
+            "steps": np.array(list(info.steps)), "values": np.array(list(info.values))}
 
 
 def mi_release_cached_memory(device=0) -> None:

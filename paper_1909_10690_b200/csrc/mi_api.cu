@@ -821,16 +821,14 @@ mi_status mi_compose_matrix(const double p[9], double T_out[12]) {
     return MI_OK;
 }
 
-mi_status mi_multimetric_gradient(mi_ctx* c, const double p[9], const double delta[9], double q, mi_interp interp,
-                                  double grad_out[9], double value_out[2]) {
-    if (!c) return MI_ERR_INVALID_ARG;
-    if (!p || !delta || !grad_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
-    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
-        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
-    mi_status st = validate_q(c, &q, 1);
-    if (st != MI_OK) return st;
-    for (int i = 0; i < 9; ++i)
-        if (!std::isfinite(p[i]) || !std::isfinite(delta[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite parameter");
+}  // extern "C"
+
+namespace {
+
+// One multi-metric gradient (arguments already validated; the device is current).
+mi_status gradient_core(mi_ctx* c, const double p[9], const double delta[9], double q, int interp,
+                        double grad_out[9], double value_out[2]) {
+    mi_status st;
     // transform 0 = p; then p + d_k e_k, p - d_k e_k for every parameter with d_k > 0
     int slot[9];
     int64_t N = 1;
@@ -854,10 +852,8 @@ mi_status mi_multimetric_gradient(mi_ctx* c, const double p[9], const double del
         pk[k] = p[k] - delta[k];
         put(slot[k] + 1, pk);
     }
-    DeviceGuard guard(c->device);
-    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
     std::vector<double> vals((size_t)N * 2);
-    st = eval_core(c, hM, N, &q, 1, (int)interp, vals.data(), nullptr, nullptr, nullptr, nullptr);
+    st = eval_core(c, hM, N, &q, 1, interp, vals.data(), nullptr, nullptr, nullptr, nullptr);
     if (st != MI_OK) return st;
     for (int k = 0; k < 9; ++k) {
         grad_out[k] = 0.0;
@@ -866,6 +862,83 @@ mi_status mi_multimetric_gradient(mi_ctx* c, const double p[9], const double del
         grad_out[k] = (vals[(size_t)slot[k] * 2 + ch] - vals[(size_t)(slot[k] + 1) * 2 + ch]) / (2.0 * delta[k]);
     }
     if (value_out) { value_out[0] = vals[0]; value_out[1] = vals[1]; }
+    return MI_OK;
+}
+
+mi_status validate_gradient_args(mi_ctx* c, const double* p, const double* delta, double q, int interp) {
+    if (!p || !delta) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
+    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
+        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
+    mi_status st = validate_q(c, &q, 1);
+    if (st != MI_OK) return st;
+    for (int i = 0; i < 9; ++i)
+        if (!std::isfinite(p[i]) || !std::isfinite(delta[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite parameter");
+    return MI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+mi_status mi_multimetric_gradient(mi_ctx* c, const double p[9], const double delta[9], double q, mi_interp interp,
+                                  double grad_out[9], double value_out[2]) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (!grad_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
+    mi_status st = validate_gradient_args(c, p, delta, q, (int)interp);
+    if (st != MI_OK) return st;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    return gradient_core(c, p, delta, q, (int)interp, grad_out, value_out);
+}
+
+mi_status mi_register(mi_ctx* c, const double p0[9], const double delta[9], const double step0[3],
+                      const double step_min[3], int32_t max_iter, double q, mi_interp interp, double p_out[9],
+                      double* trace_out, mi_register_info* info_out) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (!step0 || !step_min || !p_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
+    mi_status st = validate_gradient_args(c, p0, delta, q, (int)interp);
+    if (st != MI_OK) return st;
+    if (max_iter < 0) return fail(c, MI_ERR_INVALID_ARG, "max_iter < 0");
+    for (int g = 0; g < 3; ++g)
+        if (!std::isfinite(step0[g]) || !std::isfinite(step_min[g])) return fail(c, MI_ERR_INVALID_ARG, "non-finite step");
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    double p[9], L[3], prev[3][3], vals[2] = {0.0, 0.0};
+    bool have_prev[3] = {false, false, false};
+    for (int i = 0; i < 9; ++i) p[i] = p0[i];
+    for (int g = 0; g < 3; ++g) L[g] = step0[g];
+    if (trace_out) for (int i = 0; i < 9; ++i) trace_out[i] = p[i];
+    int it = 0;
+    while (it < max_iter) {
+        double grad[9];
+        st = gradient_core(c, p, delta, q, (int)interp, grad, vals);
+        if (st != MI_OK) return st;
+        bool moved = false;
+        for (int g = 0; g < 3; ++g) {
+            if (!(L[g] >= step_min[g] && L[g] > 0.0)) continue;
+            const double* gg = grad + 3 * g;
+            const double norm = std::sqrt(gg[0] * gg[0] + gg[1] * gg[1] + gg[2] * gg[2]);
+            if (norm == 0.0) continue;
+            const double d[3] = {gg[0] / norm, gg[1] / norm, gg[2] / norm};
+            if (have_prev[g] && d[0] * prev[g][0] + d[1] * prev[g][1] + d[2] * prev[g][2] < 0.0) L[g] = L[g] / 2.0;
+            for (int i = 0; i < 3; ++i) prev[g][i] = d[i];
+            have_prev[g] = true;
+            if (L[g] >= step_min[g]) {
+                for (int i = 0; i < 3; ++i) p[3 * g + i] = p[3 * g + i] + L[g] * d[i];
+                moved = true;
+            }
+        }
+        ++it;
+        if (trace_out) for (int i = 0; i < 9; ++i) trace_out[(size_t)it * 9 + i] = p[i];
+        if (!moved) break;
+    }
+    for (int i = 0; i < 9; ++i) p_out[i] = p[i];
+    if (info_out) {
+        info_out->iterations = it;
+        for (int g = 0; g < 3; ++g) info_out->steps[g] = L[g];
+        info_out->values[0] = vals[0];
+        info_out->values[1] = vals[1];
+    }
     return MI_OK;
 }
 

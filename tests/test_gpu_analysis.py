@@ -149,3 +149,25 @@ def test_multimetric_gradient_equals_oracle(mi):
                 assert np.all(g[delta <= 0] == 0)
         with pytest.raises(mi.MIError):
             mi.mi_multimetric_gradient(ctx, cases[0][0], cases[0][1], -1.0, 1)
+
+
+def test_register_follows_the_oracle_trajectory(mi):
+    """mi_register against oracle/multimetric.register: same rule, gradients equal to ~1e-9, so the visited
+    points agree to 1e-6 and the step halvings fall on the same iterations."""
+    from oracle import multimetric as mm
+    cfg = ph.get_config("C1")
+    args = (cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, cfg.ranges)
+    p0 = np.array([0, 0, 0, 0, 0, 0, 1, 1, 1.0])
+    runs = [(np.array([0.5, 0.5, 0.5, 0, 0, 0, 0, 0, 0.0]), (1.0, 0, 0), (0.1, 1, 1), 40, 0.5),
+            (np.array([0.5, 0.5, 0.5, 1, 1, 1, 0.02, 0.02, 0.02]), (0.5, 0.5, 0.01), (0.1, 0.1, 0.002), 12, 0.5)]
+    with mi.mi_create(cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        for delta, step0, step_min, iters, q in runs:
+            ref = mm.register(*args, p0, delta, step0, step_min, iters, q, interp=1)
+            got = mi.mi_register(ctx, p0, delta, step0, step_min, iters, q, 1)
+            assert got["iterations"] == ref["iterations"]
+            assert np.max(np.abs(got["trace"] - ref["trace"])) <= 1e-6
+            assert np.allclose(got["steps"], ref["steps"], rtol=0, atol=0)
+            assert np.max(np.abs(got["values"] - ref["values"])) <= 1e-4
+            assert np.array_equal(got["p"], got["trace"][-1])
+        r0 = mi.mi_register(ctx, p0, runs[0][0], (0, 0, 0), (1, 1, 1), 5, 0.5, 1)     # nothing may move
+        assert r0["iterations"] == 1 and np.array_equal(r0["p"], p0)
