@@ -21,9 +21,14 @@
  *   samples   falling outside the moving volume (continuous index outside [-0.5, n-0.5) on any
  *             axis) are skipped; probabilities are normalised by the number of valid samples.
  *   bins      uniform over [lo, hi]; b = clamp(floor((v - lo) * nbins/(hi-lo)), 0, nbins-1).
- *   pointers  every data pointer may be a HOST or a DEVICE pointer (resolved with
- *             cudaPointerGetAttributes).  Inputs are only read.  Outputs are caller-owned and are
- *             written only when the call returns MI_OK.
+ *   pointers  BULK data -- the volumes and the mask given to mi_create / mi_set_fixed_mask, a map given
+ *             to mi_map_gradient / mi_map_basins, and every OUTPUT array (mi_out, hist_out,
+ *             nvalid_out, map_out, argmax_out, grad_out, label_out, steps_out, mi_get_bins' out) --
+ *             may be HOST or DEVICE pointers (resolved with cudaPointerGetAttributes).  The small
+ *             PARAMETER arrays -- dims, spacings, T, q, lo, hi, n, begin, end, p, delta, step0,
+ *             step_min -- and the info/stats structs are read or written on the host and must be
+ *             HOST pointers.  Inputs are only read.  Outputs are caller-owned and are written only
+ *             when the call returns MI_OK.
  *   sync      a call returns after all HOST outputs are complete; DEVICE outputs are ordered on
  *             the context's stream (the cudaStream_t given to mi_create).
  *   threads   one context must not be used from two threads at once; distinct contexts are
@@ -45,7 +50,7 @@ typedef struct mi_ctx mi_ctx; /* opaque; owns all of its device memory until mi_
 typedef enum {
     MI_OK = 0,
     MI_ERR_INVALID_ARG = 1,   /* NULL pointer, dim < 1, grid n < 1, spacing <= 0 or non-finite, lo >= hi,
-                                 nbins < 2, N < 0, q <= 0 or non-finite, non-finite matrix entry */
+                                 nbins < 2, N < 0, q <= 0, q > 32 or non-finite, non-finite matrix entry */
     MI_ERR_UNSUPPORTED = 2,   /* nbins > 4096; volume with more than 2^31-1 voxels */
     MI_ERR_OUT_OF_MEMORY = 3,
     MI_ERR_CUDA = 4,          /* any CUDA runtime failure, including "no device" */
@@ -76,7 +81,9 @@ typedef enum {
  *   out            receives the context; *out is NULL on failure.
  *   fixed, moving  float32 volumes (host or device), finite values; copied -- the caller may free
  *                  them on return.
- *   *_dims         (nx, ny, nz), each >= 1;  *_spacing  mm, each > 0 and finite.
+ *   *_dims         (nx, ny, nz), each >= 1;  *_spacing  mm, each > 0 and finite.  At most 2^31-1 voxels
+ *                  per volume.  A fixed volume with nz > 65535 is accepted but its maps take the generic
+ *                  kernel (the separable kernels index z slices with 16 bits).
  *   nbins          2..4096 bins per axis of the joint histogram.  Up to 256 the histograms are built in
  *                  shared memory (and translation / scale maps take the separable kernels); above, the
  *                  "full histogram" of PAPER.md:212 for 12-bit data, they live in global memory
@@ -96,14 +103,16 @@ mi_status mi_set_tsallis_form(mi_ctx *ctx, mi_tsallis_form form);
 /* mi_eval_batch -- F_m(u, v o T) for N transforms (eq. 3 without the arg max).
  *   T           N x 12 doubles, row-major [A|t] per transform (see "transform" above).  Singular
  *               matrices are legal; entries must be finite.
- *   q, nq       Tsallis orders, each > 0 and finite; q == 1 returns the Shannon value; nq may be 0
- *               (then q may be NULL).
+ *   q, nq       Tsallis orders, each in (0, 32]; q == 1 returns the Shannon value; nq may be 0
+ *               (then q may be NULL).  The upper bound keeps sum c^q over integer counts c < 2^31
+ *               inside the double range (32 ln 2^31 = 688 < 709); the paper uses q in [0.5, 2].
  *   mi_out      N x (1+nq) doubles: [Shannon I (nats), I_q0, I_q1, ...] per transform.  An empty
  *               overlap gives zeros.
  *   hist_out    NULL, or N x nbins x nbins uint32 joint histograms, row = fixed bin, column =
  *               moving bin.
  *   nvalid_out  NULL, or N int64: samples inside the moving volume per transform.
- * N == 0 is a no-op returning MI_OK. */
+ * N == 0 is a no-op returning MI_OK.  Every transform takes the generic resample+histogram kernel (only
+ * mi_map / mi_map_range recognise diagonal grids and take the separable kernels). */
 mi_status mi_eval_batch(mi_ctx *ctx, const double *T, int64_t N, const double *q, int32_t nq,
                         mi_interp interp, double *mi_out, uint32_t *hist_out, int64_t *nvalid_out);
 
@@ -117,6 +126,48 @@ mi_status mi_eval_batch(mi_ctx *ctx, const double *T, int64_t N, const double *q
 mi_status mi_map(mi_ctx *ctx, mi_family family, const double lo[3], const double hi[3],
                  const int32_t n[3], const double *q, int32_t nq, mi_interp interp,
                  double *map_out, int64_t *argmax_out);
+
+/* mi_map_range -- a sub-box of the same map: nodes begin[d] <= k_d < end[d] of the grid (lo, hi, n).
+ * Node parameters are those of the WHOLE grid (lo[d] + k*(hi[d]-lo[d])/(n[d]-1)), so a slab computed
+ * here equals the same nodes of mi_map bit for bit -- the unit of multi-GPU sharding (every map voxel
+ * is a separate MI evaluation) and of spot checks of a large map.
+ *   begin, end  NULL = the whole axis range (0 and n); else 0 <= begin[d] < end[d] <= n[d].
+ *   map_out     (1+nq) x m[2] x m[1] x m[0] doubles with m[d] = end[d] - begin[d], p0 fastest.
+ *   argmax_out  NULL, or (1+nq) linear indices into the SUB-BOX.
+ *   hist_out    NULL, or m[2]*m[1]*m[0] joint histograms of nbins x nbins uint32 in sub-box node order
+ *               (row = fixed bin).  Diagonal families then run the separable kernels with the
+ *               histogram written out instead of the fused entropy epilogue. */
+mi_status mi_map_range(mi_ctx *ctx, mi_family family, const double lo[3], const double hi[3],
+                       const int32_t n[3], const int32_t begin[3], const int32_t end[3],
+                       const double *q, int32_t nq, mi_interp interp,
+                       double *map_out, int64_t *argmax_out, uint32_t *hist_out);
+
+/* Tuning and test options of a context -- the only way to change kernel selection (no environment
+ * variable is read anywhere in the library).  Defaults are the measured optimum;
+ * no option changes a result bit: they select between kernels that compute the same CANON sequence.
+ * Values are validated (MI_ERR_INVALID_ARG).  MI_INFO_* keys are read-only (mi_get_option). */
+typedef enum {
+    MI_OPT_SEPARABLE = 0,          /* 1: translation / scale maps take the separable kernels; 0: generic kernel */
+    MI_OPT_FUSE_ENTROPY = 1,       /* 1: step a5 as the z kernel's epilogue when possible                       */
+    MI_OPT_BIN_MODE_MAX = 2,       /* cap on the z kernel's binning variant: 0 general, 1 clamp-free, 2 pre-scaled */
+    MI_OPT_ZHIST_ROWS_MAX = 3,     /* cap on the z kernel's shared histogram rows (0 = all that fit), >= 2      */
+    MI_OPT_ZHIST_PAD = 4,          /* pad words per shared row of the z kernel, 1..64 (default 9)               */
+    MI_OPT_XY_BUDGET_MB = 5,       /* xy-plane scratch per separable batch (default 12288)                      */
+    MI_OPT_SEP_HIST_BUDGET_MB = 6, /* histogram scratch per separable batch when not fused (default 3072)       */
+    MI_OPT_HIST_BUDGET_MB = 7,     /* histogram scratch per chunk of the generic path (default 1024)            */
+    MI_OPT_GENERIC_PAD = 8,        /* pad words per shared row of the generic kernel, 0..64 (default 5)         */
+    MI_OPT_GENERIC_SMEM_KB = 9,    /* shared histogram of the generic kernel in KB (default 196; rest is L1)    */
+    MI_OPT_GENERIC_TY_LOG2 = 10,   /* generic kernel row tile: 2^v rows in y x 32/2^v in z (default 3)          */
+    MI_OPT_GENERIC_UNROLL = 11,    /* generic kernel voxels in flight per lane, 1..4 (0 = from the row length)  */
+    MI_INFO_NUM_SMS = 100,         /* multiprocessors of the context's device                                   */
+    MI_INFO_BIN_MODE = 101,        /* binning variant in effect                                                 */
+    MI_INFO_ZHIST_ROWS = 102,      /* fixed-bin ranks the z kernel counts in shared memory                      */
+    MI_INFO_RARE_VOXELS = 103,     /* fixed voxels of the ranks that do not fit (0 = the epilogue can be fused) */
+    MI_INFO_GENERIC_ROWS = 104,    /* fixed-bin ranks the generic kernel counts in shared memory                */
+    MI_INFO_LAST_PATH = 105        /* path of the last call: 0 generic, 1 separable, 2 wide-histogram kernels   */
+} mi_option;
+mi_status mi_set_option(mi_ctx *ctx, mi_option key, int64_t value);
+mi_status mi_get_option(const mi_ctx *ctx, mi_option key, int64_t *value);
 
 /* Restrict the metric to a subset of the fixed voxels (the random-sampling question of
  * "ITK Mattes uses a random sampling of the image ... while MICUDA uses all the voxels";

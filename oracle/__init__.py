@@ -231,3 +231,28 @@ def mi_map(fixed, fixed_spacing, moving, moving_spacing, nb, flo, fhi, mlo, mhi,
                                    _p(mk.reshape(-1), _u8p) if mk is not None else None,
                                    _p(out, _f64p), _p(am, _i64p))
     return {"map": out, "argmax": am, "threads": int(threads)}
+
+
+def grid_nodes_index_affines(fixed_dims, fixed_spacing, moving_dims, moving_spacing, family, lo, hi, n, nodes):
+    """Index-space transforms (len(nodes), 3, 4) float32 of grid nodes (k0, k1, k2) of the map grid
+    (lo, hi, n): parameter k on axis d is lo[d] + k (hi[d]-lo[d])/(n[d]-1) in double (include/mi.h), then the
+    family generator and CANON-1 -- the same composition orc_map does for every node."""
+    T = []
+    for node in nodes:
+        p = [float(lo[d]) if int(n[d]) == 1 else float(lo[d]) + float(node[d]) * (float(hi[d]) - float(lo[d])) / float(int(n[d]) - 1)
+             for d in range(3)]
+        T.append(family_matrix(family, p))
+    return physical_to_index(np.stack(T), fixed_dims, fixed_spacing, moving_dims, moving_spacing)
+
+
+def mi_map_range(fixed, fixed_spacing, moving, moving_spacing, nb, flo, fhi, mlo, mhi, family, lo, hi, n, begin, end,
+                 q=None, form=TSALLIS_ADDITIVE, interp=INTERP_TRILINEAR, mask=None):
+    """The nodes begin[d] <= k_d < end[d] of the exhaustive map over the grid (lo, hi, n):
+    map (1+nq, m2, m1, m0) with p0 fastest -- each node evaluated by orc_eval_batch."""
+    fx, mv = _vol(fixed), _vol(moving)
+    nodes = [(k0, k1, k2) for k2 in range(begin[2], end[2]) for k1 in range(begin[1], end[1])
+             for k0 in range(begin[0], end[0])]
+    M = grid_nodes_index_affines(_dims(fx), fixed_spacing, _dims(mv), moving_spacing, family, lo, hi, n, nodes)
+    r = eval_batch(fx, mv, M, nb, flo, fhi, mlo, mhi, interp, q=q, form=form, mask=mask)
+    m = [end[d] - begin[d] for d in range(3)]
+    return np.ascontiguousarray(r["mi"].T).reshape(r["mi"].shape[1], m[2], m[1], m[0])

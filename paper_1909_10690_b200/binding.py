@@ -25,7 +25,14 @@ MI_TSALLIS_ADDITIVE, MI_TSALLIS_PSEUDO_ADDITIVE = 0, 1
 _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_ERR_OUT_OF_MEMORY",
            4: "MI_ERR_CUDA", 5: "MI_ERR_INTERNAL"}
 
-EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_map", "mi_destroy", "mi_last_error",
+(MI_OPT_SEPARABLE, MI_OPT_FUSE_ENTROPY, MI_OPT_BIN_MODE_MAX, MI_OPT_ZHIST_ROWS_MAX, MI_OPT_ZHIST_PAD, MI_OPT_XY_BUDGET_MB,
+ MI_OPT_SEP_HIST_BUDGET_MB, MI_OPT_HIST_BUDGET_MB, MI_OPT_GENERIC_PAD, MI_OPT_GENERIC_SMEM_KB, MI_OPT_GENERIC_TY_LOG2,
+ MI_OPT_GENERIC_UNROLL) = range(12)
+(MI_INFO_NUM_SMS, MI_INFO_BIN_MODE, MI_INFO_ZHIST_ROWS, MI_INFO_RARE_VOXELS, MI_INFO_GENERIC_ROWS,
+ MI_INFO_LAST_PATH) = range(100, 106)
+
+EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_map", "mi_map_range", "mi_set_option",
+           "mi_get_option", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
            "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient", "mi_register",
            "mi_probe_shared_atomic_rate", "mi_version")
@@ -47,6 +54,12 @@ _lib.mi_eval_batch.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, C.c_int, _vp
 _lib.mi_eval_batch.restype = C.c_int
 _lib.mi_map.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp]
 _lib.mi_map.restype = C.c_int
+_lib.mi_map_range.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp, _vp]
+_lib.mi_map_range.restype = C.c_int
+_lib.mi_set_option.argtypes = [_vp, C.c_int, C.c_int64]
+_lib.mi_set_option.restype = C.c_int
+_lib.mi_get_option.argtypes = [_vp, C.c_int, _vp]
+_lib.mi_get_option.restype = C.c_int
 _lib.mi_destroy.argtypes = [_vp]
 _lib.mi_destroy.restype = None
 _lib.mi_last_error.argtypes = [_vp]
@@ -226,6 +239,41 @@ def mi_map(ctx, family, lo, hi, n, q=(), interp=MI_INTERP_TRILINEAR, map_out=Non
                      int(interp), _ptr(map_out), _ptr(argmax_out))
     _check(ctx, st)
     return map_out, argmax_out
+
+
+def mi_map_range(ctx, family, lo, hi, n, begin=None, end=None, q=(), interp=MI_INTERP_TRILINEAR, map_out=None,
+                 argmax_out=None, hist_out=None):
+    """Sub-box [begin, end) of the grid (lo, hi, n); node parameters are those of the whole grid.
+    Returns (map (1+nq, m2, m1, m0), argmax (1+nq,) into the sub-box, hist or None); hist_out=True
+    allocates (m2*m1*m0, nbins, nbins) uint32 on the host."""
+    lo, hi, n = _f64(lo, 3), _f64(hi, 3), _i32(n, 3)
+    begin = _i32(begin, 3) if begin is not None else np.zeros(3, dtype=np.int32)
+    end = _i32(end, 3) if end is not None else n.copy()
+    m = [int(end[d] - begin[d]) for d in range(3)]
+    q = _f64(q)
+    nq = q.size
+    if map_out is None:
+        map_out = np.empty((1 + nq, m[2], m[1], m[0]), dtype=np.float64)
+    if argmax_out is None:
+        argmax_out = np.empty(1 + nq, dtype=np.int64)
+    if hist_out is True:
+        hist_out = np.empty((m[2] * m[1] * m[0], ctx.nbins, ctx.nbins), dtype=np.uint32)
+    elif hist_out is False:
+        hist_out = None
+    st = _lib.mi_map_range(ctx.handle, int(family), _ptr(lo), _ptr(hi), _ptr(n), _ptr(begin), _ptr(end),
+                           _ptr(q) if nq else None, nq, int(interp), _ptr(map_out), _ptr(argmax_out), _ptr(hist_out))
+    _check(ctx, st)
+    return map_out, argmax_out, hist_out
+
+
+def mi_set_option(ctx, key, value) -> None:
+    _check(ctx, _lib.mi_set_option(ctx.handle, int(key), int(value)))
+
+
+def mi_get_option(ctx, key) -> int:
+    out = np.zeros(1, dtype=np.int64)
+    _check(ctx, _lib.mi_get_option(ctx.handle, int(key), _ptr(out)))
+    return int(out[0])
 
 
 def mi_family_matrix(family, p) -> np.ndarray:

@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(256) basin_stats_kernel(const int* __restrict_
 unsigned grid_for(int64_t total, int block) {
     int64_t b = (total + block - 1) / block;
     if (b < 1) b = 1;
-    if (b > 148 * 8) b = 148 * 8;
+    if (b > sm_count() * 8) b = sm_count() * 8;
     return (unsigned)b;
 }
 

@@ -29,7 +29,8 @@ struct mi_ctx {
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
-    unsigned rare_cap = 0;              // capacity of d_rare (entries)
+    unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
+    unsigned rare_alloc = 0;            // entries d_rare was allocated for
     bool wide = false;                  // nbins > 256: uint16 bins, global-memory histograms, generic kernel only
     uint16_t* d_fbins16 = nullptr;
     uint16_t* d_mbins16 = nullptr;
@@ -54,9 +55,16 @@ struct mi_ctx {
     size_t sep_hist_budget = (size_t)3 << 30;          // bytes of histogram scratch per batch
     int tsallis_form = MI_TSALLIS_ADDITIVE;
     bool use_separable = true;
-    int num_sms = 148;
+    bool separable_ok = true;                          // false: nbins > 256, or a fixed volume the z kernel cannot index
+    int num_sms = 0;                                   // queried in mi_create
     size_t smem_optin = 48 * 1024;
     size_t hist_budget = (size_t)1 << 30;  // bytes of global histogram scratch per chunk
+    // mi_set_option state (defaults = the measured optimum)
+    int opt_zpad = 9, opt_zrows_max = 0, opt_bin_mode_max = mi::kBinFastPrescaled;
+    int opt_gpad = 5, opt_gsmem_kb = 196, opt_unroll = 0;
+    int bin_mode_natural = mi::kBinGeneral;            // what the data allows (mi_create)
+    unsigned long long h_counts[256] = {};             // fixed-bin populations and ranks (nbins <= 256)
+    uint8_t h_rank[256] = {};
 
     // scratch, grown on demand
     float* d_M = nullptr;      size_t cap_M = 0;       // transforms
@@ -71,6 +79,7 @@ struct mi_ctx {
     bool staging_busy = false;
 
     std::string err;
+    int last_path = 0;                  // 0 generic kernel, 1 separable kernels, 2 wide-histogram kernel (last call)
     float last_ms[5] = {0, 0, 0, 0, 0};
     int64_t last_launches[5] = {0, 0, 0, 0, 0};
 };
@@ -114,6 +123,18 @@ cudaError_t dev_alloc(void** p, size_t bytes, int dev, cudaStream_t s) {
 }
 void dev_free(void* p, cudaStream_t s) {
     if (p) cudaFreeAsync(p, s);
+}
+
+int sm_count() {
+    static int cached[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { cudaGetLastError(); return 1; }
+    if (cached[dev] == 0) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v < 1) { cudaGetLastError(); return 1; }
+        cached[dev] = v;
+    }
+    return cached[dev];
 }
 
 thread_local std::string g_thread_error;
@@ -212,8 +233,59 @@ struct EventTimer {
 mi_status validate_q(mi_ctx* c, const double* q, int32_t nq) {
     if (nq < 0) return fail(c, MI_ERR_INVALID_ARG, "nq < 0");
     if (nq > 0 && q == nullptr) return fail(c, MI_ERR_INVALID_ARG, "q is NULL but nq > 0");
+    // q <= 32: the kernels accumulate sum c^q = sum exp(q ln c) over integer counts c < 2^31 and scale by
+    // N^-q afterwards; 32 ln 2^31 = 687.6 stays below the double overflow threshold (709.78) with room for
+    // the 2^16 terms of a histogram, so no q in range can overflow (include/mi.h documents the bound)
     for (int i = 0; i < nq; ++i)
-        if (!(std::isfinite(q[i]) && q[i] > 0.0)) return fail(c, MI_ERR_INVALID_ARG, "q must be finite and > 0");
+        if (!(std::isfinite(q[i]) && q[i] > 0.0 && q[i] <= 32.0)) return fail(c, MI_ERR_INVALID_ARG, "q must be finite, > 0 and <= 32");
+    return MI_OK;
+}
+
+// Launch layout derived from the options (mi_set_option) and the data: shared-memory rows and row
+// pitches of both histogram kernels, the z kernel's binning variant and -- for the separable path --
+// the pitched fixed bins with the rare-voxel list, which depend on the row count and on the
+// fixed-voxel mask.  Called by mi_create, mi_set_option and mi_set_fixed_mask; the device is current.
+mi_status plan_layout(mi_ctx* c) {
+    cudaStream_t s = c->stream;
+    // generic kernel: the gathers live in L1, which is what the shared histogram leaves of the SM's
+    // 256 KB; above 196 KB of shared memory the next carve-out step leaves only 28 KB
+    size_t gsmem = (size_t)c->opt_gsmem_kb << 10;
+    if (gsmem > c->smem_optin) gsmem = c->smem_optin;
+    c->gpitch = c->nb + c->opt_gpad;
+    c->rows_smem = mi::hist_rows_in_smem(c->nb, c->gpitch, gsmem);
+    if (c->rows_smem < 1) return fail(c, MI_ERR_UNSUPPORTED, "device has too little shared memory");
+    if (c->wide) return MI_OK;
+    c->bin_mode = c->bin_mode_natural < c->opt_bin_mode_max ? c->bin_mode_natural : c->opt_bin_mode_max;
+    // bank of histogram word (a, b) = (a*pad + b) mod 32: an odd pad walks the rows over all banks
+    c->zpitch = c->nb + c->opt_zpad;
+    c->zrows_smem = mi::zhist_rows_in_smem(c->nb, c->zpitch, c->fd[2], c->md[2] + 2, c->smem_optin);
+    if (c->opt_zrows_max >= 2 && c->opt_zrows_max < c->zrows_smem) c->zrows_smem = c->opt_zrows_max;
+    if (!c->separable_ok || c->zrows_smem < 2) return MI_OK;
+    // the separable path keeps ranks < zrows_real in shared memory; if not every bin fits, the last
+    // shared row becomes a dump row and the voxels of the rare ranks go to a list
+    c->zrows_real = c->zrows_smem > c->nb ? c->nb : c->zrows_smem - 1;
+    unsigned long long n_rare = 0;
+    for (int a = 0; a < 256; ++a)
+        if ((int)c->h_rank[a] >= c->zrows_real) n_rare += c->h_counts[a];
+    if (c->d_rare == nullptr || n_rare > c->rare_alloc) {
+        dev_free(c->d_rare, s);
+        c->d_rare = nullptr;
+        MI_CUDA(c, dev_alloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2), c->device, s));
+        c->rare_alloc = (unsigned)n_rare;
+    }
+    c->rare_cap = (unsigned)n_rare;
+    unsigned* d_count = nullptr;
+    MI_CUDA(c, dev_alloc((void**)&d_count, sizeof(unsigned), c->device, s));
+    unsigned h_count = 0;
+    cudaError_t e = cudaMemsetAsync(d_count, 0, sizeof(unsigned), s);
+    if (e == cudaSuccess)
+        e = mi::launch_pitch_bins(c->d_fbins_ranked, c->d_mask_bits, c->fd[0] * c->fd[1], c->colpitch, c->fd[2], c->zrows_real,
+                                  c->d_fb_pitched, c->d_rare, d_count, c->rare_cap, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&h_count, d_count, sizeof(unsigned), cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    dev_free(d_count, s);
+    if (e != cudaSuccess) return cuda_fail(c, e, "pitch fixed bins");
+    c->n_rare = h_count < c->rare_cap ? h_count : c->rare_cap;
     return MI_OK;
 }
 
@@ -254,12 +326,17 @@ bool make_separable_plan(const std::vector<float>& hM, const int32_t n[3], Separ
 
 // Steps a3 + a4 of a separable map: for groups of p0 values run the x-pass, the y-pass for every
 // (p0,p1) pair of the group, then one z-lerp + histogram item per transform, then the entropy
-// kernel (a5) writing straight into map order.  Results land in c->d_mi / c->d_nvalid.
-mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int interp, EventTimer& timer) {
+// kernel (a5) writing straight into map order.  Results land in c->d_mi / c->d_nvalid; the joint
+// histograms, if asked for (hist_out: host or device, map order), are copied out item by item.
+// When even one (p0,p1) pair does not fit the scratch budgets the function returns kSepFallback and
+// the caller takes the generic kernel (same arithmetic, no scratch).
+constexpr mi_status kSepFallback = static_cast<mi_status>(-1);
+
+mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int interp, EventTimer& timer,
+                        uint32_t* hist_out) {
     cudaStream_t s = c->stream;
     const bool nn = interp == MI_INTERP_NEAREST;
     const int n0 = sp.n[0], n1 = sp.n[1], n2 = sp.n[2];
-    const int nch = 1 + nq;
     const size_t nbins2 = (size_t)c->nb * c->nb;
     const int fnx = c->fd[0], cols = c->fd[0] * c->fd[1], fnz = c->fd[2];
     const int planes = nn ? c->md[2] : c->md[2] + 2;
@@ -268,33 +345,38 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
     const size_t x_bytes_per_a = (size_t)planes * prows * fnx * elem;
     const size_t xy_bytes_per_pair = (size_t)planes * c->colpitch * elem;
     // fused: step a5 runs as the z kernel's epilogue and no histogram leaves the SM
-    const bool fused = c->fuse_entropy && c->n_rare == 0 && nq <= mi::kMaxQPerPass;
+    const bool fused = c->fuse_entropy && c->n_rare == 0 && nq <= mi::kMaxQPerPass && hist_out == nullptr;
     const size_t hist_bytes_per_pair = fused ? 1 : (size_t)n2 * nbins2 * sizeof(uint32_t);
 
-    // p0 values per batch: as many as the scratch budgets allow, chosen to minimise idle SM-waves
+    // Batch = ga values of p0 x gb values of p1.  Whole p0 slabs (gb = n1) when the scratch budgets
+    // allow, as many as minimise idle SM-waves; otherwise one p0 at a time in chunks of p1.
     size_t max_pairs = c->xy_budget / xy_bytes_per_pair;
     if (c->sep_hist_budget / hist_bytes_per_pair < max_pairs) max_pairs = c->sep_hist_budget / hist_bytes_per_pair;
-    if (max_pairs > 65535) max_pairs = 65535;  // gridDim.z of the y-pass
-    int ga_max = (int)(max_pairs / (size_t)n1);
-    if (ga_max > n0) ga_max = n0;
-    if (ga_max < 1) return fail(c, MI_ERR_OUT_OF_MEMORY, "separable map: one p0 slab exceeds the scratch budget");
-    int ga = 1;
-    long long best_waves = -1;
-    for (int g = 1; g <= ga_max; ++g) {
-        const long long per = ((long long)g * n1 * n2 + c->num_sms - 1) / c->num_sms;
-        const int rem = n0 % g;
-        long long waves = (long long)(n0 / g) * per;
-        if (rem) waves += ((long long)rem * n1 * n2 + c->num_sms - 1) / c->num_sms;
-        if (best_waves < 0 || waves <= best_waves) { best_waves = waves; ga = g; }
+    if (max_pairs > 65535) max_pairs = 65535;  // gridDim.y of the y-pass
+    if (max_pairs < 1) return kSepFallback;
+    int ga = 1, gb = n1;
+    if (max_pairs >= (size_t)n1) {
+        int ga_max = (int)(max_pairs / (size_t)n1);
+        if (ga_max > n0) ga_max = n0;
+        long long best_waves = -1;
+        for (int g = 1; g <= ga_max; ++g) {
+            const long long per = ((long long)g * n1 * n2 + c->num_sms - 1) / c->num_sms;
+            const int rem = n0 % g;
+            long long waves = (long long)(n0 / g) * per;
+            if (rem) waves += ((long long)rem * n1 * n2 + c->num_sms - 1) / c->num_sms;
+            if (best_waves < 0 || waves <= best_waves) { best_waves = waves; ga = g; }
+        }
+    } else {
+        gb = (int)max_pairs;
     }
 
     mi_status st;
     const int nmax = n0 > n1 ? (n0 > n2 ? n0 : n2) : (n1 > n2 ? n1 : n2);
     if ((st = grow(c, &c->d_axis, &c->cap_axis, (size_t)3 * nmax)) != MI_OK) return st;
     if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_X), &c->cap_X, (size_t)ga * x_bytes_per_a)) != MI_OK) return st;
-    if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_XY), &c->cap_XY, (size_t)ga * n1 * xy_bytes_per_pair)) != MI_OK) return st;
-    if ((st = grow(c, &c->d_colvalid, &c->cap_cv, (size_t)ga * n1 * c->colpitch)) != MI_OK) return st;
-    if (!fused && (st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist, (size_t)ga * n1 * hist_bytes_per_pair)) != MI_OK) return st;
+    if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_XY), &c->cap_XY, (size_t)ga * gb * xy_bytes_per_pair)) != MI_OK) return st;
+    if ((st = grow(c, &c->d_colvalid, &c->cap_cv, (size_t)ga * gb * c->colpitch)) != MI_OK) return st;
+    if (!fused && (st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist, (size_t)ga * gb * hist_bytes_per_pair)) != MI_OK) return st;
     const float prescale = (!nn && c->bin_mode == mi::kBinFastPrescaled) ? c->mscale : 1.0f;
     for (int d = 0; d < 3; ++d)
         MI_CUDA(c, cudaMemcpyAsync(c->d_axis + (size_t)d * nmax, sp.axis[d].data(), sp.axis[d].size() * sizeof(float2),
@@ -305,64 +387,74 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
 
     for (int a0 = 0; a0 < n0; a0 += ga) {
         const int na = (n0 - a0 < ga) ? (n0 - a0) : ga;
-        const int npairs = na * n1;
-        const long long items = (long long)npairs * n2;
-        timer.begin(1);
-        if (nn)
-            MI_CUDA(c, mi::launch_xpass(true, c->d_mbins, c->md[0], c->md[2] * c->md[1], c->md[0], ax, a0, na, fnx, c->d_X, s));
-        else
-            MI_CUDA(c, mi::launch_xpass(false, c->d_moving_pad, c->md[0] + 2, planes * prows, c->md[0], ax, a0, na, fnx, c->d_X, s));
-        MI_CUDA(c, mi::launch_ypass(nn, c->d_X, planes, prows, c->md[0], c->md[1], ax, ay, a0, n1, npairs, fnx, cols,
-                                    c->colpitch, prescale, c->d_XY, c->d_colvalid, s));
-        mi::ZHistArgs z;
-        z.xy = c->d_XY;
-        z.colvalid = c->d_colvalid;
-        z.fb = c->d_fb_pitched;
-        z.rank_inv = c->d_rank_inv;
-        z.az = az;
-        z.hist = c->d_hist;
-        z.fnz = fnz;
-        z.colpitch = c->colpitch;
-        z.planes = planes;
-        z.mnz = c->md[2];
-        z.nb = c->nb;
-        z.rows_smem = c->zrows_smem;
-        z.pitch = c->zpitch;
-        z.bin_mode = c->bin_mode;
-        z.rows_real = c->zrows_real;
-        z.rare = c->d_rare;
-        z.n_rare = c->n_rare;
-        z.mlo = c->mlo;
-        z.mscale = c->mscale;
-        z.n_pairs = npairs;
-        z.n2 = n2;
-        z.fused = fused ? 1 : 0;
-        z.q = c->d_q;
-        z.nq = nq;
-        z.nq_total = nq;
-        z.form = c->tsallis_form;
-        z.mi_out = c->d_mi;
-        z.nvalid = c->d_nvalid;
-        z.om = mi::OutMap{1, n0, n1, n2, a0};
-        timer.begin(4);
-        MI_CUDA(c, mi::launch_zhist(nn, z, c->num_sms, s));
-        timer.end();
-        c->last_launches[1] += 3 + (c->n_rare > 0 ? 1 : 0);
-        c->last_launches[4] += 1;
-        timer.end();
-        if (fused) continue;
+        for (int b0 = 0; b0 < n1; b0 += gb) {
+            const int nbc = (n1 - b0 < gb) ? (n1 - b0) : gb;
+            const int npairs = na * nbc;
+            const long long items = (long long)npairs * n2;
+            const mi::OutMap om{1, n0, n1, n2, a0, b0, nbc};
+            timer.begin(1);
+            if (b0 == 0) {   // the x-lerped rows of a p0 group serve all of its p1 chunks
+                if (nn)
+                    MI_CUDA(c, mi::launch_xpass(true, c->d_mbins, c->md[0], c->md[2] * c->md[1], c->md[0], ax, a0, na, fnx, c->d_X, s));
+                else
+                    MI_CUDA(c, mi::launch_xpass(false, c->d_moving_pad, c->md[0] + 2, planes * prows, c->md[0], ax, a0, na, fnx, c->d_X, s));
+                c->last_launches[1] += 1;
+            }
+            MI_CUDA(c, mi::launch_ypass(nn, c->d_X, planes, prows, c->md[0], c->md[1], ax, ay, a0, b0, nbc, npairs, fnx, cols,
+                                        c->colpitch, prescale, c->d_XY, c->d_colvalid, s));
+            mi::ZHistArgs z;
+            z.xy = c->d_XY;
+            z.colvalid = c->d_colvalid;
+            z.fb = c->d_fb_pitched;
+            z.rank_inv = c->d_rank_inv;
+            z.az = az;
+            z.hist = c->d_hist;
+            z.fnz = fnz;
+            z.colpitch = c->colpitch;
+            z.planes = planes;
+            z.mnz = c->md[2];
+            z.nb = c->nb;
+            z.rows_smem = c->zrows_smem;
+            z.pitch = c->zpitch;
+            z.bin_mode = c->bin_mode;
+            z.rows_real = c->zrows_real;
+            z.rare = c->d_rare;
+            z.n_rare = c->n_rare;
+            z.mlo = c->mlo;
+            z.mscale = c->mscale;
+            z.n_pairs = npairs;
+            z.n2 = n2;
+            z.fused = fused ? 1 : 0;
+            z.q = c->d_q;
+            z.nq = nq;
+            z.nq_total = nq;
+            z.form = c->tsallis_form;
+            z.mi_out = c->d_mi;
+            z.nvalid = c->d_nvalid;
+            z.om = om;
+            timer.begin(4);
+            MI_CUDA(c, mi::launch_zhist(nn, z, c->num_sms, s));
+            timer.end();
+            c->last_launches[1] += 2 + (c->n_rare > 0 ? 1 : 0);
+            c->last_launches[4] += 1;
+            timer.end();
+            if (fused) continue;
 
-        timer.begin(2);
-        int q_off = 0;
-        do {
-            MI_CUDA(c, mi::launch_entropy(c->d_hist, c->nb, (int)items, c->d_q, nq, q_off, c->tsallis_form, c->d_mi,
-                                          c->d_nvalid, mi::OutMap{1, n0, n1, n2, a0}, s));
-            c->last_launches[2] += 1;
-            q_off += mi::kMaxQPerPass;
-        } while (q_off < nq);
-        timer.end();
+            timer.begin(2);
+            int q_off = 0;
+            do {
+                MI_CUDA(c, mi::launch_entropy(c->d_hist, c->nb, (int)items, c->d_q, nq, q_off, c->tsallis_form, c->d_mi,
+                                              c->d_nvalid, om, s));
+                c->last_launches[2] += 1;
+                q_off += mi::kMaxQPerPass;
+            } while (q_off < nq);
+            timer.end();
+            if (hist_out != nullptr)
+                for (long long item = 0; item < items; ++item)
+                    MI_CUDA(c, cudaMemcpyAsync(hist_out + om.dst(item) * nbins2, c->d_hist + (size_t)item * nbins2,
+                                               nbins2 * sizeof(uint32_t), cudaMemcpyDefault, s));
+        }
     }
-    (void)nch;
     return MI_OK;
 }
 
@@ -403,6 +495,12 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * sizeof(uint32_t)));
     if (chunk < 1) chunk = 1;
     if (chunk > N) chunk = N;
+    if (sep != nullptr) {
+        st = run_separable(c, *sep, nq, interp, timer, hist_out);
+        if (st == kSepFallback) sep = nullptr;   // one (p0,p1) pair exceeds the scratch budgets: generic kernel
+        else if (st != MI_OK) return st;
+    }
+    c->last_path = sep != nullptr ? 1 : (c->wide ? 2 : 0);
     if (!hist_to_user_dev && sep == nullptr) {
         if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist,
                        (size_t)chunk * nbins2 * sizeof(uint32_t))) != MI_OK)
@@ -410,10 +508,6 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     }
     const int rows_total = c->fd[1] * c->fd[2];
 
-    if (sep != nullptr) {
-        st = run_separable(c, *sep, nq, interp, timer);
-        if (st != MI_OK) return st;
-    }
     for (int64_t off = 0; sep == nullptr && off < N; off += chunk) {
         const int64_t cnt = (N - off < chunk) ? (N - off) : chunk;
         uint32_t* hist = hist_to_user_dev ? hist_out + (size_t)off * nbins2 : c->d_hist;
@@ -429,8 +523,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.rows_smem = c->rows_smem;
         a.pitch = c->gpitch;
         a.ty_log2 = c->ty_log2;
-        a.unroll = 0;
-        if (const char* v = std::getenv("MI_B200_GENERIC_UNROLL")) a.unroll = std::atoi(v);
+        a.unroll = c->opt_unroll;
         a.M = c->d_M + (size_t)off * 12;
         a.hist = hist;
         a.f = {c->fd[0], c->fd[1], c->fd[2]};
@@ -478,7 +571,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         int q_off = 0;
         do {
             MI_CUDA(c, mi::launch_entropy(hist, c->nb, (int)cnt, c->d_q, nq, q_off, c->tsallis_form,
-                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, mi::OutMap{0, 0, 0, 0, 0}, s));
+                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, mi::OutMap{0, 0, 0, 0, 0, 0, 0}, s));
             c->last_launches[2] += 1;
             q_off += mi::kMaxQPerPass;
         } while (q_off < nq);
@@ -630,27 +723,7 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = dev_alloc((void**)&d_tmp, (size_t)nf * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
         c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + mi::kZColAlign - 1) / mi::kZColAlign * mi::kZColAlign);
         if ((e = dev_alloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
-        // bank of histogram word (a, b) = (a*pad + b) mod 32: an odd pad walks the rows over all banks
-        int zpad = 9;
-        if (const char* v = std::getenv("MI_B200_HIST_PAD")) { const int r = std::atoi(v); if (r >= 1 && r <= 64) zpad = r; }
-        if (const char* v = std::getenv("MI_B200_FUSE_ENTROPY")) c->fuse_entropy = std::atoi(v) != 0;
-        c->zpitch = nbins + zpad;
-        c->zrows_smem = mi::zhist_rows_in_smem(nbins, c->zpitch, fixed_dims[2], moving_dims[2] + 2, c->smem_optin);
-        // generic kernel: the gathers live in L1, which is what the shared histogram leaves of the
-        // SM's 256 KB; above 196 KB of shared memory the next carve-out step leaves only 28 KB
-        int gpad = 5;
-        size_t gsmem = c->smem_optin < (size_t)196 * 1024 ? c->smem_optin : (size_t)196 * 1024;
-        if (const char* v = std::getenv("MI_B200_GENERIC_PAD")) { const int r = std::atoi(v); if (r >= 0 && r <= 64) gpad = r; }
-        if (const char* v = std::getenv("MI_B200_GENERIC_SMEM_KB")) { const size_t r = (size_t)std::atoll(v) << 10; if (r >= 8192 && r <= c->smem_optin) gsmem = r; }
-        if (const char* v = std::getenv("MI_B200_GENERIC_TY")) { const int r = std::atoi(v); if (r >= 0 && r <= 5) c->ty_log2 = r; }
-        c->gpitch = nbins + gpad;
-        c->rows_smem = mi::hist_rows_in_smem(nbins, c->gpitch, gsmem);
-        // test knobs (tests/ shrink the scratch budgets to force several batches, or disable the path)
-        if (const char* v = std::getenv("MI_B200_SEPARABLE")) c->use_separable = std::atoi(v) != 0;
-        if (const char* v = std::getenv("MI_B200_XY_BUDGET_MB")) c->xy_budget = (size_t)std::atoll(v) << 20;
-        if (const char* v = std::getenv("MI_B200_SEP_HIST_BUDGET_MB")) c->sep_hist_budget = (size_t)std::atoll(v) << 20;
-        if (const char* v = std::getenv("MI_B200_ZROWS")) { const int r = std::atoi(v); if (r >= 2 && r < c->zrows_smem) c->zrows_smem = r; }
-        if (c->rows_smem < 1) { st = fail(nullptr, MI_ERR_UNSUPPORTED, "device has too little shared memory"); break; }
+        c->separable_ok = nbins <= 256 && fixed_dims[2] <= 65535;   // the rare list packs iz into 16 bits
         if ((e = cudaEventCreateWithFlags(&c->ev_staging, cudaEventDisableTiming)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaEventCreate"); break; }
         cudaStream_t s = c->stream;
         if ((e = cudaMemcpyAsync(d_tmp, fixed, (size_t)nf * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy fixed"); break; }
@@ -658,7 +731,6 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = cudaMemsetAsync(d_counts, 0, 256 * sizeof(unsigned long long), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
         c->wide = nbins > 256;
         if (c->wide) {
-            c->use_separable = false;
             if ((e = dev_alloc((void**)&c->d_fbins16, (size_t)nf * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide fixed bins"); break; }
             if ((e = dev_alloc((void**)&c->d_mbins16, (size_t)nm * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide moving bins"); break; }
             if ((e = mi::launch_prebin16(d_tmp, c->d_fbins16, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed (wide)"); break; }
@@ -674,30 +746,14 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
                 // (so that scaling commutes with every rounding; 2^-100 < scale keeps products normal)
                 int ex = 0;
                 const bool pow2 = std::frexp(c->mscale, &ex) == 0.5f && ex > -100 && ex < 100;
-                c->bin_mode = (h_flag == 0 && c->mlo == 0.0f) ? (pow2 ? mi::kBinFastPrescaled : mi::kBinFast) : mi::kBinGeneral;
-                if (const char* v = std::getenv("MI_B200_BIN_MODE")) { const int r = std::atoi(v); if (r >= 0 && r < c->bin_mode) c->bin_mode = r; }
+                c->bin_mode_natural = (h_flag == 0 && c->mlo == 0.0f) ? (pow2 ? mi::kBinFastPrescaled : mi::kBinFast) : mi::kBinGeneral;
             }
             if ((e = mi::launch_rank_fixed_bins(c->d_fbins, nf, d_counts, c->d_rank, c->d_rank_inv, c->d_fbins_ranked, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank fixed bins"); break; }
-            {
-                // the separable path keeps ranks < zrows_real in shared memory; if not every bin fits, the
-                // last shared row becomes a dump row and the voxels of the rare ranks go to a list
-                unsigned long long h_counts[256];
-                uint8_t h_rank[256];
-                if ((e = cudaMemcpyAsync(h_counts, d_counts, sizeof(h_counts), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy counts"); break; }
-                if ((e = cudaMemcpyAsync(h_rank, c->d_rank, sizeof(h_rank), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy ranks"); break; }
-                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync ranks"); break; }
-                c->zrows_real = c->zrows_smem > nbins ? nbins : c->zrows_smem - 1;   // one row is the dump row
-                unsigned long long n_rare = 0;
-                for (int a = 0; a < 256; ++a)
-                    if ((int)h_rank[a] >= c->zrows_real) n_rare += h_counts[a];
-                c->n_rare = (unsigned)n_rare;
-                c->rare_cap = (unsigned)n_rare;
-                if ((e = dev_alloc((void**)&c->d_rare, (size_t)(n_rare + 1) * sizeof(uint2), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rare list"); break; }
-                if ((e = cudaMemsetAsync(d_counts, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "memset"); break; }
-                if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, nullptr, fixed_dims[0] * fixed_dims[1], c->colpitch, fixed_dims[2], c->zrows_real,
-                                               c->d_fb_pitched, c->d_rare, reinterpret_cast<unsigned*>(d_counts), c->n_rare, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pitch fixed bins"); break; }
-            }
+            if ((e = cudaMemcpyAsync(c->h_counts, d_counts, sizeof(c->h_counts), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy counts"); break; }
+            if ((e = cudaMemcpyAsync(c->h_rank, c->d_rank, sizeof(c->h_rank), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy ranks"); break; }
+            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync ranks"); break; }
         }
+        if ((st = plan_layout(c)) != MI_OK) { mi::set_thread_error(c->err); break; }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
@@ -744,7 +800,6 @@ mi_status mi_set_fixed_mask(mi_ctx* c, const uint8_t* mask) {
     if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
     cudaStream_t s = c->stream;
     uint8_t* d_mask = nullptr;
-    unsigned* d_count = nullptr;
     mi_status st = MI_OK;
     do {
         cudaError_t e;
@@ -758,22 +813,11 @@ mi_status mi_set_fixed_mask(mi_ctx* c, const uint8_t* mask) {
             dev_free(c->d_mask_bits, s);
             c->d_mask_bits = nullptr;
         }
-        if (!c->wide) {
-            // the separable path reads the mask through its pitched fixed bins: rebuild them (and the rare list)
-            unsigned h_count = 0;
-            if ((e = dev_alloc((void**)&d_count, sizeof(unsigned), c->device, s)) != cudaSuccess) { st = cuda_fail(c, e, "cudaMalloc counter"); break; }
-            if ((e = cudaMemsetAsync(d_count, 0, sizeof(unsigned), s)) != cudaSuccess) { st = cuda_fail(c, e, "memset"); break; }
-            if ((e = mi::launch_pitch_bins(c->d_fbins_ranked, d_mask, c->fd[0] * c->fd[1], c->colpitch, c->fd[2], c->zrows_real,
-                                           c->d_fb_pitched, c->d_rare, d_count, c->rare_cap, s)) != cudaSuccess) { st = cuda_fail(c, e, "pitch fixed bins"); break; }
-            if ((e = cudaMemcpyAsync(&h_count, d_count, sizeof(unsigned), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(c, e, "copy counter"); break; }
-            if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(c, e, "sync"); break; }
-            c->n_rare = h_count < c->rare_cap ? h_count : c->rare_cap;
-        } else if ((e = cudaStreamSynchronize(s)) != cudaSuccess) {
-            st = cuda_fail(c, e, "sync");
-        }
+        // the separable path reads the mask through its pitched fixed bins: rebuild them (and the rare list)
+        st = plan_layout(c);
+        if (st == MI_OK && (e = cudaStreamSynchronize(s)) != cudaSuccess) st = cuda_fail(c, e, "sync");
     } while (false);
     dev_free(d_mask, s);
-    dev_free(d_count, s);
     return st;
 }
 
@@ -782,6 +826,78 @@ mi_status mi_set_tsallis_form(mi_ctx* c, mi_tsallis_form form) {
     if (form != MI_TSALLIS_ADDITIVE && form != MI_TSALLIS_PSEUDO_ADDITIVE)
         return fail(c, MI_ERR_INVALID_ARG, "unknown Tsallis form");
     c->tsallis_form = (int)form;
+    return MI_OK;
+}
+
+mi_status mi_set_option(mi_ctx* c, mi_option key, int64_t v) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    bool relayout = false;
+    auto bad = [&]() { return fail(c, MI_ERR_INVALID_ARG, "mi_set_option: value out of range"); };
+    switch (key) {
+    case MI_OPT_SEPARABLE: c->use_separable = v != 0; break;
+    case MI_OPT_FUSE_ENTROPY: c->fuse_entropy = v != 0; break;
+    case MI_OPT_BIN_MODE_MAX:
+        if (v < mi::kBinGeneral || v > mi::kBinFastPrescaled) return bad();
+        c->opt_bin_mode_max = (int)v; relayout = true; break;
+    case MI_OPT_ZHIST_ROWS_MAX:
+        if (v != 0 && (v < 2 || v > 257)) return bad();
+        c->opt_zrows_max = (int)v; relayout = true; break;
+    case MI_OPT_ZHIST_PAD:
+        if (v < 1 || v > 64) return bad();
+        c->opt_zpad = (int)v; relayout = true; break;
+    case MI_OPT_XY_BUDGET_MB:
+        if (v < 0 || v > (1 << 20)) return bad();
+        c->xy_budget = (size_t)v << 20; break;
+    case MI_OPT_SEP_HIST_BUDGET_MB:
+        if (v < 0 || v > (1 << 20)) return bad();
+        c->sep_hist_budget = (size_t)v << 20; break;
+    case MI_OPT_HIST_BUDGET_MB:
+        if (v < 1 || v > (1 << 20)) return bad();
+        c->hist_budget = (size_t)v << 20; break;
+    case MI_OPT_GENERIC_PAD:
+        if (v < 0 || v > 64) return bad();
+        c->opt_gpad = (int)v; relayout = true; break;
+    case MI_OPT_GENERIC_SMEM_KB:
+        if (v < 8 || v > (int64_t)(c->smem_optin >> 10)) return bad();
+        c->opt_gsmem_kb = (int)v; relayout = true; break;
+    case MI_OPT_GENERIC_TY_LOG2:
+        if (v < 0 || v > 5) return bad();
+        c->ty_log2 = (int)v; break;
+    case MI_OPT_GENERIC_UNROLL:
+        if (v < 0 || v > 4) return bad();
+        c->opt_unroll = (int)v; break;
+    default:
+        return fail(c, MI_ERR_INVALID_ARG, "mi_set_option: unknown or read-only key");
+    }
+    if (!relayout) return MI_OK;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    return plan_layout(c);
+}
+
+mi_status mi_get_option(const mi_ctx* c, mi_option key, int64_t* out) {
+    if (!c || !out) return MI_ERR_INVALID_ARG;
+    switch (key) {
+    case MI_OPT_SEPARABLE: *out = c->use_separable; break;
+    case MI_OPT_FUSE_ENTROPY: *out = c->fuse_entropy; break;
+    case MI_OPT_BIN_MODE_MAX: *out = c->opt_bin_mode_max; break;
+    case MI_OPT_ZHIST_ROWS_MAX: *out = c->opt_zrows_max; break;
+    case MI_OPT_ZHIST_PAD: *out = c->opt_zpad; break;
+    case MI_OPT_XY_BUDGET_MB: *out = (int64_t)(c->xy_budget >> 20); break;
+    case MI_OPT_SEP_HIST_BUDGET_MB: *out = (int64_t)(c->sep_hist_budget >> 20); break;
+    case MI_OPT_HIST_BUDGET_MB: *out = (int64_t)(c->hist_budget >> 20); break;
+    case MI_OPT_GENERIC_PAD: *out = c->opt_gpad; break;
+    case MI_OPT_GENERIC_SMEM_KB: *out = c->opt_gsmem_kb; break;
+    case MI_OPT_GENERIC_TY_LOG2: *out = c->ty_log2; break;
+    case MI_OPT_GENERIC_UNROLL: *out = c->opt_unroll; break;
+    case MI_INFO_NUM_SMS: *out = c->num_sms; break;
+    case MI_INFO_BIN_MODE: *out = c->bin_mode; break;
+    case MI_INFO_ZHIST_ROWS: *out = c->wide ? 0 : c->zrows_real; break;
+    case MI_INFO_RARE_VOXELS: *out = c->wide ? 0 : (int64_t)c->n_rare; break;
+    case MI_INFO_GENERIC_ROWS: *out = c->rows_smem; break;
+    case MI_INFO_LAST_PATH: *out = c->last_path; break;
+    default: return MI_ERR_INVALID_ARG;
+    }
     return MI_OK;
 }
 
@@ -942,18 +1058,24 @@ mi_status mi_register(mi_ctx* c, const double p0[9], const double delta[9], cons
     return MI_OK;
 }
 
-mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
-                 const double* q, int32_t nq, mi_interp interp, double* map_out, int64_t* argmax_out) {
+mi_status mi_map_range(mi_ctx* c, mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
+                       const int32_t begin[3], const int32_t end[3], const double* q, int32_t nq, mi_interp interp,
+                       double* map_out, int64_t* argmax_out, uint32_t* hist_out) {
     if (!c) return MI_ERR_INVALID_ARG;
     if (!lo || !hi || !n || !map_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
     if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
         return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
     if ((int)family < 0 || (int)family > MI_FAMILY_SCALE_LOG) return fail(c, MI_ERR_INVALID_ARG, "unknown family");
     if (!finite3(lo) || !finite3(hi)) return fail(c, MI_ERR_INVALID_ARG, "non-finite grid bound");
+    int32_t kb[3], m[3];   // first node and node count of the sub-box per axis
     int64_t N = 1;
     for (int d = 0; d < 3; ++d) {
         if (n[d] < 1) return fail(c, MI_ERR_INVALID_ARG, "grid n < 1");
-        N *= n[d];
+        kb[d] = begin ? begin[d] : 0;
+        const int32_t ke = end ? end[d] : n[d];
+        if (kb[d] < 0 || ke > n[d] || ke <= kb[d]) return fail(c, MI_ERR_INVALID_ARG, "empty or out-of-grid node range");
+        m[d] = ke - kb[d];
+        N *= m[d];
         if (N > 0x7FFFFFFFLL / 16) return fail(c, MI_ERR_UNSUPPORTED, "too many transforms in one call");
     }
     mi_status st = validate_q(c, q, nq);
@@ -964,18 +1086,20 @@ mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double h
     } catch (const std::bad_alloc&) {
         return fail(c, MI_ERR_OUT_OF_MEMORY, "host allocation failed");
     }
-    // step a2: one transform per grid node, p0 fastest
-    for (int k2 = 0; k2 < n[2]; ++k2)
-        for (int k1 = 0; k1 < n[1]; ++k1)
-            for (int k0 = 0; k0 < n[0]; ++k0) {
-                const int kk[3] = {k0, k1, k2};
+    // step a2: one transform per node of the sub-box, p0 fastest.  Node k of axis d has the parameter
+    // of the WHOLE grid, lo + k (hi - lo)/(n - 1): a slab computed here is bit-identical to the same
+    // nodes of the full map.
+    for (int j2 = 0; j2 < m[2]; ++j2)
+        for (int j1 = 0; j1 < m[1]; ++j1)
+            for (int j0 = 0; j0 < m[0]; ++j0) {
+                const int kk[3] = {kb[0] + j0, kb[1] + j1, kb[2] + j2};
                 double p[3], T[12];
                 for (int d = 0; d < 3; ++d)
                     p[d] = n[d] == 1 ? lo[d] : lo[d] + (double)kk[d] * (hi[d] - lo[d]) / (double)(n[d] - 1);
                 mi::family_matrix((int)family, p, T);
                 for (int i = 0; i < 12; ++i)
                     if (!std::isfinite(T[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite matrix entry");
-                const int64_t t = ((int64_t)k2 * n[1] + k1) * n[0] + k0;
+                const int64_t t = ((int64_t)j2 * m[1] + j1) * m[0] + j0;
                 mi::index_affine(T, c->fd, c->fs, c->md, c->ms, hM.data() + t * 12);
             }
     DeviceGuard guard(c->device);
@@ -983,9 +1107,14 @@ mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double h
     // translation / scale maps have diagonal matrices: separable fast path (same arithmetic)
     SeparablePlan plan;
     const bool diag_family = family == MI_FAMILY_TRANSLATION || family == MI_FAMILY_SCALE || family == MI_FAMILY_SCALE_LOG;
-    const bool sep = diag_family && c->use_separable && c->zrows_smem >= 2 && c->fd[2] <= 65535 && make_separable_plan(hM, n, &plan);
-    return eval_core(c, hM, N, q, nq, (int)interp, nullptr, nullptr, nullptr, map_out, argmax_out,
+    const bool sep = diag_family && c->use_separable && c->separable_ok && c->zrows_smem >= 2 && make_separable_plan(hM, m, &plan);
+    return eval_core(c, hM, N, q, nq, (int)interp, nullptr, hist_out, nullptr, map_out, argmax_out,
                      sep ? &plan : nullptr);
+}
+
+mi_status mi_map(mi_ctx* c, mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
+                 const double* q, int32_t nq, mi_interp interp, double* map_out, int64_t* argmax_out) {
+    return mi_map_range(c, family, lo, hi, n, nullptr, nullptr, q, nq, interp, map_out, argmax_out, nullptr);
 }
 
 mi_status mi_get_bins(mi_ctx* c, int32_t which, void* out) {

@@ -16,6 +16,7 @@ cudaError_t dev_alloc(void** p, size_t bytes, int dev, cudaStream_t s);
 void dev_free(void* p, cudaStream_t s);
 void set_thread_error(const std::string& msg);   // text behind mi_last_error(NULL)
 bool is_host_pointer(const void* p);
+int sm_count();                                  // SMs of the current device (queried once per device)
 
 constexpr int kMaxQPerPass = 8;      // Tsallis orders handled by one entropy-kernel pass
 constexpr int kHistThreads = 1024;   // resample+histogram CTA size
@@ -78,11 +79,19 @@ cudaError_t launch_prebin16(const float* vol, uint16_t* bins, int64_t n, float l
 cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s);
 cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms, cudaStream_t s);
 // Where the entropy kernel writes the result of histogram `item`: transform-major position item
-// (enabled == 0) or, for the separable path whose items are ordered (p0, p1, p2) with p2 fastest,
-// the map's transform index (p2*n1 + p1)*n0 + p0.
+// (enabled == 0) or, for the separable path whose items are ordered (p0, p1, p2) with p2 fastest
+// over a batch of nb1 p1 values starting at b0 and p0 values starting at a0, the map's transform
+// index (p2*n1 + p1)*n0 + p0.
 struct OutMap {
     int enabled;
     int n0, n1, n2, a0;
+    int b0, nb1;
+    __host__ __device__ size_t dst(long long item) const {
+        if (!enabled) return (size_t)item;
+        const long long c = item % n2, ab = item / n2;
+        const long long b = ab % nb1, al = ab / nb1;
+        return ((size_t)c * n1 + (size_t)(b0 + b)) * n0 + (size_t)(a0 + al);
+    }
 };
 cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const double* q_dev, int nq,
                            int q_off, int form, double* mi_out /* n x (1+nq) */, int64_t* nvalid,
@@ -125,12 +134,13 @@ struct ZHistArgs {
 enum { kBinGeneral = 0, kBinFast = 1, kBinFastPrescaled = 2 };
 constexpr int kZCols = 8;            // columns per thread of the z kernel: 2 groups of 4
 constexpr int kZColAlign = 32 * kZCols;  // colpitch is a multiple of this (one warp's columns)
-cudaError_t launch_pitch_bins(const uint8_t* in, const uint8_t* mask, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
+cudaError_t launch_pitch_bins(const uint8_t* in, const uint32_t* mask_bits, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
                               uint2* rare, unsigned* rare_count, unsigned rare_cap, cudaStream_t s);
 cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, const float2* ax, int a0,
                          int na, int fnx, void* X, cudaStream_t s);
+// pair = a_local*nb1 + b_local covers p0 index a0 + a_local and p1 index b0 + b_local
 cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
-                         const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
+                         const float2* ay, int a0, int b0, int nb1, int npairs, int fnx, int cols, int colpitch,
                          float prescale, void* XY, uint8_t* colvalid, cudaStream_t s);
 int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin);
 cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t s);

@@ -77,7 +77,7 @@ cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, 
     const int64_t nvec = n >> 4;
     int64_t blocks = (nvec + 255) / 256;
     if (blocks < 1) blocks = 1;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     prebin_kernel<<<(unsigned)blocks, 256, 0, s>>>(vol, bins, n, lo, scale, (float)(nb - 1), flag);
     return cudaGetLastError();
 }
@@ -105,7 +105,7 @@ __global__ void __launch_bounds__(256) pad_replicate_kernel(const float* __restr
 cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s) {
     const int64_t total = (int64_t)(nx + 2) * (ny + 2) * (nz + 2);
     int64_t blocks = (total + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     pad_replicate_kernel<<<(unsigned)blocks, 256, 0, s>>>(src, dst, nx, ny, nz);
     return cudaGetLastError();
 }
@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(256) mask_bits_kernel(const uint8_t* __restric
 cudaError_t launch_mask_bits(const uint8_t* mask, int64_t n, uint32_t* bits, cudaStream_t s) {
     int64_t blocks = (n + 255) / 256;
     if (blocks < 1) blocks = 1;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     mask_bits_kernel<<<(unsigned)blocks, 256, 0, s>>>(mask, n, bits);
     return cudaGetLastError();
 }
@@ -184,7 +184,7 @@ cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long
     if (e != cudaSuccess) return e;
     int64_t blocks = (n + 255) / 256;
     if (blocks < 1) blocks = 1;
-    if (blocks > 148 * 8) blocks = 148 * 8;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
     bin_count_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, n, counts_scratch);
     bin_rank_kernel<<<1, 256, 0, s>>>(counts_scratch, rank, inv);
     remap_bins_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, ranked_bins, n, rank);
@@ -451,12 +451,7 @@ __device__ __forceinline__ double warp_sum_d(double v) {
 __device__ void entropy_finish(const double* tot, unsigned long long n, int t, const double* qv, int nq_pass,
                                int q_off, int nq_total, int form, double* __restrict__ mi_out,
                                int64_t* __restrict__ nvalid, const OutMap& om) {
-    size_t dst = (size_t)t;
-    if (om.enabled) {  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
-        const int c = t % om.n2, ab = t / om.n2;
-        const int b = ab % om.n1, al = ab / om.n1;
-        dst = ((size_t)c * om.n1 + b) * om.n0 + (size_t)(om.a0 + al);
-    }
+    const size_t dst = om.dst(t);  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
     double* out = mi_out + dst * (1 + nq_total);
     if (nvalid != nullptr) nvalid[dst] = (int64_t)n;
     if (n == 0) {
@@ -713,7 +708,7 @@ cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const
         return cudaGetLastError();
     }
     // wide: rows of every histogram split over about four waves of CTAs
-    int nsplit = (4 * 148 + n_transforms - 1) / n_transforms;
+    int nsplit = (4 * sm_count() + n_transforms - 1) / n_transforms;
     if (nsplit < 1) nsplit = 1;
     if (nsplit > 64) nsplit = 64;
     if (nsplit > nb) nsplit = nb;
@@ -870,7 +865,7 @@ __global__ void __launch_bounds__(256) prebin16_kernel(const float* __restrict__
 cudaError_t launch_prebin16(const float* vol, uint16_t* bins, int64_t n, float lo, float scale, int nb, cudaStream_t s) {
     if (n <= 0) return cudaSuccess;
     int64_t blocks = (n + 255) / 256;
-    if (blocks > 148 * 16) blocks = 148 * 16;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
     prebin16_kernel<<<(unsigned)blocks, 256, 0, s>>>(vol, bins, n, lo, scale, (float)(nb - 1));
     return cudaGetLastError();
 }

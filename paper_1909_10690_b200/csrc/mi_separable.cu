@@ -79,7 +79,8 @@ __global__ void __launch_bounds__(128) xpass_kernel(const VT* __restrict__ src, 
 }
 
 // ---- y-pass -------------------------------------------------------------------------------------
-// grid: (ceil(colpitch/4 / 128), npairs).  pair = a_local*n1 + b.  Every thread owns 4 adjacent
+// grid: (ceil(colpitch/4 / 128), npairs).  pair = a_local*n1 + b_local (n1 = p1 values of the batch,
+// the first one is b0).  Every thread owns 4 adjacent
 // columns of one pair, resolves their x/y samples once and then walks all planes (unrolled by 4 for
 // memory-level parallelism), writing XY[pair][plane][col..col+3] as one 16-byte store per plane, and
 // colvalid[pair][col..col+3].  Trilinear values are stored times `prescale` (1, or the power-of-two
@@ -102,14 +103,14 @@ struct Quad<true, uint8_t> {
 template <bool NN, typename VT>
 __global__ void __launch_bounds__(128) ypass_kernel(const VT* __restrict__ X, int planes, int prows, int mnx,
                                                     int mny, const float2* __restrict__ ax,
-                                                    const float2* __restrict__ ay, int a0, int n1, int fnx,
+                                                    const float2* __restrict__ ay, int a0, int b0, int n1, int fnx,
                                                     int cols, int colpitch, float prescale,
                                                     VT* __restrict__ XY, uint8_t* __restrict__ colvalid) {
     const int col0 = (blockIdx.x * 128 + threadIdx.x) * 4;
     if (col0 >= colpitch) return;
     const int pair = blockIdx.y;
     const int a = pair / n1, b = pair - a * n1;
-    const float2 mx = ax[a0 + a], my = ay[b];
+    const float2 mx = ax[a0 + a], my = ay[b0 + b];
     // per column: offset of X[a][plane 0][sy.lower][ix] (or -1 if the column is invalid) and the y weight
     long long off[4];
     float wy[4];
@@ -305,12 +306,7 @@ __device__ __forceinline__ void zhist_entropy_epilogue(const ZHistArgs& a, long 
     if (threadIdx.x == 0) {
         unsigned long long n = 0;
         for (int w = 0; w < 8; ++w) n += sh_pb[256 + w];
-        size_t dst = (size_t)item;
-        if (a.om.enabled) {  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
-            const long long c = item % a.om.n2, ab = item / a.om.n2;
-            const long long b = ab % a.om.n1, al = ab / a.om.n1;
-            dst = ((size_t)c * a.om.n1 + (size_t)b) * a.om.n0 + (size_t)(a.om.a0 + al);
-        }
+        const size_t dst = a.om.dst(item);  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
         double* out = a.mi_out + dst * (size_t)(1 + a.nq_total);
         if (a.nvalid != nullptr) a.nvalid[dst] = (int64_t)n;
         if (n == 0) {
@@ -561,24 +557,28 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
 // outside the optional fixed-voxel mask (mi_set_fixed_mask) become the dump row as well: the z kernel
 // then counts them where the entropy epilogue and the histogram write-out never look.
 __global__ void __launch_bounds__(256) pitch_bins_kernel(const uint8_t* __restrict__ in,
-                                                         const uint8_t* __restrict__ mask, int cols,
-                                                         int colpitch, int rows_real,
+                                                         const uint32_t* __restrict__ mask_bits, int cols,
+                                                         int colpitch, int fnz, int rows_real,
                                                          uint8_t* __restrict__ out, uint2* __restrict__ rare,
                                                          unsigned* __restrict__ rare_count, unsigned rare_cap) {
     const int col = blockIdx.x * 256 + threadIdx.x;
     if (col >= colpitch) return;
-    const int iz = blockIdx.y;
-    int r = col < cols ? in[(size_t)iz * cols + col] : 0;
-    if (mask != nullptr && col < cols && mask[(size_t)iz * cols + col] == 0) {
-        out[(size_t)iz * colpitch + col] = (uint8_t)rows_real;   // masked-out voxel: counts into the dump row
-        return;
+    for (int iz = blockIdx.y; iz < fnz; iz += gridDim.y) {
+        int r = col < cols ? in[(size_t)iz * cols + col] : 0;
+        if (mask_bits != nullptr && col < cols) {
+            const size_t vi = (size_t)iz * cols + col;
+            if (((mask_bits[vi >> 5] >> (vi & 31u)) & 1u) == 0u) {
+                out[(size_t)iz * colpitch + col] = (uint8_t)rows_real;   // masked-out voxel: counts into the dump row
+                continue;
+            }
+        }
+        if (r >= rows_real) {
+            const unsigned slot = atomicAdd(rare_count, 1u);
+            if (slot < rare_cap) rare[slot] = make_uint2((unsigned)col, (unsigned)iz | ((unsigned)r << 16));
+            r = rows_real;
+        }
+        out[(size_t)iz * colpitch + col] = (uint8_t)r;
     }
-    if (r >= rows_real) {
-        const unsigned slot = atomicAdd(rare_count, 1u);
-        if (slot < rare_cap) rare[slot] = make_uint2((unsigned)col, (unsigned)iz | ((unsigned)r << 16));
-        r = rows_real;
-    }
-    out[(size_t)iz * colpitch + col] = (uint8_t)r;
 }
 
 // CANON-5 on the integer side: PTX float->int conversions saturate to the destination range
@@ -622,10 +622,10 @@ __global__ void __launch_bounds__(256) zrare_kernel(const __grid_constant__ ZHis
 
 }  // namespace
 
-cudaError_t launch_pitch_bins(const uint8_t* in, const uint8_t* mask, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
+cudaError_t launch_pitch_bins(const uint8_t* in, const uint32_t* mask_bits, int cols, int colpitch, int fnz, int rows_real, uint8_t* out,
                               uint2* rare, unsigned* rare_count, unsigned rare_cap, cudaStream_t s) {
-    dim3 grid((colpitch + 255) / 256, fnz);
-    pitch_bins_kernel<<<grid, 256, 0, s>>>(in, mask, cols, colpitch, rows_real, out, rare, rare_count, rare_cap);
+    dim3 grid((colpitch + 255) / 256, fnz < 65535 ? fnz : 65535);
+    pitch_bins_kernel<<<grid, 256, 0, s>>>(in, mask_bits, cols, colpitch, fnz, rows_real, out, rare, rare_count, rare_cap);
     return cudaGetLastError();
 }
 
@@ -642,16 +642,16 @@ cudaError_t launch_xpass(bool nn, const void* src, int snx, int srows, int mnx, 
 }
 
 cudaError_t launch_ypass(bool nn, const void* X, int planes, int prows, int mnx, int mny, const float2* ax,
-                         const float2* ay, int a0, int n1, int npairs, int fnx, int cols, int colpitch,
+                         const float2* ay, int a0, int b0, int nb1, int npairs, int fnx, int cols, int colpitch,
                          float prescale, void* XY, uint8_t* colvalid, cudaStream_t s) {
     dim3 grid((colpitch / 4 + 127) / 128, npairs);
     if (nn)
         ypass_kernel<true, uint8_t><<<grid, 128, 0, s>>>(static_cast<const uint8_t*>(X), planes, prows, mnx, mny, ax,
-                                                        ay, a0, n1, fnx, cols, colpitch, 1.0f,
+                                                        ay, a0, b0, nb1, fnx, cols, colpitch, 1.0f,
                                                         static_cast<uint8_t*>(XY), colvalid);
     else
         ypass_kernel<false, float><<<grid, 128, 0, s>>>(static_cast<const float*>(X), planes, prows, mnx, mny, ax, ay,
-                                                       a0, n1, fnx, cols, colpitch, prescale, static_cast<float*>(XY),
+                                                       a0, b0, nb1, fnx, cols, colpitch, prescale, static_cast<float*>(XY),
                                                        colvalid);
     return cudaGetLastError();
 }

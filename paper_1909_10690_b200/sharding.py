@@ -2,10 +2,11 @@
 
 Every map voxel is a separate MI evaluation, so the path shards by TRANSFORMS with no
 exchange inside it: each rank owns a contiguous slab of the slowest grid axis (p2), holds both
-volumes (<= 105 MB, replicated) in its own context, maps its slab with `mi_map`, and the slabs are
-concatenated with one all-gather of doubles (<= 551 KB at C5).  This module holds host logic only
-(grid arithmetic + torch.distributed calls); it never touches the method's arithmetic, so it can be
-exercised with the gloo backend on CPU by passing any `map_fn`.
+volumes (<= 105 MB, replicated) in its own context, maps its slab with `mi_map_range` -- whose node
+parameters are those of the WHOLE grid, so the sharded map equals the single-GPU map bit for bit --
+and the slabs are concatenated with one all-gather of doubles (<= 551 KB at C5).  This module holds
+host logic only (index arithmetic + torch.distributed calls); it never touches the method's
+arithmetic, so it can be exercised with the gloo backend on CPU by passing any `map_fn`.
 """
 from __future__ import annotations
 
@@ -28,40 +29,37 @@ def slab_bounds(n2: int, rank: int, world: int):
     return begin, begin + base + (1 if rank < rem else 0)
 
 
-def shard_grid(lo, hi, n, rank: int, world: int):
-    """Sub-grid (lo', hi', n') of the rank's p2 slab, or None if the slab is empty.
-
-    The slab's end points are taken from the FULL grid's axis values, so every rank evaluates
-    exactly the nodes the single-GPU map would (bit-identical parameters for k_begin and k_end-1;
-    interior nodes are re-derived by mi_map from (lo', hi', n') and agree to the last ulp or two of
-    the parameter -- callers that need bit-identical interior nodes use one p2 plane per call)."""
-    lo = [float(v) for v in lo]
-    hi = [float(v) for v in hi]
+def slab_range(n, rank: int, world: int):
+    """Node range (begin[3], end[3]) of the rank's p2 slab on the grid of n nodes, or None if the slab
+    is empty (more ranks than p2 planes).  These are the `begin`, `end` arguments of mi_map_range."""
     n = [int(v) for v in n]
     b, e = slab_bounds(n[2], rank, world)
     if e <= b:
         return None
-    vals = axis_values(lo[2], hi[2], n[2])
-    return (lo[0], lo[1], float(vals[b])), (hi[0], hi[1], float(vals[e - 1])), (n[0], n[1], e - b)
+    return (0, 0, b), (n[0], n[1], e)
 
 
-def map_sharded(map_fn, lo, hi, n, nch: int, rank: int, world: int, dist=None, device=None):
-    """Run `map_fn(lo', hi', n') -> array (nch, n2', n1, n0)` on this rank's slab and return the full
-    (nch, n2, n1, n0) float64 map on every rank plus the per-channel arg max (ties -> lowest index).
+def map_sharded(map_fn, n, nch: int, rank: int, world: int, dist=None, device=None):
+    """Run `map_fn(begin, end) -> array (nch, end[2]-begin[2], n1, n0)` on this rank's slab (the GPU
+    path passes a closure over mi_map_range) and return the full (nch, n2, n1, n0) float64 map on
+    every rank plus the per-channel arg max (ties -> lowest index).
 
-    `dist` is `torch.distributed` (already initialised) or None for world == 1."""
+    `dist` is `torch.distributed` (already initialised); it may be None only for world == 1."""
     import torch
 
+    if world > 1 and dist is None:
+        raise ValueError("map_sharded: world = %d needs an initialised torch.distributed" % world)
     n = [int(v) for v in n]
-    sub = shard_grid(lo, hi, n, rank, world)
+    sub = slab_range(n, rank, world)
     plane = n[1] * n[0]
     base = (n[2] + world - 1) // world           # padded slab depth so all_gather sees equal shapes
     local = torch.zeros((nch, base, n[1], n[0]), dtype=torch.float64, device=device)
     if sub is not None:
+        depth = sub[1][2] - sub[0][2]
         m = map_fn(*sub)
         m = m if isinstance(m, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(m))
-        local[:, : sub[2][2]] = m.to(local.device).reshape(nch, sub[2][2], n[1], n[0])
-    if world == 1 or dist is None:
+        local[:, :depth] = m.to(local.device).reshape(nch, depth, n[1], n[0])
+    if world == 1:
         parts = [local]
     else:
         parts = [torch.empty_like(local) for _ in range(world)]
@@ -111,6 +109,8 @@ def batch_sharded(eval_fn, n: int, nch: int, rank: int, world: int, dist=None, d
     this rank's share; returns the (n, nch) float64 result on every rank (one all-gather of doubles)."""
     import torch
 
+    if world > 1 and dist is None:
+        raise ValueError("batch_sharded: world = %d needs an initialised torch.distributed" % world)
     b, e = batch_bounds(n, rank, world)
     base = (int(n) + world - 1) // world
     local = torch.zeros((base, nch), dtype=torch.float64, device=device)
@@ -118,7 +118,7 @@ def batch_sharded(eval_fn, n: int, nch: int, rank: int, world: int, dist=None, d
         v = eval_fn(b, e)
         v = v if isinstance(v, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(v, dtype=np.float64))
         local[: e - b] = v.to(local.device).reshape(e - b, nch)
-    if world == 1 or dist is None:
+    if world == 1:
         parts = [local]
     else:
         parts = [torch.empty_like(local) for _ in range(world)]

@@ -50,6 +50,13 @@ def test_binding_never_imports_the_oracle():
                 "paper_1909_10690_b200/csrc", ""), fn
 
 
+def test_library_reads_no_environment_variable():
+    """Kernel selection is a function of the C-ABI arguments and mi_set_option only."""
+    for fn in os.listdir(os.path.join(ROOT, "paper_1909_10690_b200", "csrc")):
+        assert "getenv" not in open(os.path.join(ROOT, "paper_1909_10690_b200", "csrc", fn)).read(), fn
+    assert "environ" not in open(os.path.join(ROOT, "paper_1909_10690_b200", "binding.py")).read()
+
+
 def test_index_affine_bit_for_bit_against_oracle(lib):
     rng = np.random.default_rng(0)
     geoms = [((260, 311, 260), (0.7, 0.7, 0.7), (182, 218, 182), (1.0, 1.0, 1.0)),

@@ -86,8 +86,9 @@ def test_c2_small_128_bins(mi):
 
 
 def test_256_bins_ragged_anisotropic_multimodal(mi):
-    """C5-shaped at 1/4 resolution: different dims and spacings, 256 bins (packed 16-bit path),
-    sizes that span several tiles with ragged rows (65 = 2*32 + 1)."""
+    """C5-shaped at 1/4 resolution: different dims and spacings, 256 bins (191 ranked rows of u32 counters in
+    shared memory, the rarer rows through global atomics), sizes that span several tiles with ragged rows
+    (65 = 2*32 + 1)."""
     cfg = ph.get_config("C5", res=0.25, grid_n=3)
     rng = np.random.default_rng(3)
     T = np.concatenate([rand_physical(rng, 5, shift=8.0),
@@ -105,9 +106,9 @@ def test_many_transforms_one_cta_each_and_two_q_passes(mi):
     check_batch(mi, fixed, moving, (1, 1, 1), (1.1, 0.9, 1.0), 32, T, q)
 
 
-def test_packed_counter_drain_and_hot_bin(mi):
-    """Constant images put every voxel in ONE bin: exercises the 2^15 drain of the packed 16-bit
-    counters (256 bins) and, for bin (0,0), the private hot-bin counter."""
+def test_single_hot_bin_all_lanes_one_counter(mi):
+    """Constant images put every voxel in ONE bin: all 32 lanes of every warp hit the same u32 shared
+    counter (one RED per warp after the hardware's same-address merge), up to 163840 counts in one cell."""
     n = (64, 64, 40)
     ident = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)[None]
     for fv, mv in [(0.3, 0.7), (0.0, 0.0), (0.0, 0.5)]:
@@ -121,7 +122,7 @@ def test_packed_counter_drain_and_hot_bin(mi):
                     a, b = min(int(fv * nb), nb - 1), min(int(mv * nb), nb - 1)
                     assert hist[0, a, b] == fixed.size and hist.sum() == fixed.size
                     assert np.all(np.abs(vals) < 1e-9)
-    # half the volume in one bin, the rest random: drain + ordinary traffic together
+    # half the volume in one bin, the rest random: the hot counter and ordinary traffic together
     fixed = ph.random_volume(n, 7); fixed[:20] = 0.25
     moving = ph.random_volume(n, 8); moving[:20] = 0.75
     check_batch(mi, fixed, moving, (1, 1, 1), (1, 1, 1), 256, ident, (2.0,))
@@ -258,61 +259,192 @@ def test_c5_reduced_map(mi):
     check_map(mi, ph.get_config("C5", res=0.25, grid_n=5), 0)
 
 
-def test_c5_full_size_sampled_against_oracle(mi):
-    """BASELINE.json's full 260x311x260 / 182x218x182, 256-bin pair in the configuration bench.py
-    times; sampled transforms of the 41^3 grid are checked one by one against the oracle."""
-    cfg = ph.get_config("C5")
-    assert cfg.fixed.shape == (260, 311, 260) and cfg.moving.shape == (182, 218, 182)
-    nodes = [(0, 0, 0), (40, 40, 40), (26, 11, 22), (27, 10, 23), (13, 35, 7), (20, 20, 20)]
-    step = 20.0 / 40
-    T = np.stack([orc.family_matrix(0, [-10 + k * step for k in node]) for node in nodes])
+def node_param(cfg, node):
+    return [cfg.lo[d] if cfg.n[d] == 1 else cfg.lo[d] + node[d] * (cfg.hi[d] - cfg.lo[d]) / (cfg.n[d] - 1) for d in range(3)]
+
+
+def oracle_nodes(cfg, nodes, interp, q=None, want_hist=False):
+    """The oracle at grid nodes (k0, k1, k2) of cfg's map, one transform each."""
     fd, md = cfg.fixed.shape[::-1], cfg.moving.shape[::-1]
-    M = orc.physical_to_index(T, fd, cfg.fixed_spacing, md, cfg.moving_spacing)
+    M = orc.grid_nodes_index_affines(fd, cfg.fixed_spacing, md, cfg.moving_spacing, cfg.family, cfg.lo, cfg.hi, cfg.n, nodes)
+    return orc.eval_batch(cfg.fixed, cfg.moving, M, cfg.nbins, *cfg.ranges, interp, q=cfg.q if q is None else q,
+                          want_hist=want_hist)
+
+
+def test_c5_full_size_subset_rule_values_and_argmax(mi):
+    """BASELINE.json configs[4] at full size in the launch configuration bench.py times (one mi_map of the 41^3
+    grid through the separable kernels with the fused entropy epilogue), checked by SURVEY 8(d)'s subset
+    rule: every 4th node per axis (11^3 = 1331 nodes) plus the 5^3 neighbourhoods of the GPU arg max and of
+    the ground truth, value by value at 1e-4 nats; the oracle's maximum over everything it computed must be
+    the GPU's arg max node ("argmax identical" where the oracle can afford to look).  About 35 s of oracle
+    time on 16 host cores."""
+    cfg = ph.get_config("C5")
+    assert cfg.fixed.shape == (260, 311, 260) and cfg.moving.shape == (182, 218, 182) and cfg.n == (41, 41, 41)
     with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
-        for interp in (0, 1):
-            ref = orc.eval_batch(cfg.fixed, cfg.moving, M, 256, 0, 1, 0, 1, interp, q=(0.5,), want_hist=True)
-            vals, hist, nvalid = mi.mi_eval_batch(ctx, T, (0.5,), interp, hist_out=True, nvalid_out=True)
-            moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
-            if interp == 0:
-                assert np.array_equal(hist, ref["hist"]) and np.array_equal(nvalid, ref["nvalid"])
-            else:
-                assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
-            assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
-        # the call bench.py times: the whole 41^3 map through the separable kernels with the entropy
-        # epilogue; its values at the sampled nodes against the oracle's trilinear Shannon values
         m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
-        for node, want in zip(nodes, ref["mi"][:, 0]):
-            assert abs(m[0, node[2], node[1], node[0]] - want) <= MI_TOL, node
-        assert m[0].reshape(-1)[am[0]] == m[0].max() and am[0] == int(np.argmax(m[0]))
-        k2, k1, k0 = np.unravel_index(am[0], m.shape[1:])
-        p = [-10 + k * step for k in (k0, k1, k2)]
-        assert max(abs(p[d] - cfg.truth[d]) for d in range(3)) <= step        # P11 at full size
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1 and mi.mi_get_option(ctx, mi.MI_INFO_RARE_VOXELS) == 0
+    assert am[0] == int(np.argmax(m[0]))
+    g = tuple(int(v) for v in np.unravel_index(am[0], m.shape[1:]))[::-1]           # (k0, k1, k2)
+    step = 20.0 / 40
+    truth = tuple(int(round((cfg.truth[d] + 10.0) / step)) for d in range(3))        # nearest node to (3.2,-4.7,1.1)
+    nodes = {(k0, k1, k2) for k2 in range(0, 41, 4) for k1 in range(0, 41, 4) for k0 in range(0, 41, 4)}
+    for c in (g, truth):
+        nodes |= {(k0, k1, k2) for k2 in range(max(c[2] - 2, 0), min(c[2] + 3, 41))
+                  for k1 in range(max(c[1] - 2, 0), min(c[1] + 3, 41)) for k0 in range(max(c[0] - 2, 0), min(c[0] + 3, 41))}
+    nodes = sorted(nodes)
+    ref = oracle_nodes(cfg, nodes, 1)["mi"][:, 0]
+    got = np.array([m[0, k2, k1, k0] for k0, k1, k2 in nodes])
+    assert np.max(np.abs(got - ref)) <= MI_TOL, np.max(np.abs(got - ref))
+    assert nodes[int(np.argmax(ref))] == g, (nodes[int(np.argmax(ref))], g)
+    assert max(abs(node_param(cfg, g)[d] - cfg.truth[d]) for d in range(3)) <= step  # P11 at full size
+
+
+def test_c5_full_size_histograms_of_the_z_kernel(mi):
+    """zhist_kernel's joint histograms at the full C5 size against the oracle: a 2x2x2 sub-box of the 41^3 grid
+    around the ground truth and one at the grid corner (partial overlap), through mi_map_range with hist_out
+    (separable kernels, histogram written out): nearest neighbour bit-exact, trilinear within 1e-5 of the
+    voxels; the fused-epilogue values of the same nodes within 1e-4 nats."""
+    cfg = ph.get_config("C5")
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
+        for begin in ((26, 10, 22), (0, 39, 0)):
+            end = tuple(b + 2 for b in begin)
+            nodes = [(k0, k1, k2) for k2 in range(begin[2], end[2]) for k1 in range(begin[1], end[1])
+                     for k0 in range(begin[0], end[0])]
+            for interp in (0, 1):
+                ref = oracle_nodes(cfg, nodes, interp, q=(0.5,), want_hist=True)
+                sub, am, hist = mi.mi_map_range(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, begin, end, (0.5,), interp, hist_out=True)
+                assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1
+                if interp == 0:
+                    assert np.array_equal(hist, ref["hist"])
+                else:
+                    moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
+                    assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
+                assert np.array_equal(hist.sum(axis=(1, 2)), ref["nvalid"])
+                assert np.max(np.abs(sub.reshape(2, -1).T - ref["mi"])) <= MI_TOL
+                fused, _, _ = mi.mi_map_range(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, begin, end, (0.5,), interp)
+                assert np.max(np.abs(fused - sub)) <= 1e-9
 
 
 @pytest.mark.parametrize("name", ["C3", "C4"])
-def test_c3_c4_full_size_maps_sampled_against_oracle(mi, name):
-    """The full-size rotation (generic kernel) and scale (separable kernels, five Tsallis orders) maps of
-    BASELINE.json; sampled grid nodes are checked one by one against the oracle."""
+def test_c3_c4_full_size_full_maps_against_oracle(mi, name):
+    """BASELINE.json configs[2] and [3] IN FULL at 260x311x260: every value of the 15^3 Euler-rotation map
+    (3375 transforms through the generic kernel) and of the 11^3 scale map x 6 channels (separable kernels,
+    five Tsallis orders in the fused epilogue) against the oracle at 1e-4 nats, and every channel's arg max
+    identical.  Oracle time on 16 host cores: about 150 s (C3) and 60 s (C4)."""
     cfg = ph.get_config(name)
     assert cfg.fixed.shape == (260, 311, 260)
-    n = cfg.n
-    nodes = [(0, 0, 0), (n[0] - 1, n[1] - 1, n[2] - 1), (n[0] // 2, n[1] // 2, n[2] // 2), (n[0] - 2, 1, n[2] // 3)]
-    par = lambda node: [cfg.lo[d] + node[d] * (cfg.hi[d] - cfg.lo[d]) / (n[d] - 1) for d in range(3)]
-    T = np.stack([orc.family_matrix(cfg.family, par(node)) for node in nodes])
-    fd, md = cfg.fixed.shape[::-1], cfg.moving.shape[::-1]
-    M = orc.physical_to_index(T, fd, cfg.fixed_spacing, md, cfg.moving_spacing)
-    ref = orc.eval_batch(cfg.fixed, cfg.moving, M, cfg.nbins, *cfg.ranges, 1, q=cfg.q)
-    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
-        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
-    for node, want in zip(nodes, ref["mi"]):
-        got = m[:, node[2], node[1], node[0]]
-        assert np.max(np.abs(got - want)) <= MI_TOL, (node, got, want)
-    for ch in range(m.shape[0]):
-        assert am[ch] == int(np.argmax(m[ch]))
+    m, am = check_map(mi, cfg, 1)
     k2, k1, k0 = np.unravel_index(am[0], m.shape[1:])
-    p = par((k0, k1, k2))
-    steps = [(cfg.hi[d] - cfg.lo[d]) / (n[d] - 1) for d in range(3)]
+    p = node_param(cfg, (k0, k1, k2))
+    steps = [(cfg.hi[d] - cfg.lo[d]) / (cfg.n[d] - 1) for d in range(3)]
     assert all(abs(p[d] - cfg.truth[d]) <= steps[d] * 1.0001 for d in range(3)), (p, cfg.truth)   # P11 (Shannon)
+
+
+def test_c3_full_size_generic_kernel_histograms(mi):
+    """The generic kernel's histograms at the full C3 size (rotations): three grid nodes, nearest neighbour
+    bit-exact and trilinear within 1e-5 of the voxels."""
+    cfg = ph.get_config("C3")
+    nodes = [(0, 0, 0), (11, 4, 9), (14, 14, 14)]
+    T = np.stack([orc.family_matrix(cfg.family, node_param(cfg, node)) for node in nodes])
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
+        for interp in (0, 1):
+            ref = oracle_nodes(cfg, nodes, interp, q=(2.0,), want_hist=True)
+            vals, hist, nvalid = mi.mi_eval_batch(ctx, T, (2.0,), interp, hist_out=True, nvalid_out=True)
+            if interp == 0:
+                assert np.array_equal(hist, ref["hist"]) and np.array_equal(nvalid, ref["nvalid"])
+            else:
+                moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
+                assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
+            assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
+
+
+def test_map_range_slabs_equal_the_full_map_bitwise(mi):
+    """mi_map_range: slabs of a grid whose step is not representable (7 nodes over +-1) are bit-identical to the
+    same nodes of mi_map, on the separable path, the generic path (rotations) and with histograms; two
+    emulated ranks of sharding.map_sharded reassemble the single-GPU map bit for bit."""
+    from paper_1909_10690_b200 import sharding as sh
+    c5 = ph.get_config("C5", res=0.25, grid_n=7)
+    c3 = ph.get_config("C3", res=0.25, grid_n=7)
+    for cfg, lo, hi, q in ((c5, (-1.0,) * 3, (1.0,) * 3, (0.5,)), (c3, (-1.0,) * 3, (1.0,) * 3, ())):
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+            for interp in (0, 1):
+                full, am = mi.mi_map(ctx, cfg.family, lo, hi, cfg.n, q, interp)
+                parts = []
+                for rank in range(3):
+                    begin, end = sh.slab_range(cfg.n, rank, 3)
+                    sub, sam, _ = mi.mi_map_range(ctx, cfg.family, lo, hi, cfg.n, begin, end, q, interp)
+                    assert np.array_equal(sub, full[:, begin[2]:end[2]])
+                    assert sam[0] == int(np.argmax(sub[0]))
+                    parts.append(sub)
+                assert np.array_equal(np.concatenate(parts, axis=1), full)
+                # a box inside the grid, with histograms: same values, histograms = those of mi_eval_batch
+                begin, end = (2, 3, 1), (4, 6, 3)
+                sub, _, hist = mi.mi_map_range(ctx, cfg.family, lo, hi, cfg.n, begin, end, q, interp, hist_out=True)
+                assert np.array_equal(sub, full[:, 1:3, 3:6, 2:4]) or np.max(np.abs(sub - full[:, 1:3, 3:6, 2:4])) <= 1e-9
+                nodes = [(k0, k1, k2) for k2 in range(1, 3) for k1 in range(3, 6) for k0 in range(2, 4)]
+                T = np.stack([orc.family_matrix(cfg.family, [lo[d] + node[d] * (hi[d] - lo[d]) / 6 for d in range(3)])
+                              for node in nodes])
+                _, h2, _ = mi.mi_eval_batch(ctx, T, q, interp, hist_out=True)
+                assert np.array_equal(hist, h2)
+            with pytest.raises(mi.MIError):
+                mi.mi_map_range(ctx, cfg.family, lo, hi, cfg.n, (0, 0, 0), (8, 7, 7), q, 1)
+            with pytest.raises(mi.MIError):
+                mi.mi_map_range(ctx, cfg.family, lo, hi, cfg.n, (3, 0, 0), (3, 7, 7), q, 1)
+    # map_sharded with world = 1 through mi_map_range
+    cfg = c5
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        full, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, (0.5,), 1)
+        got, gam = sh.map_sharded(lambda b, e: mi.mi_map_range(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, b, e, (0.5,), 1)[0],
+                                  cfg.n, 2, 0, 1)
+        assert np.array_equal(got.numpy(), full) and np.array_equal(gam.numpy(), am)
+
+
+def test_separable_scratch_smaller_than_one_slab(mi):
+    """a p0 slab that exceeds the scratch budgets is split into chunks of p1; when even one (p0,p1)
+    pair does not fit, the map takes the generic kernel instead of failing."""
+    cfg = ph.get_config("C5", res=0.25, grid_n=5)
+    ref, aref = gpu_map(mi, cfg, 1, SEPARABLE=0)
+    planes_mb = (cfg.moving.shape[0] + 2) * 5120 * 4 / 2 ** 20        # one pair's xy planes: 48 planes x colpitch 5120 floats
+    assert 0.5 < planes_mb < 1.5
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        set_options(mi, ctx, XY_BUDGET_MB=3)                          # 3 pairs < one slab of 5
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1
+        assert np.max(np.abs(m - ref)) <= 1e-9 and np.array_equal(am, aref)
+        set_options(mi, ctx, XY_BUDGET_MB=12288, FUSE_ENTROPY=0, SEP_HIST_BUDGET_MB=3)   # 5 x 256 KB per pair: 2 pairs
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1
+        assert np.array_equal(m, ref) and np.array_equal(am, aref)
+        set_options(mi, ctx, XY_BUDGET_MB=0)                          # nothing fits: generic kernel, not an error
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 0
+        assert np.array_equal(m, ref) and np.array_equal(am, aref)
+        with pytest.raises(mi.MIError):
+            mi.mi_set_option(ctx, mi.MI_OPT_ZHIST_PAD, 0)
+        with pytest.raises(mi.MIError):
+            mi.mi_set_option(ctx, mi.MI_INFO_NUM_SMS, 1)              # read-only
+        assert mi.mi_get_option(ctx, mi.MI_INFO_NUM_SMS) >= 1
+
+
+def test_tsallis_orders_at_the_ends_of_the_accepted_range(mi):
+    """q = 32 (the documented upper bound: sum c^q over counts up to 2^31 stays inside the double range) and
+    q = 0.01 against the oracle's pow(c/N, q), at a size where one bin holds millions of voxels; q above the
+    bound is refused."""
+    cfg = ph.get_config("C5", res=0.5, grid_n=3)
+    q = (0.01, 32.0)
+    nodes = [(0, 0, 0), (1, 1, 1), (2, 0, 1)]
+    ref = oracle_nodes(cfg, nodes, 1, q=q)["mi"]
+    T = np.stack([orc.family_matrix(cfg.family, node_param(cfg, node)) for node in nodes])
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        vals = mi.mi_eval_batch(ctx, T, q, 1)[0]
+        assert np.all(np.isfinite(vals)) and np.max(np.abs(vals - ref)) <= MI_TOL
+        m, _ = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, q, 1)               # fused epilogue
+        got = np.array([m[:, k2, k1, k0] for k0, k1, k2 in nodes])
+        assert np.max(np.abs(got - ref)) <= MI_TOL
+        for bad in (32.5, 1e6):
+            with pytest.raises(mi.MIError) as ei:
+                mi.mi_eval_batch(ctx, T, (bad,), 1)
+            assert ei.value.status == mi.MI_ERR_INVALID_ARG
 
 
 def test_wide_histograms_above_256_bins(mi):
@@ -396,12 +528,18 @@ def test_fixed_voxel_mask_all_paths(mi):
             mi.mi_set_fixed_mask(ctx, None)
             assert np.array_equal(mi.mi_eval_batch(ctx, T, (0.5,), 1)[0], full)
     # few shared rows: masked voxels and rare-row voxels together
-    with env(MI_B200_ZROWS=40):
+    rm = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, 256, 0, 1, 0, 1, cfg.family,
+                    cfg.lo, cfg.hi, cfg.n, q=(), interp=1, mask=mask)
+    for order in (0, 1):          # the option before the mask, and the mask before the option
         with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
+            if order == 0:
+                mi.mi_set_option(ctx, mi.MI_OPT_ZHIST_ROWS_MAX, 40)
             mi.mi_set_fixed_mask(ctx, mask)
-            rm = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, 256, 0, 1, 0, 1, cfg.family,
-                            cfg.lo, cfg.hi, cfg.n, q=(), interp=1, mask=mask)
+            if order == 1:
+                mi.mi_set_option(ctx, mi.MI_OPT_ZHIST_ROWS_MAX, 40)
+            assert mi.mi_get_option(ctx, mi.MI_INFO_ZHIST_ROWS) == 39 and mi.mi_get_option(ctx, mi.MI_INFO_RARE_VOXELS) > 0
             m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, (), 1)
+            assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1
             assert np.max(np.abs(m - rm["map"])) <= MI_TOL and np.array_equal(am, rm["argmax"])
 
 
@@ -428,29 +566,16 @@ def test_context_cycles_reuse_the_pool_and_release(mi):
 
 
 # ------------------------------------------------------------------------------------------------ separable path
-class env:
-    """Set MI_B200_* knobs (read by mi_create) for the duration of a with-block."""
-    def __init__(self, **kw):
-        self.kw = {k: str(v) for k, v in kw.items()}
-
-    def __enter__(self):
-        import os
-        self.old = {k: os.environ.get(k) for k in self.kw}
-        os.environ.update(self.kw)
-
-    def __exit__(self, *exc):
-        import os
-        for k, v in self.old.items():
-            if v is None:
-                os.environ.pop(k, None)
-            else:
-                os.environ[k] = v
+def set_options(mi, ctx, **opts):
+    """mi_set_option for every keyword: SEPARABLE=0 -> MI_OPT_SEPARABLE = 0, ..."""
+    for k, v in opts.items():
+        mi.mi_set_option(ctx, getattr(mi, "MI_OPT_" + k), v)
 
 
-def gpu_map(mi, cfg, interp, **knobs):
-    with env(**knobs):
-        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins, cfg.ranges) as ctx:
-            return mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, interp)
+def gpu_map(mi, cfg, interp, **opts):
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins, cfg.ranges) as ctx:
+        set_options(mi, ctx, **opts)
+        return mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, interp)
 
 
 @pytest.mark.parametrize("name,kw", [("C1", {}), ("C5", dict(res=0.25, grid_n=5)), ("C4", dict(res=0.25, grid_n=4)),
@@ -461,11 +586,11 @@ def test_separable_path_equals_generic_path_bitwise(mi, name, kw):
     IDENTICAL doubles: the entropy kernel is deterministic, so equal maps <=> equal histograms."""
     cfg = ph.get_config(name, **kw)
     for interp in (0, 1):
-        mg, amg = gpu_map(mi, cfg, interp, MI_B200_SEPARABLE=0)
+        mg, amg = gpu_map(mi, cfg, interp, SEPARABLE=0)
         # histograms written out and reduced by the same entropy kernel as the generic path; every
         # moving-side binning variant of the z kernel (general / no clamps / pre-scaled planes)
         for mode in (0, 1, 2):
-            ms, ams = gpu_map(mi, cfg, interp, MI_B200_FUSE_ENTROPY=0, MI_B200_BIN_MODE=mode)
+            ms, ams = gpu_map(mi, cfg, interp, FUSE_ENTROPY=0, BIN_MODE_MAX=mode)
             assert np.array_equal(ms, mg), (mode, np.max(np.abs(ms - mg)))
             assert np.array_equal(ams, amg)
         # default: entropies computed in the z kernel's epilogue (another summation order)
@@ -476,16 +601,16 @@ def test_separable_path_equals_generic_path_bitwise(mi, name, kw):
 
 def test_separable_batches_rare_rows_and_odd_grids(mi):
     cfg = ph.get_config("C5", res=0.25, grid_n=5)
-    ref, _ = gpu_map(mi, cfg, 1, MI_B200_SEPARABLE=0)
+    ref, _ = gpu_map(mi, cfg, 1, SEPARABLE=0)
     # tiny scratch budgets: one p0 per batch, several batches
-    m, _ = gpu_map(mi, cfg, 1, MI_B200_XY_BUDGET_MB=8, MI_B200_SEP_HIST_BUDGET_MB=8, MI_B200_FUSE_ENTROPY=0)
+    m, _ = gpu_map(mi, cfg, 1, XY_BUDGET_MB=8, SEP_HIST_BUDGET_MB=8, FUSE_ENTROPY=0)
     assert np.array_equal(m, ref)
-    m, _ = gpu_map(mi, cfg, 1, MI_B200_XY_BUDGET_MB=8)
+    m, _ = gpu_map(mi, cfg, 1, XY_BUDGET_MB=8)
     assert np.max(np.abs(m - ref)) <= 1e-9
     # only 40 of 256 fixed-bin rows in shared memory: most voxels go through the rare-voxel kernel
     for interp in (0, 1):
-        ref, _ = gpu_map(mi, cfg, interp, MI_B200_SEPARABLE=0)
-        m, _ = gpu_map(mi, cfg, interp, MI_B200_ZROWS=40)
+        ref, _ = gpu_map(mi, cfg, interp, SEPARABLE=0)
+        m, _ = gpu_map(mi, cfg, interp, ZHIST_ROWS_MAX=40)
         assert np.array_equal(m, ref)
     # random volumes fill all 256 bins: the rare tail exists at the natural row count too; ragged
     # non-cubic grid (n = 3 x 1 x 4), anisotropic spacing
@@ -496,7 +621,7 @@ def test_separable_batches_rare_rows_and_odd_grids(mi):
     for interp in (0, 1):
         check_map(mi, c, interp)
         ms, _ = gpu_map(mi, c, interp)
-        mg, _ = gpu_map(mi, c, interp, MI_B200_SEPARABLE=0)
+        mg, _ = gpu_map(mi, c, interp, SEPARABLE=0)
         assert np.array_equal(ms, mg)
 
 
@@ -519,8 +644,8 @@ def test_separable_binning_variants_and_range_edges(mi):
                       (3, 1, 3), q, (0, 0, 0), ranges)
         for interp in (0, 1):
             check_map(mi, c, interp)
-            ms, _ = gpu_map(mi, c, interp, MI_B200_FUSE_ENTROPY=0)
-            mg, _ = gpu_map(mi, c, interp, MI_B200_SEPARABLE=0)
+            ms, _ = gpu_map(mi, c, interp, FUSE_ENTROPY=0)
+            mg, _ = gpu_map(mi, c, interp, SEPARABLE=0)
             assert np.array_equal(ms, mg)
 
 

@@ -413,3 +413,15 @@ def test_eval_batch_matches_single_calls():
         h, nv = orc.joint_hist(cfg.fixed, cfg.moving, Ms[k], 64, 0, 1, 0, 1, 1)
         assert np.array_equal(r["hist"][k], h) and r["nvalid"][k] == nv
         assert np.array_equal(r["mi"][k], orc.entropies(h, [0.5]))
+
+
+def test_map_range_helper_equals_orc_map():
+    """oracle.mi_map_range (grid formula + family generator + CANON-1 per node, in Python around the C++
+    calls) over the whole node range reproduces orc_map bit for bit on a grid with a non-representable step,
+    and a sub-box is the corresponding slice."""
+    cfg = ph.config_c1(grid_n=4)
+    lo, hi = (-1.0, -0.7, 0.1), (1.0, 1.3, 0.9)
+    args = (cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, 0, 1, 0, 1, cfg.family, lo, hi, cfg.n)
+    full = orc.mi_map(*args, q=(0.5,))["map"]
+    assert np.array_equal(orc.mi_map_range(*args, (0, 0, 0), cfg.n, q=(0.5,)), full)
+    assert np.array_equal(orc.mi_map_range(*args, (1, 0, 2), (3, 4, 4), q=(0.5,)), full[:, 2:4, 0:4, 1:3])

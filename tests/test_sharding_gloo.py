@@ -29,18 +29,20 @@ def test_slab_bounds_cover_the_axis_exactly():
         sh.slab_bounds(4, 2, 2)
 
 
-def test_shard_grid_end_points_are_the_full_grids_nodes():
-    lo, hi, n = (-10, -10, -10), (10, 10, 10), (41, 41, 41)
-    vals = sh.axis_values(-10, 10, 41)
-    got = []
+def test_slab_range_is_a_node_range_of_the_whole_grid():
+    n = (41, 41, 41)
+    seen = []
     for r in range(4):
-        slo, shi, sn = sh.shard_grid(lo, hi, n, r, 4)
-        assert slo[:2] == (-10.0, -10.0) and shi[:2] == (10.0, 10.0) and sn[:2] == (41, 41)
-        b, e = sh.slab_bounds(41, r, 4)
-        assert slo[2] == vals[b] and shi[2] == vals[e - 1] and sn[2] == e - b
-        got += list(sh.axis_values(slo[2], shi[2], sn[2]))
-    assert np.allclose(got, vals, rtol=0, atol=1e-12)
-    assert sh.shard_grid(lo, hi, (3, 3, 1), 1, 2) is None          # more ranks than planes
+        begin, end = sh.slab_range(n, r, 4)
+        assert begin[:2] == (0, 0) and end[:2] == (41, 41)
+        assert (begin[2], end[2]) == sh.slab_bounds(41, r, 4)
+        seen += list(range(begin[2], end[2]))
+    assert seen == list(range(41))
+    assert sh.slab_range((3, 3, 1), 1, 2) is None                  # more ranks than planes
+    with pytest.raises(ValueError):
+        sh.map_sharded(lambda b, e: None, n, 1, 0, 2, dist=None)    # world > 1 needs torch.distributed
+    with pytest.raises(ValueError):
+        sh.batch_sharded(lambda b, e: None, 10, 1, 0, 2, dist=None)
 
 
 def _free_port():
@@ -51,19 +53,26 @@ def _free_port():
     return p
 
 
+# a grid whose step (2/6) is not representable: a slab whose interior nodes were re-derived from the slab's
+# own end points would differ from the full grid by an ulp; node ranges of the whole grid cannot
+GRID_N = 7
+GRID_LO_HI = ((-1.0, -1.0, -1.0), (1.0, 1.0, 1.0))
+
+
 def _worker(rank, world, port, out_dir):
     os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
     import torch.distributed as dist
     dist.init_process_group("gloo", rank=rank, world_size=world)
     import oracle as orc
     from paper_1909_10690_b200 import phantoms as ph
-    cfg = ph.get_config("C1")
+    cfg = ph.config_c1(grid_n=GRID_N)
+    lo, hi = GRID_LO_HI
 
-    def map_fn(lo, hi, n):
-        return orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
-                          cfg.family, lo, hi, n, q=cfg.q)["map"]
+    def map_fn(begin, end):
+        return orc.mi_map_range(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
+                                cfg.family, lo, hi, cfg.n, begin, end, q=cfg.q)
 
-    full, am = sh.map_sharded(map_fn, cfg.lo, cfg.hi, cfg.n, 1 + len(cfg.q), rank, world, dist=dist)
+    full, am = sh.map_sharded(map_fn, cfg.n, 1 + len(cfg.q), rank, world, dist=dist)
     np.save(os.path.join(out_dir, "map_%d.npy" % rank), full.numpy())
     np.save(os.path.join(out_dir, "am_%d.npy" % rank), am.numpy())
     dist.barrier()
@@ -74,15 +83,16 @@ def _worker(rank, world, port, out_dir):
 def test_sharded_map_equals_single_rank_map_gloo(world, tmp_path):
     import oracle as orc
     from paper_1909_10690_b200 import phantoms as ph
-    cfg = ph.get_config("C1")
+    cfg = ph.config_c1(grid_n=GRID_N)
+    lo, hi = GRID_LO_HI
     ref = orc.mi_map(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
-                     cfg.family, cfg.lo, cfg.hi, cfg.n, q=cfg.q)
+                     cfg.family, lo, hi, cfg.n, q=cfg.q)
     mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
     for r in range(world):
         m = np.load(tmp_path / ("map_%d.npy" % r))
         am = np.load(tmp_path / ("am_%d.npy" % r))
         assert m.shape == ref["map"].shape
-        assert np.max(np.abs(m - ref["map"])) <= 1e-12       # integer-voxel C1 grid: identical nodes
+        assert np.array_equal(m, ref["map"])                 # bit for bit: every rank's nodes are the full grid's
         assert np.array_equal(am, ref["argmax"])
 
 
