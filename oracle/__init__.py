@@ -20,6 +20,8 @@ _lib = None
 
 INTERP_NEAREST = 0
 INTERP_TRILINEAR = 1
+INTERP_PARTIAL_VOLUME = 2
+PV_UNITS_PER_VOXEL = 1 << 15      # reading A21: per-axis weights in 1/32 voxel, a sample adds 32^3 units
 TSALLIS_ADDITIVE = 0
 TSALLIS_PSEUDO_ADDITIVE = 1
 FAMILY_TRANSLATION = 0
@@ -33,6 +35,7 @@ _f64p = C.POINTER(C.c_double)
 _i32p = C.POINTER(C.c_int32)
 _i64p = C.POINTER(C.c_int64)
 _u32p = C.POINTER(C.c_uint32)
+_u64p = C.POINTER(C.c_uint64)
 _u8p = C.POINTER(C.c_uint8)
 
 
@@ -72,6 +75,14 @@ def lib():
                                      C.c_float, C.c_float, C.c_float, C.c_int, _f64p, _f64p, _i32p, _f64p,
                                      C.c_int, C.c_int, C.c_int, _u8p, _f64p, _i64p]
         L.orc_map_masked.restype = C.c_int
+        L.orc_entropies_u64.argtypes = [_u64p, C.c_int, _f64p, C.c_int, C.c_int, _f64p, _f64p]
+        L.orc_entropies_u64.restype = None
+        L.orc_joint_hist_pv.argtypes = [_f32p, _i32p, _f32p, _i32p, _f32p, C.c_int, C.c_float, C.c_float, C.c_float,
+                                        C.c_float, _u8p, _u64p]
+        L.orc_joint_hist_pv.restype = C.c_int64
+        L.orc_eval_batch_pv.argtypes = [_f32p, _i32p, _f32p, _i32p, _f32p, C.c_int64, C.c_int, C.c_float, C.c_float,
+                                        C.c_float, C.c_float, _f64p, C.c_int, C.c_int, _u8p, _f64p, _u64p, _i64p]
+        L.orc_eval_batch_pv.restype = C.c_int
         L.orc_max_threads.argtypes = []
         L.orc_max_threads.restype = C.c_int
         _lib = L
@@ -164,15 +175,33 @@ def joint_hist(fixed, moving, M, nb, flo, fhi, mlo, mhi, interp, f64_coords: boo
 
 
 def entropies(hist, q=None, form: int = TSALLIS_ADDITIVE, detail: bool = False):
-    """[Shannon I, I_q...] (and [H(A), H(B), H(A,B)] if detail) from a joint histogram."""
-    h = np.ascontiguousarray(hist, dtype=np.uint32)
+    """[Shannon I, I_q...] (and [H(A), H(B), H(A,B)] if detail) from a joint histogram (uint32 counts, or
+    uint64 partial-volume weight units when the array's dtype is uint64)."""
+    wide = np.asarray(hist).dtype == np.uint64
+    h = np.ascontiguousarray(hist, dtype=np.uint64 if wide else np.uint32)
     nb = h.shape[0]
     assert h.shape == (nb, nb)
     qa, nq = _q(q)
     out = np.empty(1 + nq, dtype=np.float64)
     det = np.empty(3, dtype=np.float64)
-    lib().orc_entropies(_p(h, _u32p), nb, _p(qa, _f64p), nq, int(form), _p(out, _f64p), _p(det, _f64p))
+    if wide:
+        lib().orc_entropies_u64(_p(h, _u64p), nb, _p(qa, _f64p), nq, int(form), _p(out, _f64p), _p(det, _f64p))
+    else:
+        lib().orc_entropies(_p(h, _u32p), nb, _p(qa, _f64p), nq, int(form), _p(out, _f64p), _p(det, _f64p))
     return (out, det) if detail else out
+
+
+def joint_hist_pv(fixed, moving, M, nb, flo, fhi, mlo, mhi, mask=None):
+    """Partial-volume joint histogram (reading A21): (nb, nb) uint64 in units of 2^-15 voxel, nvalid."""
+    fx, mv = _vol(fixed), _vol(moving)
+    fd, md = _dims(fx), _dims(mv)
+    M = np.ascontiguousarray(M, dtype=np.float32).reshape(12)
+    hist = np.empty((nb, nb), dtype=np.uint64)
+    mk = _mask(mask, fx)
+    nv = lib().orc_joint_hist_pv(_p(fx, _f32p), _p(fd, _i32p), _p(mv, _f32p), _p(md, _i32p), _p(M, _f32p), int(nb),
+                                 flo, fhi, mlo, mhi, _p(mk.reshape(-1), _u8p) if mk is not None else None,
+                                 _p(hist, _u64p))
+    return hist, int(nv)
 
 
 def _mask(mask, fx):
@@ -195,8 +224,15 @@ def eval_batch(fixed, moving, M, nb, flo, fhi, mlo, mhi, interp, q=None, form=TS
     qa, nq = _q(q)
     mi = np.empty((N, 1 + nq), dtype=np.float64)
     nvalid = np.empty(N, dtype=np.int64)
-    hist = np.empty((N, nb, nb), dtype=np.uint32) if want_hist else None
     mk = _mask(mask, fx)
+    if int(interp) == INTERP_PARTIAL_VOLUME:      # uint64 histograms in units of 2^-15 voxel
+        hist = np.empty((N, nb, nb), dtype=np.uint64) if want_hist else None
+        threads = lib().orc_eval_batch_pv(_p(fx, _f32p), _p(fd, _i32p), _p(mv, _f32p), _p(md, _i32p), _p(M, _f32p), N,
+                                          int(nb), flo, fhi, mlo, mhi, _p(qa, _f64p), nq, int(form),
+                                          _p(mk.reshape(-1), _u8p) if mk is not None else None, _p(mi, _f64p),
+                                          _p(hist, _u64p) if want_hist else None, _p(nvalid, _i64p))
+        return {"mi": mi, "nvalid": nvalid, "hist": hist, "threads": int(threads)}
+    hist = np.empty((N, nb, nb), dtype=np.uint32) if want_hist else None
     threads = lib().orc_eval_batch_masked(_p(fx, _f32p), _p(fd, _i32p), _p(mv, _f32p), _p(md, _i32p),
                                           _p(M, _f32p), N, int(nb), flo, fhi, mlo, mhi, int(interp),
                                           _p(qa, _f64p), nq, int(form),

@@ -22,6 +22,10 @@
 // counts are integers, entropies are fp64.  orc_joint_hist_f64 does the geometry in fp64 so the
 // effect of that reading can be reported (pin P12).
 //
+// Partial-volume interpolation (reading A21; Maes et al., the paper's ref. [5], PAPER.md:228;
+// "the effects of interpolation") is orc_joint_hist_pv below, pinned by
+// tests/test_oracle_pv_pins.py (PV1..PV7).
+//
 // Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): P1..P12 of DESIGN.md.  The one point with
 // no pin is the sign/character of Tsallis maps versus the paper's figures -- "parity unpinned"
 // (the paper prints no Tsallis formula; reading A1/A2).
@@ -334,11 +338,14 @@ int64_t orc_joint_hist_f64(const float* fixed, const int32_t fd[3], const float*
     return nvalid;
 }
 
-// CANON-7: joint histogram -> [Shannon I, I_q0, I_q1, ...]  (eq. 1-2, PAPER.md:25-32; Tsallis per
-// reading A1).  form 0 = ADDITIVE, 1 = PSEUDO_ADDITIVE.  detail (may be NULL) receives
-// [H(A), H(B), H(A,B)].  Empty histogram -> all zeros (reading A13).
-void orc_entropies(const uint32_t* hist, int nb, const double* q, int nq, int form, double* out,
-                   double* detail) {
+}  // extern "C"
+
+namespace {
+
+// CANON-7 on a table of counts (uint32 voxel counts, or uint64 partial-volume weight units -- the
+// probabilities h/N do not depend on the unit).
+template <typename CountT>
+void entropies_of(const CountT* hist, int nb, const double* q, int nq, int form, double* out, double* detail) {
     std::vector<double> joint((size_t)nb * nb), pa(nb, 0.0), pb(nb, 0.0);
     double N = 0.0;
     for (int a = 0; a < nb; ++a)
@@ -369,6 +376,104 @@ void orc_entropies(const uint32_t* hist, int nb, const double* q, int nq, int fo
         if (form == 1) Iq += (1.0 - q[k]) * SA * SB;
         out[1 + k] = Iq;
     }
+}
+
+}  // namespace
+
+extern "C" {
+
+// CANON-7: joint histogram -> [Shannon I, I_q0, I_q1, ...]  (eq. 1-2, PAPER.md:25-32; Tsallis per
+// reading A1).  form 0 = ADDITIVE, 1 = PSEUDO_ADDITIVE.  detail (may be NULL) receives
+// [H(A), H(B), H(A,B)].  Empty histogram -> all zeros (reading A13).
+void orc_entropies(const uint32_t* hist, int nb, const double* q, int nq, int form, double* out,
+                   double* detail) {
+    entropies_of(hist, nb, q, nq, form, out, detail);
+}
+void orc_entropies_u64(const uint64_t* hist, int nb, const double* q, int nq, int form, double* out,
+                       double* detail) {
+    entropies_of(hist, nb, q, nq, form, out, detail);
+}
+
+// Partial-volume interpolation (reading A21).  The method of Maes et al. (ref. [5] of the paper,
+// PAPER.md:228) interpolates no intensity: the sample point's eight neighbours n_i of the moving grid
+// each add their trilinear weight w_i (sum 1) to the cell (bin u(x), bin v(n_i)).  The paper only
+// names the problem ("we start to see the effects of interpolation") and the open
+// question about bins; the arithmetic is this build's reading:
+//   * coordinates, validity region, floor / fraction and the edge clamp are CANON-2 and CANON-4;
+//   * the fraction f_k of each axis is rounded to 1/32 voxel, u_k = floor(32 f_k + 0.5) in 0..32
+//     (both fp32 operations are exact or a single rounding), and the weight of the neighbour with
+//     offsets (dx,dy,dz) is the integer (dx ? u_x : 32-u_x)(dy ? u_y : 32-u_y)(dz ? u_z : 32-u_z):
+//     the eight weights of a sample sum to 2^15 exactly, every histogram is an exact integer table
+//     independent of summation order, and 2^15 units are one voxel;
+//   * neighbours of weight 0 are skipped; the neighbour's bin is CANON-5 of its own value.
+// Returns the number of valid samples; sum(hist) = 2^15 * that number.
+int64_t orc_joint_hist_pv(const float* fixed, const int32_t fd[3], const float* moving, const int32_t md[3],
+                          const float M[12], int nb, float flo, float fhi, float mlo, float mhi,
+                          const uint8_t* mask, uint64_t* hist) {
+    std::memset(hist, 0, sizeof(uint64_t) * (size_t)nb * nb);
+    const float fscale = bin_scale(nb, flo, fhi);
+    const float mscale = bin_scale(nb, mlo, mhi);
+    const size_t nx = md[0], ny = md[1];
+    int64_t nvalid = 0;
+    for (int iz = 0; iz < fd[2]; ++iz)
+        for (int iy = 0; iy < fd[1]; ++iy)
+            for (int ix = 0; ix < fd[0]; ++ix) {
+                size_t i = ((size_t)iz * fd[1] + iy) * fd[0] + ix;
+                if (mask != nullptr && mask[i] == 0) continue;
+                float c[3];
+                coords(M, ix, iy, iz, c);
+                int idx[3][2];   // the two neighbours per axis, clamped to the volume
+                int w[3][2];     // their weights in 1/32
+                bool ok = true;
+                for (int k = 0; k < 3; ++k) {
+                    if (!(c[k] >= -0.5f && c[k] < (float)md[k] - 0.5f)) { ok = false; break; }
+                    float g = floorf(c[k]);
+                    float f = c[k] - g;
+                    int u = (int)floorf(f * 32.0f + 0.5f);
+                    int gi = (int)g;
+                    idx[k][0] = gi > 0 ? gi : 0;
+                    idx[k][1] = (gi + 1 < md[k] - 1) ? gi + 1 : md[k] - 1;
+                    w[k][0] = 32 - u;
+                    w[k][1] = u;
+                }
+                if (!ok) continue;
+                int a = bin_of(fixed[i], flo, fscale, nb);
+                for (int dz = 0; dz < 2; ++dz)
+                    for (int dy = 0; dy < 2; ++dy)
+                        for (int dx = 0; dx < 2; ++dx) {
+                            int wt = w[0][dx] * w[1][dy] * w[2][dz];
+                            if (wt == 0) continue;
+                            float v = moving[((size_t)idx[2][dz] * ny + idx[1][dy]) * nx + idx[0][dx]];
+                            int b = bin_of(v, mlo, mscale, nb);
+                            hist[(size_t)a * nb + b] += (uint64_t)wt;
+                        }
+                ++nvalid;
+            }
+    return nvalid;
+}
+
+// N transforms with partial-volume interpolation -> N x (1+nq) MI values (+ optional uint64
+// histograms and valid counts); OpenMP over transforms as orc_eval_batch_masked.
+int orc_eval_batch_pv(const float* fixed, const int32_t fd[3], const float* moving, const int32_t md[3],
+                      const float* M, int64_t N, int nb, float flo, float fhi, float mlo, float mhi,
+                      const double* q, int nq, int form, const uint8_t* mask, double* mi_out,
+                      uint64_t* hist_out, int64_t* nvalid_out) {
+    int nthreads = 1;
+#ifdef _OPENMP
+    nthreads = omp_get_max_threads();
+#endif
+#pragma omp parallel
+    {
+        std::vector<uint64_t> h((size_t)nb * nb);
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t t = 0; t < N; ++t) {
+            int64_t nv = orc_joint_hist_pv(fixed, fd, moving, md, M + t * 12, nb, flo, fhi, mlo, mhi, mask, h.data());
+            orc_entropies_u64(h.data(), nb, q, nq, form, mi_out + t * (1 + nq), nullptr);
+            if (hist_out) std::memcpy(hist_out + (size_t)t * nb * nb, h.data(), sizeof(uint64_t) * h.size());
+            if (nvalid_out) nvalid_out[t] = nv;
+        }
+    }
+    return nthreads;
 }
 
 // N index-space transforms -> N x (1+nq) MI values (+ optional histograms and valid counts).
@@ -406,6 +511,7 @@ int orc_eval_batch(const float* fixed, const int32_t fd[3], const float* moving,
 }
 
 // Exhaustive map: grid value k on axis d is lo[d] + k (hi[d]-lo[d])/(n[d]-1);
+// interp: 0 nearest, 1 trilinear, 2 partial volume.
 // map_out is (1+nq) x n[2] x n[1] x n[0], channel-major, p0 fastest; argmax per channel with ties
 // to the lowest linear index (eq. 3).  Returns the number of threads used.
 int orc_map_masked(const float* fixed, const int32_t fd[3], const double fs[3], const float* moving,
@@ -427,8 +533,11 @@ int orc_map_masked(const float* fixed, const int32_t fd[3], const double fs[3], 
                 orc_index_affine(T, fd, fs, md, ms, M.data() + t * 12);
             }
     std::vector<double> mi((size_t)NT * (1 + nq));
-    int nthreads = orc_eval_batch_masked(fixed, fd, moving, md, M.data(), NT, nb, flo, fhi, mlo, mhi, interp,
-                                         q, nq, form, mask, mi.data(), nullptr, nullptr);
+    int nthreads = interp == 2
+        ? orc_eval_batch_pv(fixed, fd, moving, md, M.data(), NT, nb, flo, fhi, mlo, mhi, q, nq, form, mask,
+                            mi.data(), nullptr, nullptr)
+        : orc_eval_batch_masked(fixed, fd, moving, md, M.data(), NT, nb, flo, fhi, mlo, mhi, interp,
+                                q, nq, form, mask, mi.data(), nullptr, nullptr);
     for (int ch = 0; ch < 1 + nq; ++ch) {
         int64_t best = 0;
         for (int64_t t = 0; t < NT; ++t) {
