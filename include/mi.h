@@ -57,7 +57,14 @@ typedef enum {
     MI_ERR_INTERNAL = 5
 } mi_status;
 
-typedef enum { MI_INTERP_NEAREST = 0, MI_INTERP_TRILINEAR = 1 } mi_interp;
+/* Interpolation of the Transform block v(T(x)) ("the effects of interpolation").
+ * NEAREST and TRILINEAR interpolate the intensity and add one count per sample.  PARTIAL_VOLUME is the
+ * method of Maes et al. (the paper's ref. [5]; reading A21): no intensity is
+ * interpolated, the eight neighbours of the sample point each add their trilinear weight to the cell
+ * (bin u(x), bin v(neighbour)).  Weights are products of per-axis fractions rounded to 1/32 voxel, so one
+ * sample adds exactly 2^15 integer units and the histogram does not depend on the order of the updates.
+ * nbins <= 256 only; every transform takes the generic path. */
+typedef enum { MI_INTERP_NEAREST = 0, MI_INTERP_TRILINEAR = 1, MI_INTERP_PARTIAL_VOLUME = 2 } mi_interp;
 
 /* Tsallis entropy S_q(X) = (1 - sum_{p>0} p^q)/(q - 1).  The paper prints no Tsallis formula
  * (reading A1); ADDITIVE puts S_q into the paper's own eq. 2 and is the default. */
@@ -109,12 +116,18 @@ mi_status mi_set_tsallis_form(mi_ctx *ctx, mi_tsallis_form form);
  *   mi_out      N x (1+nq) doubles: [Shannon I (nats), I_q0, I_q1, ...] per transform.  An empty
  *               overlap gives zeros.
  *   hist_out    NULL, or N x nbins x nbins uint32 joint histograms, row = fixed bin, column =
- *               moving bin.
+ *               moving bin.  Must be NULL with MI_INTERP_PARTIAL_VOLUME (see mi_eval_batch_pv).
  *   nvalid_out  NULL, or N int64: samples inside the moving volume per transform.
  * N == 0 is a no-op returning MI_OK.  Every transform takes the generic resample+histogram kernel (only
  * mi_map / mi_map_range recognise diagonal grids and take the separable kernels). */
 mi_status mi_eval_batch(mi_ctx *ctx, const double *T, int64_t N, const double *q, int32_t nq,
                         mi_interp interp, double *mi_out, uint32_t *hist_out, int64_t *nvalid_out);
+
+/* mi_eval_batch with MI_INTERP_PARTIAL_VOLUME and the histograms in their own unit: hist_out is NULL or
+ * N x nbins x nbins uint64 weights in units of 2^-15 voxel (sum = 2^15 * nvalid).  Other arguments as
+ * mi_eval_batch.  MI_ERR_UNSUPPORTED for nbins > 256. */
+mi_status mi_eval_batch_pv(mi_ctx *ctx, const double *T, int64_t N, const double *q, int32_t nq,
+                           double *mi_out, uint64_t *hist_out, int64_t *nvalid_out);
 
 /* mi_map -- the exhaustive map of one family: "map with the MI function all
  * the space in a finite range and build a 3D image".
@@ -136,7 +149,8 @@ mi_status mi_map(mi_ctx *ctx, mi_family family, const double lo[3], const double
  *   argmax_out  NULL, or (1+nq) linear indices into the SUB-BOX.
  *   hist_out    NULL, or m[2]*m[1]*m[0] joint histograms of nbins x nbins uint32 in sub-box node order
  *               (row = fixed bin).  Diagonal families then run the separable kernels with the
- *               histogram written out instead of the fused entropy epilogue. */
+ *               histogram written out instead of the fused entropy epilogue.  Must be NULL with
+ *               MI_INTERP_PARTIAL_VOLUME. */
 mi_status mi_map_range(mi_ctx *ctx, mi_family family, const double lo[3], const double hi[3],
                        const int32_t n[3], const int32_t begin[3], const int32_t end[3],
                        const double *q, int32_t nq, mi_interp interp,
@@ -164,7 +178,7 @@ typedef enum {
     MI_INFO_ZHIST_ROWS = 102,      /* fixed-bin ranks the z kernel counts in shared memory                      */
     MI_INFO_RARE_VOXELS = 103,     /* fixed voxels of the ranks that do not fit (0 = the epilogue can be fused) */
     MI_INFO_GENERIC_ROWS = 104,    /* fixed-bin ranks the generic kernel counts in shared memory                */
-    MI_INFO_LAST_PATH = 105        /* path of the last call: 0 generic, 1 separable, 2 wide-histogram kernels   */
+    MI_INFO_LAST_PATH = 105        /* path of the last call: 0 generic, 1 separable, 2 wide-histogram, 3 partial-volume kernels */
 } mi_option;
 mi_status mi_set_option(mi_ctx *ctx, mi_option key, int64_t value);
 mi_status mi_get_option(const mi_ctx *ctx, mi_option key, int64_t *value);

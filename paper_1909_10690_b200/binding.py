@@ -18,7 +18,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmi_b200.so")
 
 MI_OK, MI_ERR_INVALID_ARG, MI_ERR_UNSUPPORTED, MI_ERR_OUT_OF_MEMORY, MI_ERR_CUDA, MI_ERR_INTERNAL = range(6)
-MI_INTERP_NEAREST, MI_INTERP_TRILINEAR = 0, 1
+MI_INTERP_NEAREST, MI_INTERP_TRILINEAR, MI_INTERP_PARTIAL_VOLUME = 0, 1, 2
+MI_PV_UNITS_PER_VOXEL = 1 << 15
 MI_TSALLIS_ADDITIVE, MI_TSALLIS_PSEUDO_ADDITIVE = 0, 1
 (MI_FAMILY_TRANSLATION, MI_FAMILY_ROTATION_EULER_DEG, MI_FAMILY_ROTATION_VERSOR, MI_FAMILY_SCALE,
  MI_FAMILY_SCALE_LOG) = range(5)
@@ -31,7 +32,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 (MI_INFO_NUM_SMS, MI_INFO_BIN_MODE, MI_INFO_ZHIST_ROWS, MI_INFO_RARE_VOXELS, MI_INFO_GENERIC_ROWS,
  MI_INFO_LAST_PATH) = range(100, 106)
 
-EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_map", "mi_map_range", "mi_set_option",
+EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_map", "mi_map_range", "mi_set_option",
            "mi_get_option", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
            "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient", "mi_register",
@@ -52,6 +53,8 @@ _lib.mi_set_fixed_mask.argtypes = [_vp, _vp]
 _lib.mi_set_fixed_mask.restype = C.c_int
 _lib.mi_eval_batch.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, C.c_int, _vp, _vp, _vp]
 _lib.mi_eval_batch.restype = C.c_int
+_lib.mi_eval_batch_pv.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp, _vp]
+_lib.mi_eval_batch_pv.restype = C.c_int
 _lib.mi_map.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp]
 _lib.mi_map.restype = C.c_int
 _lib.mi_map_range.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp, _vp]
@@ -222,6 +225,31 @@ def mi_eval_batch(ctx, T, q=(), interp=MI_INTERP_TRILINEAR, mi_out=None, hist_ou
         nvalid_out = None
     st = _lib.mi_eval_batch(ctx.handle, _ptr(T), N, _ptr(q) if nq else None, nq, int(interp), _ptr(mi_out),
                             _ptr(hist_out), _ptr(nvalid_out))
+    _check(ctx, st)
+    return mi_out, hist_out, nvalid_out
+
+
+def mi_eval_batch_pv(ctx, T, q=(), mi_out=None, hist_out=None, nvalid_out=None):
+    """Partial-volume interpolation: as mi_eval_batch, histograms are (N, nbins, nbins) uint64 in units of
+    2^-15 voxel.  Returns (mi, hist, nvalid)."""
+    T = _f64(T)
+    N = T.size // 12
+    assert T.size == N * 12
+    q = _f64(q)
+    nq = q.size
+    nb = ctx.nbins
+    if mi_out is None or mi_out is True:
+        mi_out = np.empty((N, 1 + nq), dtype=np.float64)
+    if hist_out is True:
+        hist_out = np.empty((N, nb, nb), dtype=np.uint64)
+    elif hist_out is False:
+        hist_out = None
+    if nvalid_out is True:
+        nvalid_out = np.empty(N, dtype=np.int64)
+    elif nvalid_out is False:
+        nvalid_out = None
+    st = _lib.mi_eval_batch_pv(ctx.handle, _ptr(T), N, _ptr(q) if nq else None, nq, _ptr(mi_out), _ptr(hist_out),
+                               _ptr(nvalid_out))
     _check(ctx, st)
     return mi_out, hist_out, nvalid_out
 

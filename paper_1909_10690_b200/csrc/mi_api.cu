@@ -28,6 +28,7 @@ struct mi_ctx {
     int* d_rank_inv = nullptr;          // 256: rank -> fixed bin
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     uint8_t* d_mbins = nullptr;
+    uint8_t* d_mbins_pad = nullptr;     // replicate-padded moving bins (partial-volume interpolation)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
     unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
     unsigned rare_alloc = 0;            // entries d_rare was allocated for
@@ -190,6 +191,15 @@ mi_status grow(mi_ctx* c, T** p, size_t* cap, size_t need) {
     if (*p) { dev_free(*p, c->stream); *p = nullptr; *cap = 0; }
     MI_CUDA(c, dev_alloc(reinterpret_cast<void**>(p), need * sizeof(T), c->device, c->stream));
     *cap = need;
+    return MI_OK;
+}
+
+// interpolation argument of the compute entry points; partial volume needs the shared-memory path
+mi_status validate_interp(mi_ctx* c, int interp) {
+    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR && interp != MI_INTERP_PARTIAL_VOLUME)
+        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
+    if (interp == MI_INTERP_PARTIAL_VOLUME && c->wide)
+        return fail(c, MI_ERR_UNSUPPORTED, "partial-volume interpolation needs nbins <= 256");
     return MI_OK;
 }
 
@@ -462,10 +472,15 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
 // memory.  If map_out != NULL the result is assembled channel-major (step a6) instead of being
 // returned transform-major.  If sep != NULL the histograms are built by the separable path.
 mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const double* q, int32_t nq,
-                    int interp, double* mi_out, uint32_t* hist_out, int64_t* nvalid_out,
+                    int interp, double* mi_out, void* hist_out_v, int64_t* nvalid_out,
                     double* map_out, int64_t* argmax_out, const SeparablePlan* sep = nullptr) {
     const int nch = 1 + nq;
     const size_t nbins2 = (size_t)c->nb * c->nb;
+    // partial-volume histograms hold uint64 weight units, the others uint32 counts
+    const bool pv = interp == MI_INTERP_PARTIAL_VOLUME;
+    const size_t helem = pv ? sizeof(unsigned long long) : sizeof(uint32_t);
+    uint32_t* const hist_out = static_cast<uint32_t*>(hist_out_v);
+    if (pv) sep = nullptr;
     cudaStream_t s = c->stream;
     for (int k = 0; k < 5; ++k) { c->last_ms[k] = 0.f; c->last_launches[k] = 0; }
     EventTimer timer(s);
@@ -492,7 +507,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
 
     // ---- chunk plan --------------------------------------------------------------------------------
     const bool hist_to_user_dev = hist_out != nullptr && !is_host_ptr(hist_out);
-    int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * sizeof(uint32_t)));
+    int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * helem));
     if (chunk < 1) chunk = 1;
     if (chunk > N) chunk = N;
     if (sep != nullptr) {
@@ -500,20 +515,21 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         if (st == kSepFallback) sep = nullptr;   // one (p0,p1) pair exceeds the scratch budgets: generic kernel
         else if (st != MI_OK) return st;
     }
-    c->last_path = sep != nullptr ? 1 : (c->wide ? 2 : 0);
+    c->last_path = sep != nullptr ? 1 : (pv ? 3 : (c->wide ? 2 : 0));
     if (!hist_to_user_dev && sep == nullptr) {
         if ((st = grow(c, reinterpret_cast<uint8_t**>(&c->d_hist), &c->cap_hist,
-                       (size_t)chunk * nbins2 * sizeof(uint32_t))) != MI_OK)
+                       (size_t)chunk * nbins2 * helem)) != MI_OK)
             return st;
     }
     const int rows_total = c->fd[1] * c->fd[2];
 
     for (int64_t off = 0; sep == nullptr && off < N; off += chunk) {
         const int64_t cnt = (N - off < chunk) ? (N - off) : chunk;
-        uint32_t* hist = hist_to_user_dev ? hist_out + (size_t)off * nbins2 : c->d_hist;
+        uint32_t* hist = hist_to_user_dev
+            ? reinterpret_cast<uint32_t*>(static_cast<char*>(hist_out_v) + (size_t)off * nbins2 * helem) : c->d_hist;
 
         timer.begin(1);
-        MI_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)cnt * nbins2 * sizeof(uint32_t), s));
+        MI_CUDA(c, cudaMemsetAsync(hist, 0, (size_t)cnt * nbins2 * helem, s));
         mi::ResampleArgs a;
         a.fbins_ranked = c->d_fbins_ranked;
         a.rank_inv = c->d_rank_inv;
@@ -543,7 +559,23 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         }
         a.nslabs = nslabs;
         timer.begin(4);
-        if (c->wide) {
+        if (pv) {
+            mi::PvArgs pa;
+            pa.fbins_ranked = c->d_fbins_ranked;
+            pa.rank_inv = c->d_rank_inv;
+            pa.mask_bits = c->d_mask_bits;
+            pa.mbins_pad = c->d_mbins_pad;
+            pa.M = a.M;
+            pa.hist = reinterpret_cast<unsigned long long*>(hist);
+            pa.rows_smem = c->rows_smem;
+            pa.pitch = c->gpitch;
+            pa.f = a.f;
+            pa.m = a.m;
+            pa.nb = c->nb;
+            pa.n_transforms = (int)cnt;
+            pa.nchunks = 0;
+            MI_CUDA(c, mi::launch_resample_hist_pv(pa, c->num_sms, s));
+        } else if (c->wide) {
             mi::WideArgs w;
             w.fbins = c->d_fbins16;
             w.mbins = c->d_mbins16;
@@ -570,6 +602,11 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         timer.begin(2);
         int q_off = 0;
         do {
+            if (pv)
+                MI_CUDA(c, mi::launch_entropy_pv(reinterpret_cast<const unsigned long long*>(hist), c->nb, (int)cnt, c->d_q, nq,
+                                                 q_off, c->tsallis_form, c->d_mi + (size_t)off * nch, c->d_nvalid + off,
+                                                 mi::OutMap{0, 0, 0, 0, 0, 0, 0}, s));
+            else
             MI_CUDA(c, mi::launch_entropy(hist, c->nb, (int)cnt, c->d_q, nq, q_off, c->tsallis_form,
                                           c->d_mi + (size_t)off * nch, c->d_nvalid + off, mi::OutMap{0, 0, 0, 0, 0, 0, 0}, s));
             c->last_launches[2] += 1;
@@ -578,8 +615,8 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         timer.end();
 
         if (hist_out != nullptr && !hist_to_user_dev)
-            MI_CUDA(c, cudaMemcpyAsync(hist_out + (size_t)off * nbins2, hist,
-                                       (size_t)cnt * nbins2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, s));
+            MI_CUDA(c, cudaMemcpyAsync(static_cast<char*>(hist_out_v) + (size_t)off * nbins2 * helem, hist,
+                                       (size_t)cnt * nbins2 * helem, cudaMemcpyDeviceToHost, s));
     }
 
     // ---- outputs -----------------------------------------------------------------------------------
@@ -754,6 +791,10 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync ranks"); break; }
         }
         if ((st = plan_layout(c)) != MI_OK) { mi::set_thread_error(c->err); break; }
+        if (!c->wide) {
+            if ((e = dev_alloc((void**)&c->d_mbins_pad, (size_t)npad, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving bins"); break; }
+            if ((e = mi::launch_pad_replicate_u8(c->d_mbins, c->d_mbins_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving bins"); break; }
+        }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
@@ -773,7 +814,7 @@ void mi_destroy(mi_ctx* c) {
     DeviceGuard guard(c->device);
     if (guard.ok) {
         void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mask_bits, c->d_fbins16, c->d_mbins16, c->d_mbins,
-                        c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
+                        c->d_mbins_pad, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);
@@ -901,13 +942,13 @@ mi_status mi_get_option(const mi_ctx* c, mi_option key, int64_t* out) {
     return MI_OK;
 }
 
-mi_status mi_eval_batch(mi_ctx* c, const double* T, int64_t N, const double* q, int32_t nq,
-                        mi_interp interp, double* mi_out, uint32_t* hist_out, int64_t* nvalid_out) {
+static mi_status eval_batch_impl(mi_ctx* c, const double* T, int64_t N, const double* q, int32_t nq, int interp,
+                                 double* mi_out, void* hist_out, int64_t* nvalid_out) {
     if (!c) return MI_ERR_INVALID_ARG;
     if (N < 0) return fail(c, MI_ERR_INVALID_ARG, "N < 0");
-    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
-        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
-    mi_status st = validate_q(c, q, nq);
+    mi_status st = validate_interp(c, interp);
+    if (st != MI_OK) return st;
+    st = validate_q(c, q, nq);
     if (st != MI_OK) return st;
     if (N == 0) return MI_OK;
     if (T == nullptr || mi_out == nullptr) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
@@ -926,7 +967,19 @@ mi_status mi_eval_batch(mi_ctx* c, const double* T, int64_t N, const double* q, 
     }
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
-    return eval_core(c, hM, N, q, nq, (int)interp, mi_out, hist_out, nvalid_out, nullptr, nullptr);
+    return eval_core(c, hM, N, q, nq, interp, mi_out, hist_out, nvalid_out, nullptr, nullptr);
+}
+
+mi_status mi_eval_batch(mi_ctx* c, const double* T, int64_t N, const double* q, int32_t nq,
+                        mi_interp interp, double* mi_out, uint32_t* hist_out, int64_t* nvalid_out) {
+    if (c && interp == MI_INTERP_PARTIAL_VOLUME && hist_out != nullptr)
+        return fail(c, MI_ERR_INVALID_ARG, "partial-volume histograms are uint64: use mi_eval_batch_pv");
+    return eval_batch_impl(c, T, N, q, nq, (int)interp, mi_out, hist_out, nvalid_out);
+}
+
+mi_status mi_eval_batch_pv(mi_ctx* c, const double* T, int64_t N, const double* q, int32_t nq,
+                           double* mi_out, uint64_t* hist_out, int64_t* nvalid_out) {
+    return eval_batch_impl(c, T, N, q, nq, MI_INTERP_PARTIAL_VOLUME, mi_out, hist_out, nvalid_out);
 }
 
 mi_status mi_compose_matrix(const double p[9], double T_out[12]) {
@@ -983,9 +1036,9 @@ mi_status gradient_core(mi_ctx* c, const double p[9], const double delta[9], dou
 
 mi_status validate_gradient_args(mi_ctx* c, const double* p, const double* delta, double q, int interp) {
     if (!p || !delta) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
-    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
-        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
-    mi_status st = validate_q(c, &q, 1);
+    mi_status st = validate_interp(c, interp);
+    if (st != MI_OK) return st;
+    st = validate_q(c, &q, 1);
     if (st != MI_OK) return st;
     for (int i = 0; i < 9; ++i)
         if (!std::isfinite(p[i]) || !std::isfinite(delta[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite parameter");
@@ -1063,8 +1116,10 @@ mi_status mi_map_range(mi_ctx* c, mi_family family, const double lo[3], const do
                        double* map_out, int64_t* argmax_out, uint32_t* hist_out) {
     if (!c) return MI_ERR_INVALID_ARG;
     if (!lo || !hi || !n || !map_out) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
-    if (interp != MI_INTERP_NEAREST && interp != MI_INTERP_TRILINEAR)
-        return fail(c, MI_ERR_INVALID_ARG, "unknown interpolation");
+    mi_status st = validate_interp(c, (int)interp);
+    if (st != MI_OK) return st;
+    if (interp == MI_INTERP_PARTIAL_VOLUME && hist_out != nullptr)
+        return fail(c, MI_ERR_INVALID_ARG, "partial-volume histograms are uint64: use mi_eval_batch_pv");
     if ((int)family < 0 || (int)family > MI_FAMILY_SCALE_LOG) return fail(c, MI_ERR_INVALID_ARG, "unknown family");
     if (!finite3(lo) || !finite3(hi)) return fail(c, MI_ERR_INVALID_ARG, "non-finite grid bound");
     int32_t kb[3], m[3];   // first node and node count of the sub-box per axis
@@ -1078,7 +1133,7 @@ mi_status mi_map_range(mi_ctx* c, mi_family family, const double lo[3], const do
         N *= m[d];
         if (N > 0x7FFFFFFFLL / 16) return fail(c, MI_ERR_UNSUPPORTED, "too many transforms in one call");
     }
-    mi_status st = validate_q(c, q, nq);
+    st = validate_q(c, q, nq);
     if (st != MI_OK) return st;
     std::vector<float> hM;
     try {
@@ -1107,7 +1162,8 @@ mi_status mi_map_range(mi_ctx* c, mi_family family, const double lo[3], const do
     // translation / scale maps have diagonal matrices: separable fast path (same arithmetic)
     SeparablePlan plan;
     const bool diag_family = family == MI_FAMILY_TRANSLATION || family == MI_FAMILY_SCALE || family == MI_FAMILY_SCALE_LOG;
-    const bool sep = diag_family && c->use_separable && c->separable_ok && c->zrows_smem >= 2 && make_separable_plan(hM, m, &plan);
+    const bool sep = diag_family && interp != MI_INTERP_PARTIAL_VOLUME && c->use_separable && c->separable_ok &&
+                     c->zrows_smem >= 2 && make_separable_plan(hM, m, &plan);
     return eval_core(c, hM, N, q, nq, (int)interp, nullptr, hist_out, nullptr, map_out, argmax_out,
                      sep ? &plan : nullptr);
 }

@@ -15,6 +15,7 @@
 #include <math_constants.h>
 #include <stdint.h>
 
+#include "mi_device.cuh"
 #include "mi_internal.h"
 
 namespace mi {
@@ -194,21 +195,10 @@ cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long
 // ------------------------------------------------------------------------------------------------
 // a3 + a4: resample + joint histogram (generic affine)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned warp_sum(unsigned v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
 // CANON-4 lerp: L(p,q,f) = fma(f, q - p, p) with q - p rounded first.
 __device__ __forceinline__ float lerp_rn(float p, float q, float f) {
     return __fmaf_rn(f, __fsub_rn(q, p), p);
 }
-
-// floor() of |c| < 2^22 without a conversion instruction: RD(c + 1.5*2^23) = 1.5*2^23 + floor(c)
-// exactly (ulp is 1 there), so the low mantissa bits ARE floor(c) as a two's-complement offset.
-constexpr float kFloorMagic = 12582912.0f;        // 1.5 * 2^23
-constexpr int kFloorMagicBits = 0x4B400000;
 
 struct Sample {
     bool ok;   // inside the moving volume (CANON-3/4 validity)
@@ -440,46 +430,6 @@ cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms,
 // ------------------------------------------------------------------------------------------------
 // a5: entropy reduction (DESIGN.md CANON-7)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double warp_sum_d(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-// Last step of a5 for transform t from the three distributions' sums (tot[0..2] = sum c ln c of A, B, AB;
-// tot[3 + 3k + {0,1,2}] = sum c^q_k) and the sample count n: eq. 1-2 and the Tsallis forms.
-__device__ void entropy_finish(const double* tot, unsigned long long n, int t, const double* qv, int nq_pass,
-                               int q_off, int nq_total, int form, double* __restrict__ mi_out,
-                               int64_t* __restrict__ nvalid, const OutMap& om) {
-    const size_t dst = om.dst(t);  // item order (p0, p1, p2 fastest) -> map order (p2, p1, p0 fastest)
-    double* out = mi_out + dst * (1 + nq_total);
-    if (nvalid != nullptr) nvalid[dst] = (int64_t)n;
-    if (n == 0) {
-        out[0] = 0.0;
-        for (int k = 0; k < nq_pass; ++k) out[1 + q_off + k] = 0.0;
-        return;
-    }
-    const double N = (double)n, lnN = log(N);
-    const double HA = lnN - tot[0] / N, HB = lnN - tot[1] / N, HAB = lnN - tot[2] / N;
-    const double I = HA + HB - HAB;  // eq. 2
-    out[0] = I;
-    for (int k = 0; k < nq_pass; ++k) {
-        const double qq = qv[k];
-        double val;
-        if (qq == 1.0) {
-            val = I;
-        } else {
-            const double sc = exp(-qq * lnN);
-            const double SA = (1.0 - tot[3 + 3 * k + 0] * sc) / (qq - 1.0);
-            const double SB = (1.0 - tot[3 + 3 * k + 1] * sc) / (qq - 1.0);
-            const double SAB = (1.0 - tot[3 + 3 * k + 2] * sc) / (qq - 1.0);
-            val = SA + SB - SAB;
-            if (form == MI_TSALLIS_PSEUDO_ADDITIVE) val += (1.0 - qq) * SA * SB;
-        }
-        out[1 + q_off + k] = val;
-    }
-}
-
 // One CTA per transform.  With c the integer counts and N their total:
 //   H = -sum (c/N) ln (c/N) = ln N - (sum c ln c)/N,      sum p^q = exp(-q ln N) * sum c^q.
 // Accumulators per distribution X in {A, B, AB}: L_X = sum c ln c and P_X[k] = sum c^q_k.
@@ -571,7 +521,7 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
         }
         unsigned long long n = 0;
         for (int w = 0; w < NW; ++w) n += sh_n[w];
-        entropy_finish(tot, n, t, qv, nq_pass, q_off, nq_total, form, mi_out, nvalid, om);
+        entropy_finish(tot, (double)n, (long long)n, t, qv, nq_pass, q_off, nq_total, form, mi_out, nvalid, om);
     }
 }
 
@@ -692,7 +642,7 @@ entropy_wide_final_kernel(int nb, const double* __restrict__ q, int nq_total, in
         }
         unsigned long long n = 0;
         for (int w = 0; w < NW; ++w) n += sh_n[w];
-        entropy_finish(tot, n, t, qv, nq_pass, q_off, nq_total, form, mi_out, nvalid, om);
+        entropy_finish(tot, (double)n, (long long)n, t, qv, nq_pass, q_off, nq_total, form, mi_out, nvalid, om);
     }
 }
 

@@ -1,0 +1,240 @@
+// mi_pv.cu -- partial-volume interpolation (reading A21): the joint histogram
+// of Maes et al. (the paper's ref. [5]), which interpolates no intensity -- "we start to see
+// the effects of interpolation", PAPER.md:214 -- but lets the eight neighbours n_i of a sample point each
+// add their trilinear weight to the cell (bin u(x), bin v(n_i)).
+//
+// Arithmetic (reading A21): coordinates, validity, floor / fraction and edge clamp are CANON-2 / CANON-4;
+// the fraction of each axis is rounded to 1/32 voxel, u = floor(32 f + 0.5), and a neighbour's weight is the
+// integer product of (u or 32 - u) over the axes, so a sample adds exactly 2^15 units and every histogram is an
+// integer table that does not depend on the order of the updates.  Neighbour bins come from the pre-binned,
+// replicate-padded moving volume (eight byte gathers, no lerps).
+//
+//   resample_hist_pv_kernel   CTA-private u32 histogram in shared memory, one (transform, voxel chunk) item
+//                             at a time; a chunk holds at most 131040 voxels so that no counter can pass
+//                             2^32 (131040 * 2^15 < 2^32); merged into the transform's uint64 histogram
+//   entropy_pv_kernel         step a5 on uint64 counts (unit 2^-15 voxel; probabilities are unit-free)
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "mi_device.cuh"
+#include "mi_internal.h"
+
+namespace mi {
+
+namespace {
+
+constexpr int kPvChunkVoxels = 131040;   // multiple of 32; 131040 * 32768 = 4293918720 < 2^32
+
+__global__ void __launch_bounds__(256) pad_replicate_u8_kernel(const uint8_t* __restrict__ src,
+                                                               uint8_t* __restrict__ dst, int nx, int ny, int nz) {
+    const int px = nx + 2, py = ny + 2, pz = nz + 2;
+    const int64_t total = (int64_t)px * py * pz;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % px);
+        const int64_t r = i / px;
+        const int y = (int)(r % py), z = (int)(r / py);
+        const int sx = min(max(x - 1, 0), nx - 1), sy = min(max(y - 1, 0), ny - 1), sz = min(max(z - 1, 0), nz - 1);
+        dst[i] = src[((int64_t)sz * ny + sy) * nx + sx];
+    }
+}
+
+// One axis: validity (CANON-4 region), padded lower index floor(c) + 1 and the weight pair (32 - u, u).
+struct PvAxis {
+    bool ok;
+    int lower;
+    unsigned w0, w1;
+};
+__device__ __forceinline__ PvAxis pv_axis(float c, float half_hi) {
+    PvAxis a;
+    a.ok = c >= -0.5f && c < half_hi;
+    const float t = __fadd_rd(c, kFloorMagic);
+    a.lower = __float_as_int(t) - kFloorMagicBits + 1;
+    const float f = __fsub_rn(c, __fsub_rn(t, kFloorMagic));
+    const int u = __float2int_rd(__fadd_rn(__fmul_rn(f, 32.0f), 0.5f));
+    a.w1 = (unsigned)u;
+    a.w0 = 32u - (unsigned)u;
+    return a;
+}
+
+__global__ void __launch_bounds__(kHistThreads, 1) resample_hist_pv_kernel(const __grid_constant__ PvArgs a) {
+    extern __shared__ __align__(16) uint32_t sh_hist[];
+    const int nb = a.nb, pitch = a.pitch, rows_smem = a.rows_smem;
+    const int words = rows_smem * pitch;
+    for (int w = threadIdx.x; w < words; w += blockDim.x) sh_hist[w] = 0u;
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    const int fnx = a.f.nx, fny = a.f.ny;
+    const long long nf = (long long)a.f.nx * a.f.ny * a.f.nz;
+    const int pnx = a.m.nx + 2, pny = a.m.ny + 2;
+    const float hx = __fsub_rn((float)a.m.nx, 0.5f), hy = __fsub_rn((float)a.m.ny, 0.5f), hz = __fsub_rn((float)a.m.nz, 0.5f);
+    const long long nitems = (long long)a.n_transforms * a.nchunks;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int t = (int)(item / a.nchunks);
+        const int chunk = (int)(item - (long long)t * a.nchunks);
+        const long long v_lo = (long long)chunk * kPvChunkVoxels;
+        const long long v_hi = v_lo + kPvChunkVoxels < nf ? v_lo + kPvChunkVoxels : nf;
+        float m[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
+        unsigned long long* gh = a.hist + (size_t)t * nb * nb;
+        for (long long v0 = v_lo + warp * 32; v0 < v_hi; v0 += nwarps * 32) {
+            const long long v = v0 + lane;
+            if (v >= v_hi) continue;
+            const int ix = (int)(v % fnx);
+            const long long row = v / fnx;
+            const int iy = (int)(row % fny), iz = (int)(row / fny);
+            if (a.mask_bits != nullptr && ((__ldg(a.mask_bits + (v >> 5)) >> (v & 31)) & 1u) == 0u) continue;
+            const float fx = (float)ix, fy = (float)iy, fz = (float)iz;
+            // CANON-2
+            const float cx = __fmaf_rn(m[0], fx, __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3])));
+            const float cy = __fmaf_rn(m[4], fx, __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7])));
+            const float cz = __fmaf_rn(m[8], fx, __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11])));
+            const PvAxis ax = pv_axis(cx, hx), ay = pv_axis(cy, hy), az = pv_axis(cz, hz);
+            if (!(ax.ok && ay.ok && az.ok)) continue;
+            const int fa = __ldg(a.fbins_ranked + v);
+            const uint8_t* __restrict__ p = a.mbins_pad + ((size_t)az.lower * pny + ay.lower) * pnx + ax.lower;
+            const uint8_t* __restrict__ pz = p + (size_t)pnx * pny;
+            const unsigned b000 = __ldg(p), b100 = __ldg(p + 1), b010 = __ldg(p + pnx), b110 = __ldg(p + pnx + 1);
+            const unsigned b001 = __ldg(pz), b101 = __ldg(pz + 1), b011 = __ldg(pz + pnx), b111 = __ldg(pz + pnx + 1);
+            const unsigned wy0z0 = ay.w0 * az.w0, wy1z0 = ay.w1 * az.w0, wy0z1 = ay.w0 * az.w1, wy1z1 = ay.w1 * az.w1;
+            const unsigned bins[8] = {b000, b100, b010, b110, b001, b101, b011, b111};
+            const unsigned wts[8] = {ax.w0 * wy0z0, ax.w1 * wy0z0, ax.w0 * wy1z0, ax.w1 * wy1z0,
+                                     ax.w0 * wy0z1, ax.w1 * wy0z1, ax.w0 * wy1z1, ax.w1 * wy1z1};
+            if (fa < rows_smem) {
+                uint32_t* row_ptr = sh_hist + fa * pitch;
+#pragma unroll
+                for (int k = 0; k < 8; ++k)
+                    if (wts[k]) atomicAdd(row_ptr + bins[k], wts[k]);
+            } else {
+                unsigned long long* grow = gh + (size_t)__ldg(a.rank_inv + fa) * nb;
+#pragma unroll
+                for (int k = 0; k < 8; ++k)
+                    if (wts[k]) atomicAdd(grow + bins[k], (unsigned long long)wts[k]);
+            }
+        }
+        __syncthreads();
+        for (int r = warp; r < rows_smem; r += nwarps) {
+            unsigned long long* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
+            for (int b = lane; b < nb; b += 32) {
+                const uint32_t c = sh_hist[r * pitch + b];
+                if (c) {
+                    sh_hist[r * pitch + b] = 0u;
+                    atomicAdd(grow + b, (unsigned long long)c);
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Step a5 on a uint64 histogram whose unit is 2^-15 voxel: counts are scaled back to voxels (an exact
+// division by a power of two), so sum c^q keeps the range argument of include/mi.h (q <= 32).
+__global__ void __launch_bounds__(kEntropyThreads)
+entropy_pv_kernel(const unsigned long long* __restrict__ hist, int nb, const double* __restrict__ q, int nq_total,
+                  int q_off, int nq_pass, int form, double* __restrict__ mi_out, int64_t* __restrict__ nvalid,
+                  const OutMap om) {
+    constexpr int NW = kEntropyThreads / 32;
+    constexpr int NACC = 3 * (1 + kMaxQPerPass);
+    constexpr double kUnit = 1.0 / 32768.0;
+    __shared__ unsigned long long sh_pa[256], sh_pb[256];
+    __shared__ double sh_red[NACC][NW];
+    __shared__ unsigned long long sh_n[NW];
+    const int t = blockIdx.x;
+    const unsigned long long* __restrict__ h = hist + (size_t)t * nb * nb;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double qv[kMaxQPerPass];
+#pragma unroll
+    for (int k = 0; k < kMaxQPerPass; ++k) qv[k] = k < nq_pass ? q[q_off + k] : 1.0;
+    for (int i = threadIdx.x; i < 256; i += kEntropyThreads) { sh_pa[i] = 0ull; sh_pb[i] = 0ull; }
+    __syncthreads();
+    double acc[NACC];
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
+    auto add_terms = [&](unsigned long long c, int which) {
+        const double dv = (double)c * kUnit, lc = log(dv);
+        acc[which] += dv * lc;
+#pragma unroll
+        for (int k = 0; k < kMaxQPerPass; ++k)
+            if (k < nq_pass) acc[3 + 3 * k + which] += exp(qv[k] * lc);
+    };
+    for (int r = warp; r < nb; r += NW) {
+        unsigned long long rowsum = 0ull;
+        for (int c = lane; c < nb; c += 32) {
+            const unsigned long long v = h[(size_t)r * nb + c];
+            if (v) {
+                rowsum += v;
+                atomicAdd(&sh_pb[c], v);
+                add_terms(v, 2);
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) rowsum += __shfl_xor_sync(0xffffffffu, rowsum, o);
+        if (lane == 0) sh_pa[r] = rowsum;
+    }
+    __syncthreads();
+    unsigned long long n_local = 0ull;
+    for (int i = threadIdx.x; i < nb; i += kEntropyThreads) {
+        const unsigned long long ca = sh_pa[i], cb = sh_pb[i];
+        n_local += ca;
+        if (ca) add_terms(ca, 0);
+        if (cb) add_terms(cb, 1);
+    }
+#pragma unroll
+    for (int i = 0; i < NACC; ++i) {
+        const double s = warp_sum_d(acc[i]);
+        if (lane == 0) sh_red[i][warp] = s;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) n_local += __shfl_xor_sync(0xffffffffu, n_local, o);
+    if (lane == 0) sh_n[warp] = n_local;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot[NACC];
+        for (int i = 0; i < NACC; ++i) {
+            double s = 0.0;
+            for (int w = 0; w < NW; ++w) s += sh_red[i][w];
+            tot[i] = s;
+        }
+        unsigned long long n = 0ull;
+        for (int w = 0; w < NW; ++w) n += sh_n[w];
+        entropy_finish(tot, (double)n * kUnit, (long long)(n >> 15), t, qv, nq_pass, q_off, nq_total, form, mi_out,
+                       nvalid, om);
+    }
+}
+
+}  // namespace
+
+cudaError_t launch_pad_replicate_u8(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, cudaStream_t s) {
+    const int64_t total = (int64_t)(nx + 2) * (ny + 2) * (nz + 2);
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
+    pad_replicate_u8_kernel<<<(unsigned)blocks, 256, 0, s>>>(src, dst, nx, ny, nz);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_resample_hist_pv(PvArgs a, int num_sms, cudaStream_t s) {
+    if (a.rows_smem < 1 || a.pitch < a.nb || a.nb > 256) return cudaErrorInvalidConfiguration;
+    const long long nf = (long long)a.f.nx * a.f.ny * a.f.nz;
+    a.nchunks = (int)((nf + kPvChunkVoxels - 1) / kPvChunkVoxels);
+    const long long nitems = (long long)a.n_transforms * a.nchunks;
+    if (nitems < 1) return cudaSuccess;
+    const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
+    cudaError_t e = cudaFuncSetAttribute(resample_hist_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const long long grid = nitems < num_sms ? nitems : num_sms;
+    resample_hist_pv_kernel<<<(unsigned)grid, kHistThreads, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_entropy_pv(const unsigned long long* hist, int nb, int n_transforms, const double* q_dev, int nq,
+                              int q_off, int form, double* mi_out, int64_t* nvalid, OutMap om, cudaStream_t s) {
+    if (n_transforms <= 0) return cudaSuccess;
+    if (nb > 256) return cudaErrorInvalidConfiguration;
+    int nq_pass = nq - q_off;
+    if (nq_pass > kMaxQPerPass) nq_pass = kMaxQPerPass;
+    if (nq_pass < 0) nq_pass = 0;
+    entropy_pv_kernel<<<n_transforms, kEntropyThreads, 0, s>>>(hist, nb, q_dev, nq, q_off, nq_pass, form, mi_out, nvalid, om);
+    return cudaGetLastError();
+}
+
+}  // namespace mi
