@@ -173,11 +173,19 @@ typedef enum {
     MI_OPT_GENERIC_SMEM_KB = 9,    /* shared histogram of the generic kernel in KB (default 196; rest is L1)    */
     MI_OPT_GENERIC_TY_LOG2 = 10,   /* generic kernel row tile: 2^v rows in y x 32/2^v in z (default 3)          */
     MI_OPT_GENERIC_UNROLL = 11,    /* generic kernel voxels in flight per lane, 1..4 (0 = from the row length)  */
+    MI_OPT_ZHIST_MATCH_ANY = 12,   /* 1: the z kernel aggregates equal addresses with __match_any_sync before the shared
+                                      atomic (the scheme BASELINE.json's north_star names) instead of one plain RED per
+                                      lane; slower on B200 (profiles/), kept so the choice stays a measured one  */
+    MI_OPT_GENERIC_GATHER = 13,    /* generic kernel, trilinear: 1 (default) two 16-byte loads per sample from a yz-quad
+                                      copy of the moving volume; 0 eight 4-byte loads from the padded volume        */
     MI_INFO_NUM_SMS = 100,         /* multiprocessors of the context's device                                   */
     MI_INFO_BIN_MODE = 101,        /* binning variant in effect                                                 */
     MI_INFO_ZHIST_ROWS = 102,      /* fixed-bin ranks the z kernel counts in shared memory                      */
     MI_INFO_RARE_VOXELS = 103,     /* fixed voxels of the ranks that do not fit (0 = the epilogue can be fused) */
     MI_INFO_GENERIC_ROWS = 104,    /* fixed-bin ranks the generic kernel counts in shared memory                */
+    MI_INFO_LAST_UPDATES_ISSUED = 106, /* shared-memory histogram updates the z kernel issued in the last call
+                                      (-1 if the call did not take the separable path): evaluations minus the z
+                                      slices that fall outside the moving volume                               */
     MI_INFO_LAST_PATH = 105        /* path of the last call: 0 generic, 1 separable, 2 wide-histogram, 3 partial-volume kernels */
 } mi_option;
 mi_status mi_set_option(mi_ctx *ctx, mi_option key, int64_t value);
@@ -308,6 +316,14 @@ mi_status mi_last_timing(const mi_ctx *ctx, float ms[5], int64_t launches[5]);
  * 2 all lanes on one address.  Host pointers. */
 mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
                                       double *updates_per_s);
+
+/* Gather-rate probe for the roofline of the generic (rotation) path: the resample+histogram kernel of
+ * mi_eval_batch WITHOUT its histogram updates, run on the context's own volumes for the n physical
+ * transforms T (n x 12 doubles, host) with the context's current options; reports fixed-voxel samples per
+ * second (best of `reps` runs after one warm-up).  What it measures is the rate at which L1TEX delivers the
+ * eight neighbours of every trilinear sample -- the term SURVEY.md 8(d) calls t_LSU -- for this data and these
+ * angles; the full kernel adds one shared-memory update per sample on the same load/store pipe. */
+mi_status mi_probe_gather_rate(mi_ctx *ctx, const double *T, int32_t n, int32_t reps, double *samples_per_s);
 
 const char *mi_version(void);
 

@@ -28,15 +28,15 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 
 (MI_OPT_SEPARABLE, MI_OPT_FUSE_ENTROPY, MI_OPT_BIN_MODE_MAX, MI_OPT_ZHIST_ROWS_MAX, MI_OPT_ZHIST_PAD, MI_OPT_XY_BUDGET_MB,
  MI_OPT_SEP_HIST_BUDGET_MB, MI_OPT_HIST_BUDGET_MB, MI_OPT_GENERIC_PAD, MI_OPT_GENERIC_SMEM_KB, MI_OPT_GENERIC_TY_LOG2,
- MI_OPT_GENERIC_UNROLL) = range(12)
+ MI_OPT_GENERIC_UNROLL, MI_OPT_ZHIST_MATCH_ANY, MI_OPT_GENERIC_GATHER) = range(14)
 (MI_INFO_NUM_SMS, MI_INFO_BIN_MODE, MI_INFO_ZHIST_ROWS, MI_INFO_RARE_VOXELS, MI_INFO_GENERIC_ROWS,
- MI_INFO_LAST_PATH) = range(100, 106)
+ MI_INFO_LAST_PATH, MI_INFO_LAST_UPDATES_ISSUED) = range(100, 107)
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_map", "mi_map_range", "mi_set_option",
            "mi_get_option", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
            "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient", "mi_register",
-           "mi_probe_shared_atomic_rate", "mi_version")
+           "mi_probe_shared_atomic_rate", "mi_probe_gather_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError("%s is missing: build it with `python -m paper_1909_10690_b200.build` "
@@ -89,6 +89,8 @@ _lib.mi_last_timing.argtypes = [_vp, _vp, _vp]
 _lib.mi_last_timing.restype = C.c_int
 _lib.mi_probe_shared_atomic_rate.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_int32, _vp]
 _lib.mi_probe_shared_atomic_rate.restype = C.c_int
+_lib.mi_probe_gather_rate.argtypes = [_vp, _vp, C.c_int32, C.c_int32, _vp]
+_lib.mi_probe_gather_rate.restype = C.c_int
 _lib.mi_version.argtypes = []
 _lib.mi_version.restype = C.c_char_p
 
@@ -440,6 +442,15 @@ def mi_release_cached_memory(device=0) -> None:
     st = _lib.mi_release_cached_memory(int(device))
     if st != MI_OK:
         raise MIError(st, "mi_release_cached_memory")
+
+
+def mi_probe_gather_rate(ctx, T, reps=3) -> float:
+    """Samples per second of the generic kernel without its histogram updates on transforms T (n, 3, 4)."""
+    T = _f64(T)
+    n = T.size // 12
+    out = np.zeros(1, dtype=np.float64)
+    _check(ctx, _lib.mi_probe_gather_rate(ctx.handle, _ptr(T), n, int(reps), _ptr(out)))
+    return float(out[0])
 
 
 def mi_probe_shared_atomic_rate(device=0, nbins=256, pattern=1, iters=4096) -> float:

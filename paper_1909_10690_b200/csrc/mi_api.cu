@@ -27,6 +27,7 @@ struct mi_ctx {
     uint8_t* d_rank = nullptr;          // 256: fixed bin -> rank
     int* d_rank_inv = nullptr;          // 256: rank -> fixed bin
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
+    float4* d_moving_quad = nullptr;    // its yz-quads (generic kernel, trilinear): 16 bytes per padded voxel
     uint8_t* d_mbins = nullptr;
     uint8_t* d_mbins_pad = nullptr;     // replicate-padded moving bins (partial-volume interpolation)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
@@ -62,7 +63,9 @@ struct mi_ctx {
     size_t hist_budget = (size_t)1 << 30;  // bytes of global histogram scratch per chunk
     // mi_set_option state (defaults = the measured optimum)
     int opt_zpad = 9, opt_zrows_max = 0, opt_bin_mode_max = mi::kBinFastPrescaled;
-    int opt_gpad = 5, opt_gsmem_kb = 196, opt_unroll = 0;
+    int opt_gpad = 5, opt_gsmem_kb = 196, opt_unroll = 0, opt_match_any = 0, opt_gather = 1;
+    unsigned long long* d_red_count = nullptr;         // histogram updates issued by the z kernel (last call)
+    long long last_reds = 0;
     int bin_mode_natural = mi::kBinGeneral;            // what the data allows (mi_create)
     unsigned long long h_counts[256] = {};             // fixed-bin populations and ranks (nbins <= 256)
     uint8_t h_rank[256] = {};
@@ -442,6 +445,8 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
             z.mi_out = c->d_mi;
             z.nvalid = c->d_nvalid;
             z.om = om;
+            z.match_any = c->opt_match_any;
+            z.red_count = c->d_red_count;
             timer.begin(4);
             MI_CUDA(c, mi::launch_zhist(nn, z, c->num_sms, s));
             timer.end();
@@ -510,7 +515,9 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * helem));
     if (chunk < 1) chunk = 1;
     if (chunk > N) chunk = N;
+    c->last_reds = -1;   // -1: not counted (only the z kernel of the separable path counts its updates)
     if (sep != nullptr) {
+        MI_CUDA(c, cudaMemsetAsync(c->d_red_count, 0, sizeof(unsigned long long), s));
         st = run_separable(c, *sep, nq, interp, timer, hist_out);
         if (st == kSepFallback) sep = nullptr;   // one (p0,p1) pair exceeds the scratch budgets: generic kernel
         else if (st != MI_OK) return st;
@@ -535,6 +542,9 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.rank_inv = c->d_rank_inv;
         a.mask_bits = c->d_mask_bits;
         a.moving_pad = c->d_moving_pad;
+        a.moving_quad = c->d_moving_quad;
+        a.gather = c->opt_gather;
+        a.sink = nullptr;
         a.mbins = c->d_mbins;
         a.rows_smem = c->rows_smem;
         a.pitch = c->gpitch;
@@ -655,7 +665,10 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     if (hist_out != nullptr && !hist_to_user_dev) host_out = true;
     // Host outputs must be complete on return.  The per-class timings need the events anyway, so
     // the call always drains its own work; device outputs stay ordered on the stream.
+    unsigned long long h_reds = 0;
+    if (sep != nullptr) MI_CUDA(c, cudaMemcpyAsync(&h_reds, c->d_red_count, sizeof(h_reds), cudaMemcpyDeviceToHost, s));
     MI_CUDA(c, cudaStreamSynchronize(s));
+    if (sep != nullptr) c->last_reds = (long long)h_reds;
     (void)host_out;
     timer.collect(c->last_ms);
     return MI_OK;
@@ -761,6 +774,7 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         c->colpitch = (int)(((int64_t)fixed_dims[0] * fixed_dims[1] + mi::kZColAlign - 1) / mi::kZColAlign * mi::kZColAlign);
         if ((e = dev_alloc((void**)&c->d_fb_pitched, (size_t)c->colpitch * fixed_dims[2] + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc pitched bins"); break; }
         c->separable_ok = nbins <= 256 && fixed_dims[2] <= 65535;   // the rare list packs iz into 16 bits
+        if ((e = dev_alloc((void**)&c->d_red_count, sizeof(unsigned long long), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc counter"); break; }
         if ((e = cudaEventCreateWithFlags(&c->ev_staging, cudaEventDisableTiming)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaEventCreate"); break; }
         cudaStream_t s = c->stream;
         if ((e = cudaMemcpyAsync(d_tmp, fixed, (size_t)nf * sizeof(float), cudaMemcpyDefault, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy fixed"); break; }
@@ -796,6 +810,10 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             if ((e = mi::launch_pad_replicate_u8(c->d_mbins, c->d_mbins_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving bins"); break; }
         }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
+        if (!c->wide) {
+            if ((e = dev_alloc((void**)&c->d_moving_quad, (size_t)npad * sizeof(float4), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving quads"); break; }
+            if ((e = mi::launch_quad_build(c->d_moving_pad, c->d_moving_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving quads"); break; }
+        }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
     dev_free(d_tmp, c->stream);
@@ -814,7 +832,7 @@ void mi_destroy(mi_ctx* c) {
     DeviceGuard guard(c->device);
     if (guard.ok) {
         void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mask_bits, c->d_fbins16, c->d_mbins16, c->d_mbins,
-                        c->d_mbins_pad, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
+                        c->d_mbins_pad, c->d_moving_quad, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);
@@ -907,6 +925,10 @@ mi_status mi_set_option(mi_ctx* c, mi_option key, int64_t v) {
     case MI_OPT_GENERIC_UNROLL:
         if (v < 0 || v > 4) return bad();
         c->opt_unroll = (int)v; break;
+    case MI_OPT_ZHIST_MATCH_ANY: c->opt_match_any = v != 0; break;
+    case MI_OPT_GENERIC_GATHER:
+        if (v < 0 || v > 1) return bad();
+        c->opt_gather = (int)v; break;
     default:
         return fail(c, MI_ERR_INVALID_ARG, "mi_set_option: unknown or read-only key");
     }
@@ -931,6 +953,9 @@ mi_status mi_get_option(const mi_ctx* c, mi_option key, int64_t* out) {
     case MI_OPT_GENERIC_SMEM_KB: *out = c->opt_gsmem_kb; break;
     case MI_OPT_GENERIC_TY_LOG2: *out = c->ty_log2; break;
     case MI_OPT_GENERIC_UNROLL: *out = c->opt_unroll; break;
+    case MI_OPT_ZHIST_MATCH_ANY: *out = c->opt_match_any; break;
+    case MI_OPT_GENERIC_GATHER: *out = c->opt_gather; break;
+    case MI_INFO_LAST_UPDATES_ISSUED: *out = c->last_reds; break;
     case MI_INFO_NUM_SMS: *out = c->num_sms; break;
     case MI_INFO_BIN_MODE: *out = c->bin_mode; break;
     case MI_INFO_ZHIST_ROWS: *out = c->wide ? 0 : c->zrows_real; break;
@@ -1197,6 +1222,67 @@ mi_status mi_last_timing(const mi_ctx* c, float ms[5], int64_t launches[5]) {
         if (ms) ms[k] = c->last_ms[k];
         if (launches) launches[k] = c->last_launches[k];
     }
+    return MI_OK;
+}
+
+mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms, int32_t reps, double* samples_per_s) {
+    if (!c) return MI_ERR_INVALID_ARG;
+    if (!T || !samples_per_s || n_transforms < 1 || n_transforms > (1 << 20) || reps < 1)
+        return fail(c, MI_ERR_INVALID_ARG, "mi_probe_gather_rate: bad argument");
+    if (c->wide) return fail(c, MI_ERR_UNSUPPORTED, "mi_probe_gather_rate needs nbins <= 256");
+    std::vector<float> hM((size_t)n_transforms * 12);
+    for (int t = 0; t < n_transforms; ++t) {
+        for (int i = 0; i < 12; ++i)
+            if (!std::isfinite(T[(size_t)t * 12 + i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite matrix entry");
+        mi::index_affine(T + (size_t)t * 12, c->fd, c->fs, c->md, c->ms, hM.data() + (size_t)t * 12);
+    }
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
+    cudaStream_t s = c->stream;
+    mi_status st;
+    if ((st = grow(c, &c->d_M, &c->cap_M, (size_t)n_transforms * 12)) != MI_OK) return st;
+    MI_CUDA(c, cudaMemcpyAsync(c->d_M, hM.data(), hM.size() * sizeof(float), cudaMemcpyHostToDevice, s));
+    MI_CUDA(c, cudaMemsetAsync(c->d_red_count, 0, sizeof(unsigned long long), s));
+    mi::ResampleArgs a;
+    a.fbins_ranked = c->d_fbins_ranked;
+    a.rank_inv = c->d_rank_inv;
+    a.mask_bits = c->d_mask_bits;
+    a.moving_pad = c->d_moving_pad;
+    a.moving_quad = c->d_moving_quad;
+    a.gather = c->opt_gather;
+    a.sink = reinterpret_cast<unsigned*>(c->d_red_count);
+    a.mbins = c->d_mbins;
+    a.rows_smem = c->rows_smem;      // the probe keeps the kernel's shared-memory size: same L1 carve-out
+    a.pitch = c->gpitch;
+    a.ty_log2 = c->ty_log2;
+    a.unroll = c->opt_unroll;
+    a.M = c->d_M;
+    a.hist = nullptr;
+    a.f = {c->fd[0], c->fd[1], c->fd[2]};
+    a.m = {c->md[0], c->md[1], c->md[2]};
+    a.nb = c->nb;
+    a.mlo = c->mlo;
+    a.mscale = c->mscale;
+    a.n_transforms = n_transforms;
+    a.nslabs = 1;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    MI_CUDA(c, cudaEventCreate(&e0));
+    MI_CUDA(c, cudaEventCreate(&e1));
+    float best = 1e30f;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep <= reps && e == cudaSuccess; ++rep) {   // the first run warms up
+        cudaEventRecord(e0, s);
+        e = mi::launch_resample_hist(a, MI_INTERP_TRILINEAR, c->num_sms, s);
+        cudaEventRecord(e1, s);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (e != cudaSuccess) return cuda_fail(c, e, "gather probe");
+    *samples_per_s = (double)c->nf * n_transforms / (best * 1e-3);
     return MI_OK;
 }
 

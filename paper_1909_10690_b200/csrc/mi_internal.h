@@ -40,6 +40,9 @@ struct ResampleArgs {
     const int* rank_inv;          // rank -> fixed bin
     const uint32_t* mask_bits;    // NULL, or one bit per fixed voxel (flat index): 0 = the voxel takes no part
     const float* moving_pad;      // replicate-padded moving float32, dims (mx+2, my+2, mz+2)
+    const float4* moving_quad;    // yz-quads of the padded volume (same dims), or NULL
+    int gather;                   // trilinear gather scheme: 0 eight 4-byte loads, 1 two 16-byte quad loads
+    unsigned* sink;               // NULL; or (roofline probe) no histogram is built, bins are summed here
     const uint8_t* mbins;         // moving bin indices (nearest neighbour), unpadded
     const float* M;               // n_transforms x 12 index-space affines (device)
     uint32_t* hist;               // n_transforms x nb x nb (row = fixed bin), zero on entry
@@ -58,6 +61,7 @@ struct ResampleArgs {
 cudaError_t launch_prebin(const float* vol, uint8_t* bins, int64_t n, float lo, float scale, int nb,
                           unsigned* flag, cudaStream_t s);
 cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, int nz, cudaStream_t s);
+cudaError_t launch_quad_build(const float* pad, float4* quad, int nx, int ny, int nz, cudaStream_t s);
 cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
                                    uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s);
 int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes);
@@ -140,6 +144,8 @@ struct ZHistArgs {
     double* mi_out;
     int64_t* nvalid;
     OutMap om;
+    int match_any;                  // 1: __match_any_sync aggregation instead of the plain RED (measurement option)
+    unsigned long long* red_count;  // NULL, or device counter of the histogram updates issued
 };
 // Moving-side binning variants of the z kernel (CANON-5, t = (v - mlo) * mscale, clamp, floor):
 //   kBinGeneral        the full sequence

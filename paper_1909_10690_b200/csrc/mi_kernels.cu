@@ -111,6 +111,32 @@ cudaError_t launch_pad_replicate(const float* src, float* dst, int nx, int ny, i
     return cudaGetLastError();
 }
 
+// yz-quads of the padded moving volume: quad[z][y][x] = {pad[z][y][x], pad[z][y+1][x], pad[z+1][y][x],
+// pad[z+1][y+1][x]} (indices clamped to the padded volume: the last row / plane is never a cell's base).  The
+// 2x2x2 cell at padded base index i is then quad[i] (its x = jx face) and quad[i + 1] (its x = jx + 1 face): two
+// adjacent 16-byte loads instead of eight 4-byte gathers -- the four values of a face travel together, and the
+// 32 lanes of a warp (consecutive x) read 512 contiguous bytes per load when the row stays in one moving row.
+__global__ void __launch_bounds__(256) quad_build_kernel(const float* __restrict__ pad, float4* __restrict__ quad,
+                                                         int px, int py, int pz) {
+    const int64_t total = (int64_t)px * py * pz;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % px);
+        const int64_t r = i / px;
+        const int y = (int)(r % py), z = (int)(r / py);
+        const int y1 = min(y + 1, py - 1), z1 = min(z + 1, pz - 1);
+        quad[i] = make_float4(pad[((int64_t)z * py + y) * px + x], pad[((int64_t)z * py + y1) * px + x],
+                              pad[((int64_t)z1 * py + y) * px + x], pad[((int64_t)z1 * py + y1) * px + x]);
+    }
+}
+
+cudaError_t launch_quad_build(const float* pad, float4* quad, int nx, int ny, int nz, cudaStream_t s) {
+    const int64_t total = (int64_t)(nx + 2) * (ny + 2) * (nz + 2);
+    int64_t blocks = (total + 255) / 256;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
+    quad_build_kernel<<<(unsigned)blocks, 256, 0, s>>>(pad, quad, nx + 2, ny + 2, nz + 2);
+    return cudaGetLastError();
+}
+
 // One bit per voxel from a byte mask (bit i of word i/32 = mask[i] != 0).
 __global__ void __launch_bounds__(256) mask_bits_kernel(const uint8_t* __restrict__ mask, int64_t n,
                                                         uint32_t* __restrict__ bits) {
@@ -210,6 +236,7 @@ struct MovingView {
     const float* __restrict__ pad_y;   // pad + (nx+2)
     const float* __restrict__ pad_z;   // pad + (nx+2)*(ny+2)
     const float* __restrict__ pad_yz;  // pad + (nx+2)*(ny+2) + (nx+2)
+    const float4* __restrict__ quad;   // yz-quads of the padded volume (quad_build_kernel)
     const uint8_t* __restrict__ bins;  // unpadded bin volume (nearest neighbour)
     int nx, ny;                        // unpadded dims (nearest neighbour indexing)
     int pnx, pny;                      // padded dims
@@ -220,7 +247,11 @@ struct MovingView {
     int top;                           // nb - 1
 };
 
-template <int INTERP>
+// GATHER (trilinear): kGatherScalar = eight 4-byte loads from the padded volume; kGatherQuad = two adjacent
+// 16-byte loads from the yz-quad volume (same eight floats, same lerp sequence).
+enum { kGatherScalar = 0, kGatherQuad = 1 };
+
+template <int INTERP, int GATHER>
 __device__ __forceinline__ Sample sample_bin(const MovingView& mv, float cx, float cy, float cz) {
     Sample s;
     if (INTERP == MI_INTERP_NEAREST) {
@@ -245,10 +276,17 @@ __device__ __forceinline__ Sample sample_bin(const MovingView& mv, float cx, flo
         unsigned idx = (__float_as_uint(tz) * (unsigned)mv.pny + __float_as_uint(ty)) * (unsigned)mv.pnx +
                        __float_as_uint(tx) - mv.fold;
         idx = s.ok ? idx : 0u;
-        const float a000 = __ldg(mv.pad + idx), a100 = __ldg(mv.pad + idx + 1);
-        const float a010 = __ldg(mv.pad_y + idx), a110 = __ldg(mv.pad_y + idx + 1);
-        const float a001 = __ldg(mv.pad_z + idx), a101 = __ldg(mv.pad_z + idx + 1);
-        const float a011 = __ldg(mv.pad_yz + idx), a111 = __ldg(mv.pad_yz + idx + 1);
+        float a000, a100, a010, a110, a001, a101, a011, a111;
+        if (GATHER == kGatherQuad) {
+            const float4 q0 = __ldg(mv.quad + idx), q1 = __ldg(mv.quad + idx + 1);
+            a000 = q0.x; a010 = q0.y; a001 = q0.z; a011 = q0.w;
+            a100 = q1.x; a110 = q1.y; a101 = q1.z; a111 = q1.w;
+        } else {
+            a000 = __ldg(mv.pad + idx); a100 = __ldg(mv.pad + idx + 1);
+            a010 = __ldg(mv.pad_y + idx); a110 = __ldg(mv.pad_y + idx + 1);
+            a001 = __ldg(mv.pad_z + idx); a101 = __ldg(mv.pad_z + idx + 1);
+            a011 = __ldg(mv.pad_yz + idx); a111 = __ldg(mv.pad_yz + idx + 1);
+        }
         const float v00 = lerp_rn(a000, a100, wx);
         const float v10 = lerp_rn(a010, a110, wx);
         const float v01 = lerp_rn(a001, a101, wx);
@@ -268,7 +306,9 @@ __device__ __forceinline__ Sample sample_bin(const MovingView& mv, float cx, flo
 // see profiles/).  Fixed bins arrive RANKED by population: the `rows_smem` most populated fixed-bin
 // rows are in shared memory, the rare tail (only when nb*nb*4 B exceeds shared memory, i.e. 256
 // bins) is added straight to the global histogram.
-template <int INTERP, int UNROLL>
+// HIST = false is the roofline probe (mi_probe_gather_rate): the same kernel without the histogram updates --
+// the moving bins are summed into a.sink instead -- i.e. the rate at which L1TEX delivers the samples.
+template <int INTERP, int UNROLL, int GATHER, bool HIST>
 __global__ void __launch_bounds__(kHistThreads, 1)
 resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     extern __shared__ __align__(16) uint32_t sh_hist[];
@@ -298,6 +338,7 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     mv.pad_y = a.moving_pad + mv.pnx;
     mv.pad_z = a.moving_pad + (size_t)mv.pnx * mv.pny;
     mv.pad_yz = mv.pad_z + mv.pnx;
+    mv.quad = a.moving_quad;
     mv.bins = a.mbins;
     mv.nx = a.m.nx; mv.ny = a.m.ny;
     // padded index of cell (jx+1, jy+1, jz+1) from the raw float bits T_k = magic + j_k:
@@ -307,6 +348,7 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     mv.hx = __fsub_rn(mv.fx, 0.5f); mv.hy = __fsub_rn(mv.fy, 0.5f); mv.hz = __fsub_rn(mv.fz, 0.5f);
     mv.lo = a.mlo; mv.scale = a.mscale; mv.top = nb - 1;
 
+    unsigned probe_acc = 0u;
     const long long nitems = (long long)a.n_transforms * a.nslabs;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int t = (int)(item / a.nslabs);
@@ -340,7 +382,7 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
                     const float cx = __fmaf_rn(m[0], fx, rx);
                     const float cy = __fmaf_rn(m[4], fx, ry);
                     const float cz = __fmaf_rn(m[8], fx, rz);
-                    smp[u] = sample_bin<INTERP>(mv, cx, cy, cz);
+                    smp[u] = sample_bin<INTERP, GATHER>(mv, cx, cy, cz);
                     smp[u].ok = smp[u].ok && (ix0 + 32 * u < fnx);
                     if (a.mask_bits != nullptr) {
                         const unsigned vi = (unsigned)row * (unsigned)fnx + (unsigned)ix;
@@ -351,12 +393,14 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
 #pragma unroll
                 for (int u = 0; u < UNROLL; ++u) {
                     if (smp[u].ok) {
-                        if (fa[u] < rows_smem) atomicAdd(&sh_hist[fa[u] * pitch + smp[u].b], 1u);
+                        if (!HIST) probe_acc += (unsigned)(fa[u] * pitch + smp[u].b);
+                        else if (fa[u] < rows_smem) atomicAdd(&sh_hist[fa[u] * pitch + smp[u].b], 1u);
                         else atomicAdd(&gh[__ldg(a.rank_inv + fa[u]) * nb + smp[u].b], 1u);
                     }
                 }
             }
         }
+        if (!HIST) continue;
         __syncthreads();
         // merge the CTA-private rows into the transform's global histogram (un-ranking the fixed
         // bin) and re-zero them for the next item
@@ -372,12 +416,16 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
         }
         __syncthreads();
     }
+    if (!HIST) {
+        probe_acc = warp_sum(probe_acc);
+        if (lane == 0) atomicAdd(a.sink, probe_acc);
+    }
 }
 
-template <int INTERP, int UNROLL>
+template <int INTERP, int UNROLL, int GATHER, bool HIST>
 static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStream_t s) {
     const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
-    auto kern = resample_hist_kernel<INTERP, UNROLL>;
+    auto kern = resample_hist_kernel<INTERP, UNROLL, GATHER, HIST>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     // leave the rest of the SM's 256 KB to L1 (the gathers live there)
@@ -416,15 +464,27 @@ cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms,
         }
     }
     if (interp == MI_INTERP_NEAREST) {
-        if (unroll == 1) return launch_resample_t<MI_INTERP_NEAREST, 1>(a, num_sms, s);
-        if (unroll == 2) return launch_resample_t<MI_INTERP_NEAREST, 2>(a, num_sms, s);
-        if (unroll == 3) return launch_resample_t<MI_INTERP_NEAREST, 3>(a, num_sms, s);
-        return launch_resample_t<MI_INTERP_NEAREST, 4>(a, num_sms, s);
+        if (a.sink != nullptr) return cudaErrorInvalidConfiguration;
+        if (unroll == 1) return launch_resample_t<MI_INTERP_NEAREST, 1, kGatherScalar, true>(a, num_sms, s);
+        if (unroll == 2) return launch_resample_t<MI_INTERP_NEAREST, 2, kGatherScalar, true>(a, num_sms, s);
+        if (unroll == 3) return launch_resample_t<MI_INTERP_NEAREST, 3, kGatherScalar, true>(a, num_sms, s);
+        return launch_resample_t<MI_INTERP_NEAREST, 4, kGatherScalar, true>(a, num_sms, s);
     }
-    if (unroll == 1) return launch_resample_t<MI_INTERP_TRILINEAR, 1>(a, num_sms, s);
-    if (unroll == 2) return launch_resample_t<MI_INTERP_TRILINEAR, 2>(a, num_sms, s);
-    if (unroll == 3) return launch_resample_t<MI_INTERP_TRILINEAR, 3>(a, num_sms, s);
-    return launch_resample_t<MI_INTERP_TRILINEAR, 4>(a, num_sms, s);
+#define MI_TRI(G, H)                                                                                  \
+    do {                                                                                              \
+        if (unroll == 1) return launch_resample_t<MI_INTERP_TRILINEAR, 1, G, H>(a, num_sms, s);       \
+        if (unroll == 2) return launch_resample_t<MI_INTERP_TRILINEAR, 2, G, H>(a, num_sms, s);       \
+        if (unroll == 3) return launch_resample_t<MI_INTERP_TRILINEAR, 3, G, H>(a, num_sms, s);       \
+        return launch_resample_t<MI_INTERP_TRILINEAR, 4, G, H>(a, num_sms, s);                        \
+    } while (0)
+    const bool quad = a.gather == kGatherQuad && a.moving_quad != nullptr;
+    if (a.sink != nullptr) {   // roofline probe: no histogram
+        if (quad) MI_TRI(kGatherQuad, false);
+        MI_TRI(kGatherScalar, false);
+    }
+    if (quad) MI_TRI(kGatherQuad, true);
+    MI_TRI(kGatherScalar, true);
+#undef MI_TRI
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -181,6 +181,19 @@ __device__ __forceinline__ uint32_t ld_u32(const uint8_t* p) { return __ldg(rein
 __device__ __forceinline__ void red_shared_inc(unsigned addr) {
     asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
 }
+// The alternative BASELINE.json's north_star names: software warp aggregation -- the lanes that hit the same
+// counter are found with __match_any_sync and their leader adds the group's size.  Kept as an option
+// (MI_OPT_ZHIST_MATCH_ANY) so that the choice of the plain RED stays a measured one (profiles/).
+__device__ __forceinline__ void match_any_inc(unsigned addr) {
+    const unsigned active = __activemask();
+    const unsigned peers = __match_any_sync(active, addr);
+    if ((unsigned)(threadIdx.x & 31) == (unsigned)(__ffs(peers) - 1))
+        asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(addr), "r"((unsigned)__popc(peers)) : "memory");
+}
+template <bool AGG>
+__device__ __forceinline__ void hist_inc(unsigned addr) {
+    if (AGG) match_any_inc(addr); else red_shared_inc(addr);
+}
 
 __device__ __forceinline__ unsigned warp_sum_u(unsigned v) {
 #pragma unroll
@@ -367,7 +380,7 @@ __device__ __forceinline__ void zhist_entropy_epilogue(const ZHistArgs& a, long 
 // of both marginals in double, then eq. 2 and its Tsallis forms, written to the
 // item's position in the map.  Entropies do not depend on the order of the bins, so the ranked rows
 // are used as they are.
-template <bool NN, int MODE>
+template <bool NN, int MODE, bool AGG>
 __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_constant__ ZHistArgs a) {
     extern __shared__ __align__(16) uint32_t sh_raw[];
     int* run_hi = reinterpret_cast<int*>(sh_raw);
@@ -391,6 +404,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
     const unsigned cbase = sbase - 4u * (unsigned)kMagicBits;   // modulo 2^32
     const float mlo = a.mlo, mscale = a.mscale;
+    unsigned long long issued = 0ull;   // histogram updates this thread issued (a.red_count)
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int pair = (int)(item / a.n2);
@@ -434,6 +448,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                     dump.w[j] = (~keep.w[j]) & ((uint32_t)a.rows_real * 0x01010101u);
                 }
                 if (any == 0u) continue;
+                issued += (unsigned long long)(kZCols * (iz_hi - iz_lo));
                 const uint8_t* __restrict__ fbq = a.fb + (size_t)iz_lo * colpitch + col0;
                 Bins fa_next;
                 ld_bins(fa_next, fbq);
@@ -454,7 +469,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                             if (iz + 1 < iz_hi) ld_bins(fa_next, fbq);
 #pragma unroll
                             for (int k = 0; k < kZCols; ++k)
-                                red_shared_inc(sbase + (byte_of(fa.w[k / 4], k & 3) * pitch + byte_of(v.w[k / 4], k & 3)) * 4u);
+                                hist_inc<AGG>(sbase + (byte_of(fa.w[k / 4], k & 3) * pitch + byte_of(v.w[k / 4], k & 3)) * 4u);
                         }
                     }
                 } else {
@@ -498,7 +513,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                                 }
                                 const unsigned mbits = byte_of(fa.w[k / 4], k & 3) * pitch + (unsigned)kMagicBits;
                                 const float r = __fadd_rd(t, __uint_as_float(mbits));
-                                red_shared_inc(__float_as_uint(r) * 4u + cbase);
+                                hist_inc<AGG>(__float_as_uint(r) * 4u + cbase);
                             }
                         }
                         ++p;
@@ -548,6 +563,11 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
         if (a.rows_real < rows_smem)   // the dump row is only re-zeroed
             for (unsigned b = threadIdx.x; b <= nb; b += blockDim.x) sh_hist[a.rows_real * pitch + b] = 0u;
         __syncthreads();
+    }
+    if (a.red_count != nullptr) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) issued += __shfl_xor_sync(0xffffffffu, issued, o);
+        if (lane == 0 && issued) atomicAdd(a.red_count, issued);
     }
 }
 
@@ -666,9 +686,9 @@ int zhist_rows_in_smem(int nb, int pitch, int fnz, int planes, size_t smem_optin
     return (int)rows;
 }
 
-template <bool NN, int MODE>
+template <bool NN, int MODE, bool AGG>
 static cudaError_t launch_zhist_t(const ZHistArgs& a, unsigned grid, size_t smem, cudaStream_t s) {
-    auto kern = zhist_kernel<NN, MODE>;
+    auto kern = zhist_kernel<NN, MODE, AGG>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     kern<<<grid, kHistThreads, smem, s>>>(a);
@@ -685,10 +705,15 @@ cudaError_t launch_zhist(bool nn, const ZHistArgs& a, int num_sms, cudaStream_t 
     if (grid < 1) return cudaSuccess;
     cudaError_t e;
     const unsigned g = (unsigned)grid;
-    if (nn) e = launch_zhist_t<true, kBinGeneral>(a, g, smem, s);
-    else if (a.bin_mode == kBinFastPrescaled) e = launch_zhist_t<false, kBinFastPrescaled>(a, g, smem, s);
-    else if (a.bin_mode == kBinFast) e = launch_zhist_t<false, kBinFast>(a, g, smem, s);
-    else e = launch_zhist_t<false, kBinGeneral>(a, g, smem, s);
+    if (a.match_any) {
+        if (nn) e = launch_zhist_t<true, kBinGeneral, true>(a, g, smem, s);
+        else if (a.bin_mode == kBinFastPrescaled) e = launch_zhist_t<false, kBinFastPrescaled, true>(a, g, smem, s);
+        else if (a.bin_mode == kBinFast) e = launch_zhist_t<false, kBinFast, true>(a, g, smem, s);
+        else e = launch_zhist_t<false, kBinGeneral, true>(a, g, smem, s);
+    } else if (nn) e = launch_zhist_t<true, kBinGeneral, false>(a, g, smem, s);
+    else if (a.bin_mode == kBinFastPrescaled) e = launch_zhist_t<false, kBinFastPrescaled, false>(a, g, smem, s);
+    else if (a.bin_mode == kBinFast) e = launch_zhist_t<false, kBinFast, false>(a, g, smem, s);
+    else e = launch_zhist_t<false, kBinGeneral, false>(a, g, smem, s);
     if (e != cudaSuccess) return e;
     if (a.n_rare > 0) {
         long long g2 = nitems < 8LL * num_sms ? nitems : 8LL * num_sms;
