@@ -178,6 +178,9 @@ typedef enum {
                                       lane; slower on B200 (profiles/), kept so the choice stays a measured one  */
     MI_OPT_GENERIC_GATHER = 13,    /* generic kernel, trilinear: 1 (default) two 16-byte loads per sample from a yz-quad
                                       copy of the moving volume; 0 eight 4-byte loads from the padded volume        */
+    MI_OPT_GENERIC_THREADS = 14,   /* CTA size of the quad-gather kernel: 512, 768 or 1024 (default)               */
+    MI_OPT_GENERIC_SLAB_MB = 15,   /* quad-gather kernel: z slabs of the fixed volume sized so that a slab's share of
+                                      the quad volume is at most this many MB (default 16; 0 = one slab)           */
     MI_INFO_NUM_SMS = 100,         /* multiprocessors of the context's device                                   */
     MI_INFO_BIN_MODE = 101,        /* binning variant in effect                                                 */
     MI_INFO_ZHIST_ROWS = 102,      /* fixed-bin ranks the z kernel counts in shared memory                      */
@@ -224,6 +227,14 @@ const char *mi_last_error(const mi_ctx *ctx);
 
 /* Host side: physical 3x4 [A|t] of the nine parameters. */
 mi_status mi_compose_matrix(const double p[9], double T_out[12]);
+
+/* The hand-off "coarse exhaustive map -> gradient ascent" (an exhaustive search is the robust
+ * way to start; then the multi-metric gradient): the nine parameters of the map node with
+ * linear index `index` (an argmax_out of mi_map) on the grid (lo, hi, n) of `family`, identity in the other
+ * parameter groups -- the p0 of mi_register.  Translation / Euler / scale nodes are copied, log-scale nodes
+ * become factors exp(p), versor nodes the Euler angles of their rotation matrix.  Host pointers. */
+mi_status mi_seed_from_map(mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
+                           int64_t index, double p_out[9]);
 
 /* delta[k] <= 0 skips component k (grad_out[k] = 0).  grad_out: 9 doubles; value_out: NULL or 2
  * doubles (Shannon, Tsallis_q at p).  Host pointers; q > 0 and finite. */

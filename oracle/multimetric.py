@@ -68,6 +68,36 @@ def multimetric_gradient(fixed, fixed_spacing, moving, moving_spacing, nbins, ra
     return grad, vals[0].copy()
 
 
+def seed_from_map(family, lo, hi, n, index) -> np.ndarray:
+    """Hand-off from an exhaustive map to `register` (reading A22; "exhaustive search over all the parameters"
+    as the robust start, then the multi-metric gradient of PAPER.md:199, 210): the nine parameters
+    of the map node with linear index `index` (p0 fastest) on the grid (lo, hi, n) of `family`, identity in the
+    other groups.  Node k of axis d is lo + k (hi - lo)/(n - 1) as everywhere.  Translation / Euler / scale
+    nodes are copied; log-scale nodes become factors exp(p); a versor node becomes the Euler angles of its
+    rotation matrix R = Rz Ry Rx: ay = -asin(R20), ax = atan2(R21, R22), az = atan2(R10, R00)."""
+    n = [int(v) for v in n]
+    k = (index % n[0], (index // n[0]) % n[1], index // (n[0] * n[1]))
+    node = [float(lo[d]) if n[d] == 1 else float(lo[d]) + float(k[d]) * (float(hi[d]) - float(lo[d])) / float(n[d] - 1)
+            for d in range(3)]
+    p = np.array([0, 0, 0, 0, 0, 0, 1, 1, 1], dtype=np.float64)
+    if family == _orc.FAMILY_TRANSLATION:
+        p[0:3] = node
+    elif family == _orc.FAMILY_ROTATION_EULER_DEG:
+        p[3:6] = node
+    elif family == _orc.FAMILY_SCALE:
+        p[6:9] = node
+    elif family == _orc.FAMILY_SCALE_LOG:
+        p[6:9] = np.exp(np.asarray(node))
+    elif family == _orc.FAMILY_ROTATION_VERSOR:
+        R = _orc.family_matrix(family, node)[:, :3]
+        p[4] = np.degrees(np.arcsin(min(1.0, max(-1.0, -R[2, 0]))))
+        p[3] = np.degrees(np.arctan2(R[2, 1], R[2, 2]))
+        p[5] = np.degrees(np.arctan2(R[1, 0], R[0, 0]))
+    else:
+        raise ValueError("unknown family %r" % (family,))
+    return p
+
+
 GROUPS = ((0, 1, 2), (3, 4, 5), (6, 7, 8))      # translation [mm], rotation [deg], scale [factor]
 
 

@@ -7,7 +7,7 @@ function without the built CUDA library raises.  `phantoms` is the seeded input 
 """
 _API = ("mi_create", "mi_destroy", "mi_eval_batch", "mi_eval_batch_pv", "mi_map", "mi_map_range", "mi_set_option", "mi_get_option", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_last_error",
         "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
-        "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient", "mi_register", "mi_probe_shared_atomic_rate", "mi_probe_gather_rate", "mi_version", "MIContext", "MIError")
+        "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_seed_from_map", "mi_multimetric_gradient", "mi_register", "mi_probe_shared_atomic_rate", "mi_probe_gather_rate", "mi_version", "MIContext", "MIError")
 
 
 def __getattr__(name):

@@ -28,14 +28,15 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 
 (MI_OPT_SEPARABLE, MI_OPT_FUSE_ENTROPY, MI_OPT_BIN_MODE_MAX, MI_OPT_ZHIST_ROWS_MAX, MI_OPT_ZHIST_PAD, MI_OPT_XY_BUDGET_MB,
  MI_OPT_SEP_HIST_BUDGET_MB, MI_OPT_HIST_BUDGET_MB, MI_OPT_GENERIC_PAD, MI_OPT_GENERIC_SMEM_KB, MI_OPT_GENERIC_TY_LOG2,
- MI_OPT_GENERIC_UNROLL, MI_OPT_ZHIST_MATCH_ANY, MI_OPT_GENERIC_GATHER) = range(14)
+ MI_OPT_GENERIC_UNROLL, MI_OPT_ZHIST_MATCH_ANY, MI_OPT_GENERIC_GATHER, MI_OPT_GENERIC_THREADS,
+ MI_OPT_GENERIC_SLAB_MB) = range(16)
 (MI_INFO_NUM_SMS, MI_INFO_BIN_MODE, MI_INFO_ZHIST_ROWS, MI_INFO_RARE_VOXELS, MI_INFO_GENERIC_ROWS,
  MI_INFO_LAST_PATH, MI_INFO_LAST_UPDATES_ISSUED) = range(100, 107)
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_map", "mi_map_range", "mi_set_option",
            "mi_get_option", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
-           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_multimetric_gradient", "mi_register",
+           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_seed_from_map", "mi_multimetric_gradient", "mi_register",
            "mi_probe_shared_atomic_rate", "mi_probe_gather_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
@@ -75,6 +76,8 @@ _lib.mi_get_bins.argtypes = [_vp, C.c_int32, _vp]
 _lib.mi_get_bins.restype = C.c_int
 _lib.mi_release_cached_memory.argtypes = [C.c_int32]
 _lib.mi_release_cached_memory.restype = C.c_int
+_lib.mi_seed_from_map.argtypes = [C.c_int, _vp, _vp, _vp, C.c_int64, _vp]
+_lib.mi_seed_from_map.restype = C.c_int
 _lib.mi_compose_matrix.argtypes = [_vp, _vp]
 _lib.mi_compose_matrix.restype = C.c_int
 _lib.mi_multimetric_gradient.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp]
@@ -402,6 +405,16 @@ def mi_set_fixed_mask(ctx, mask) -> None:
         m = np.ascontiguousarray(np.asarray(mask) != 0, dtype=np.uint8)
     assert tuple(m.shape) == ctx.fixed_dims[::-1]
     _check(ctx, _lib.mi_set_fixed_mask(ctx.handle, _ptr(m)))
+
+
+def mi_seed_from_map(family, lo, hi, n, index) -> np.ndarray:
+    """Nine registration parameters of map node `index` (e.g. an arg max of mi_map): the p0 of mi_register."""
+    lo, hi, n = _f64(lo, 3), _f64(hi, 3), _i32(n, 3)
+    p = np.empty(9, dtype=np.float64)
+    st = _lib.mi_seed_from_map(int(family), _ptr(lo), _ptr(hi), _ptr(n), int(index), _ptr(p))
+    if st != MI_OK:
+        raise MIError(st, "mi_seed_from_map")
+    return p
 
 
 def mi_compose_matrix(p) -> np.ndarray:

@@ -63,9 +63,10 @@ struct mi_ctx {
     size_t hist_budget = (size_t)1 << 30;  // bytes of global histogram scratch per chunk
     // mi_set_option state (defaults = the measured optimum)
     int opt_zpad = 9, opt_zrows_max = 0, opt_bin_mode_max = mi::kBinFastPrescaled;
-    int opt_gpad = 5, opt_gsmem_kb = 196, opt_unroll = 0, opt_match_any = 0, opt_gather = 1;
+    int opt_gpad = 5, opt_gsmem_kb = 196, opt_unroll = 0, opt_match_any = 0, opt_gather = 1, opt_gthreads = 1024, opt_slab_mb = 16;
     unsigned long long* d_red_count = nullptr;         // histogram updates issued by the z kernel (last call)
     long long last_reds = 0;
+    bool generic_has_rare = true;                      // a populated fixed-bin rank has no shared row in the generic kernel
     int bin_mode_natural = mi::kBinGeneral;            // what the data allows (mi_create)
     unsigned long long h_counts[256] = {};             // fixed-bin populations and ranks (nbins <= 256)
     uint8_t h_rank[256] = {};
@@ -119,11 +120,18 @@ cudaError_t device_pool(int dev, cudaMemPool_t* out) {
 }
 
 // Stream-ordered allocation on the context's stream (every use of the memory is ordered on it too).
+// Sizes are rounded up to 2 MB, so every buffer starts on a 2 MB boundary whatever was allocated before it.
+// This is a measured requirement, not tidiness: the z kernel streams three pitched arrays (xy planes, fixed bins,
+// column flags) and its time depends on where they sit relative to each other -- one extra 8-byte allocation
+// early in mi_create, which shifted everything behind it by 512 bytes, cost 21 % of the headline step (773 ms
+// against 636 ms, the CTAs on three SMs running 8-22 % longer, round 2).
 cudaError_t dev_alloc(void** p, size_t bytes, int dev, cudaStream_t s) {
     cudaMemPool_t pool = nullptr;
     cudaError_t e = device_pool(dev, &pool);
     if (e != cudaSuccess) return e;
-    return cudaMallocFromPoolAsync(p, bytes ? bytes : 1, pool, s);
+    constexpr size_t kGranule = (size_t)2 << 20;
+    bytes = ((bytes ? bytes : 1) + kGranule - 1) / kGranule * kGranule;
+    return cudaMallocFromPoolAsync(p, bytes, pool, s);
 }
 void dev_free(void* p, cudaStream_t s) {
     if (p) cudaFreeAsync(p, s);
@@ -268,6 +276,9 @@ mi_status plan_layout(mi_ctx* c) {
     c->rows_smem = mi::hist_rows_in_smem(c->nb, c->gpitch, gsmem);
     if (c->rows_smem < 1) return fail(c, MI_ERR_UNSUPPORTED, "device has too little shared memory");
     if (c->wide) return MI_OK;
+    c->generic_has_rare = false;
+    for (int a = 0; a < 256; ++a)
+        if ((int)c->h_rank[a] >= c->rows_smem && c->h_counts[a] > 0) c->generic_has_rare = true;
     c->bin_mode = c->bin_mode_natural < c->opt_bin_mode_max ? c->bin_mode_natural : c->opt_bin_mode_max;
     // bank of histogram word (a, b) = (a*pad + b) mod 32: an odd pad walks the rows over all banks
     c->zpitch = c->nb + c->opt_zpad;
@@ -544,6 +555,8 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.moving_pad = c->d_moving_pad;
         a.moving_quad = c->d_moving_quad;
         a.gather = c->opt_gather;
+        a.threads = c->opt_gthreads;
+        a.has_rare = c->generic_has_rare ? 1 : 0;
         a.sink = nullptr;
         a.mbins = c->d_mbins;
         a.rows_smem = c->rows_smem;
@@ -566,6 +579,14 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             nslabs = (int)((want + cnt - 1) / cnt);
             const int cap = rows_total / 64 > 1 ? rows_total / 64 : 1;
             if (nslabs > cap) nslabs = cap;
+        }
+        if (interp == MI_INTERP_TRILINEAR && !c->wide && c->opt_gather == 1 && c->opt_slab_mb > 0) {
+            // z slabs small enough that the slab's share of the 16-byte-per-voxel quad volume (plus the margin a
+            // rotation adds) stays in L2 while all SMs work on it (items are ordered slab-major)
+            const size_t quad_bytes = (size_t)(c->md[0] + 2) * (c->md[1] + 2) * (c->md[2] + 2) * sizeof(float4);
+            const int by_l2 = (int)((quad_bytes + ((size_t)c->opt_slab_mb << 20) - 1) / ((size_t)c->opt_slab_mb << 20));
+            const int cap = rows_total / 64 > 1 ? rows_total / 64 : 1;
+            if (by_l2 > nslabs) nslabs = by_l2 < cap ? by_l2 : cap;
         }
         a.nslabs = nslabs;
         timer.begin(4);
@@ -929,6 +950,12 @@ mi_status mi_set_option(mi_ctx* c, mi_option key, int64_t v) {
     case MI_OPT_GENERIC_GATHER:
         if (v < 0 || v > 1) return bad();
         c->opt_gather = (int)v; break;
+    case MI_OPT_GENERIC_THREADS:
+        if (v != 512 && v != 768 && v != 1024) return bad();
+        c->opt_gthreads = (int)v; break;
+    case MI_OPT_GENERIC_SLAB_MB:
+        if (v < 0 || v > (1 << 20)) return bad();
+        c->opt_slab_mb = (int)v; break;
     default:
         return fail(c, MI_ERR_INVALID_ARG, "mi_set_option: unknown or read-only key");
     }
@@ -955,6 +982,8 @@ mi_status mi_get_option(const mi_ctx* c, mi_option key, int64_t* out) {
     case MI_OPT_GENERIC_UNROLL: *out = c->opt_unroll; break;
     case MI_OPT_ZHIST_MATCH_ANY: *out = c->opt_match_any; break;
     case MI_OPT_GENERIC_GATHER: *out = c->opt_gather; break;
+    case MI_OPT_GENERIC_THREADS: *out = c->opt_gthreads; break;
+    case MI_OPT_GENERIC_SLAB_MB: *out = c->opt_slab_mb; break;
     case MI_INFO_LAST_UPDATES_ISSUED: *out = c->last_reds; break;
     case MI_INFO_NUM_SMS: *out = c->num_sms; break;
     case MI_INFO_BIN_MODE: *out = c->bin_mode; break;
@@ -1005,6 +1034,18 @@ mi_status mi_eval_batch(mi_ctx* c, const double* T, int64_t N, const double* q, 
 mi_status mi_eval_batch_pv(mi_ctx* c, const double* T, int64_t N, const double* q, int32_t nq,
                            double* mi_out, uint64_t* hist_out, int64_t* nvalid_out) {
     return eval_batch_impl(c, T, N, q, nq, MI_INTERP_PARTIAL_VOLUME, mi_out, hist_out, nvalid_out);
+}
+
+mi_status mi_seed_from_map(mi_family family, const double lo[3], const double hi[3], const int32_t n[3],
+                           int64_t index, double p_out[9]) {
+    if (!lo || !hi || !n || !p_out) return MI_ERR_INVALID_ARG;
+    if (!finite3(lo) || !finite3(hi) || n[0] < 1 || n[1] < 1 || n[2] < 1) return MI_ERR_INVALID_ARG;
+    const int64_t total = (int64_t)n[0] * n[1] * n[2];
+    if (index < 0 || index >= total) return MI_ERR_INVALID_ARG;
+    const int64_t k[3] = {index % n[0], (index / n[0]) % n[1], index / ((int64_t)n[0] * n[1])};
+    double p[3];
+    for (int d = 0; d < 3; ++d) p[d] = n[d] == 1 ? lo[d] : lo[d] + (double)k[d] * (hi[d] - lo[d]) / (double)(n[d] - 1);
+    return mi::seed_from_node((int)family, p, p_out) == 0 ? MI_OK : MI_ERR_INVALID_ARG;
 }
 
 mi_status mi_compose_matrix(const double p[9], double T_out[12]) {
@@ -1250,6 +1291,8 @@ mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms,
     a.moving_pad = c->d_moving_pad;
     a.moving_quad = c->d_moving_quad;
     a.gather = c->opt_gather;
+    a.threads = c->opt_gthreads;
+    a.has_rare = c->generic_has_rare ? 1 : 0;
     a.sink = reinterpret_cast<unsigned*>(c->d_red_count);
     a.mbins = c->d_mbins;
     a.rows_smem = c->rows_smem;      // the probe keeps the kernel's shared-memory size: same L1 carve-out

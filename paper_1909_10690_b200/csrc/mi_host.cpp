@@ -103,6 +103,33 @@ int family_matrix(int family, const double p[3], double T[12]) {
     }
 }
 
+// Hand-off from an exhaustive map to the registration loop (A22): the nine parameters
+// (t [mm], Euler angles [deg], scale factors) of map node (k0,k1,k2) of a family's grid, identity elsewhere.
+// Translation, Euler and scale nodes are copied; log-scale nodes become factors exp(p); a versor node becomes
+// the Euler angles of its rotation matrix R = Rz Ry Rx: ay = -asin(R20), ax = atan2(R21, R22), az = atan2(R10, R00).
+int seed_from_node(int family, const double p[3], double out[9]) {
+    for (int i = 0; i < 9; ++i) out[i] = i < 6 ? 0.0 : 1.0;
+    switch (family) {
+    case MI_FAMILY_TRANSLATION: out[0] = p[0]; out[1] = p[1]; out[2] = p[2]; return 0;
+    case MI_FAMILY_ROTATION_EULER_DEG: out[3] = p[0]; out[4] = p[1]; out[5] = p[2]; return 0;
+    case MI_FAMILY_SCALE: out[6] = p[0]; out[7] = p[1]; out[8] = p[2]; return 0;
+    case MI_FAMILY_SCALE_LOG: out[6] = std::exp(p[0]); out[7] = std::exp(p[1]); out[8] = std::exp(p[2]); return 0;
+    case MI_FAMILY_ROTATION_VERSOR: {
+        double T[12];
+        family_matrix(family, p, T);
+        const double deg = 180.0 / 3.14159265358979323846;
+        double s = -T[8];
+        if (s > 1.0) s = 1.0;
+        if (s < -1.0) s = -1.0;
+        out[4] = std::asin(s) * deg;
+        out[3] = std::atan2(T[9], T[10]) * deg;
+        out[5] = std::atan2(T[4], T[0]) * deg;
+        return 0;
+    }
+    default: return 1;
+    }
+}
+
 // CANON-1.  Voxel i of a volume (dims n, spacing s) sits at s*(i - h), h = (n-1)/2; a transform
 // is y = A x + t from fixed-physical to moving-physical (direction of eq. 3).  The
 // continuous moving index is c = M i + m0 with

@@ -26,6 +26,7 @@ constexpr int kMaxBinsWide = 4096;   // largest nbins (above 256: uint16 bins, g
 // ---- host-side double math (mi_host.cpp; compiled with -ffp-contract=off) --------------------
 int family_matrix(int family, const double p[3], double T[12]);
 void compose_matrix(const double p[9], double T[12]);
+int seed_from_node(int family, const double p[3], double out[9]);
 void index_affine(const double T[12], const int32_t fd[3], const double fs[3], const int32_t md[3],
                   const double ms[3], float out[12]);
 float bin_scale(int nbins, float lo, float hi);
@@ -42,6 +43,8 @@ struct ResampleArgs {
     const float* moving_pad;      // replicate-padded moving float32, dims (mx+2, my+2, mz+2)
     const float4* moving_quad;    // yz-quads of the padded volume (same dims), or NULL
     int gather;                   // trilinear gather scheme: 0 eight 4-byte loads, 1 two 16-byte quad loads
+    int threads;                  // CTA size of the quad kernel: 512, 768 or 1024
+    int has_rare;                 // a populated fixed-bin rank >= rows_smem exists (its updates go to global memory)
     unsigned* sink;               // NULL; or (roofline probe) no histogram is built, bins are summed here
     const uint8_t* mbins;         // moving bin indices (nearest neighbour), unpadded
     const float* M;               // n_transforms x 12 index-space affines (device)

@@ -351,8 +351,8 @@ resample_hist_kernel(const __grid_constant__ ResampleArgs a) {
     unsigned probe_acc = 0u;
     const long long nitems = (long long)a.n_transforms * a.nslabs;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
-        const int t = (int)(item / a.nslabs);
-        const int slab = (int)(item - (long long)t * a.nslabs);
+        const int slab = (int)(item / a.n_transforms);                   // slab-major (see resample_quad_kernel)
+        const int t = (int)(item - (long long)slab * a.n_transforms);
         const int tile_lo = (int)((long long)tiles_total * slab / a.nslabs);
         const int tile_hi = (int)((long long)tiles_total * (slab + 1) / a.nslabs);
         float m[12];
@@ -442,6 +442,191 @@ static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStr
     return cudaGetLastError();
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// a3 + a4, trilinear, yz-quad gathers: the kernel rotations (and every other non-diagonal transform) take.
+// Same arithmetic as resample_hist_kernel<TRILINEAR> (CANON-2, CANON-4, CANON-5), organised around what the
+// first ncu capture of the quad gathers showed (profiles/r2_ncu_generic.md): the kernel waits on memory, not
+// on the load/store pipe --
+//   * every trip first resolves the cells of its U samples per lane and issues all 2U 16-byte loads (and the
+//     U fixed-bin loads), then lerps, bins and counts: U independent load pairs are in flight per lane (the
+//     64-register budget of a 1024-thread CTA made the compiler reuse one register set for all samples, i.e.
+//     one pair in flight; THREADS < 1024 buys the registers);
+//   * items are ordered SLAB-major (all transforms of a z slab of the fixed volume before the next slab), so
+//     the SMs work on one region of the 16-byte-per-voxel quad volume at a time and it stays L2-resident
+//     (launch_resample_hist picks the slab count from the quad volume's size);
+//   * shared-memory updates use a 32-bit shared address computed once (RED.shared), tiles advance by counters
+//     instead of a division per row.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void red_shared_inc32(unsigned addr) {
+    asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(addr) : "memory");
+}
+
+template <int THREADS, int U, bool HIST, bool MASK, bool RARE>
+__global__ void __launch_bounds__(THREADS, 1) resample_quad_kernel(const __grid_constant__ ResampleArgs a) {
+    extern __shared__ __align__(16) uint32_t sh_hist[];
+    constexpr int NW = THREADS / 32;
+    constexpr int TZ = NW / 8;                 // the CTA's warps cover 8 (y) x TZ (z) fixed rows at a time
+    const int nb = a.nb, pitch = a.pitch, rows_smem = a.rows_smem;
+    const int words = rows_smem * pitch;
+    for (int w = threadIdx.x; w < words; w += THREADS) sh_hist[w] = 0u;
+    __syncthreads();
+    unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
+    asm volatile("" : "+r"(sbase));            // keep the shared base in a register (else it is re-derived per update)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wy = warp & 7, wz = warp >> 3;
+    const int fnx = a.f.nx, fny = a.f.ny, fnz = a.f.nz;
+    const int tiles_y = (fny + 7) >> 3;
+    const int tiles_total = tiles_y * ((fnz + TZ - 1) / TZ);
+    const unsigned pnx = (unsigned)a.m.nx + 2u, pny = (unsigned)a.m.ny + 2u;
+    // padded index of cell (jx+1, jy+1, jz+1) from the raw float bits T_k = magic + j_k (see MovingView::fold)
+    const unsigned fold = (unsigned)(kFloorMagicBits - 1) * (pny * pnx + pnx + 1u);
+    const float hx = __fsub_rn((float)a.m.nx, 0.5f), hy = __fsub_rn((float)a.m.ny, 0.5f), hz = __fsub_rn((float)a.m.nz, 0.5f);
+    const float mlo = a.mlo, mscale = a.mscale;
+    const int top = nb - 1;
+    const float4* __restrict__ quad = a.moving_quad;
+    const float flane = (float)lane;
+    unsigned probe_acc = 0u;
+
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int slab = (int)(item / a.n_transforms);                   // slab-major: neighbours in time share a slab
+        const int t = (int)(item - (long long)slab * a.n_transforms);
+        const int tile_lo = (int)((long long)tiles_total * slab / a.nslabs);
+        const int tile_hi = (int)((long long)tiles_total * (slab + 1) / a.nslabs);
+        float m[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
+        uint32_t* gh = a.hist + (size_t)t * nb * nb;
+
+        int tz = tile_lo / tiles_y, ty = tile_lo - tz * tiles_y;
+        for (int tile = tile_lo; tile < tile_hi; ++tile, ++ty) {
+            if (ty == tiles_y) { ty = 0; ++tz; }
+            const int iy = (ty << 3) + wy, iz = tz * TZ + wz;
+            if (iy >= fny || iz >= fnz) continue;
+            const unsigned row = (unsigned)(iz * fny + iy);
+            const float fy = (float)iy, fz = (float)iz;
+            // CANON-2: row terms, then one fma per voxel and axis
+            const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
+            const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
+            const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
+            const uint8_t* __restrict__ frow = a.fbins_ranked + (size_t)row * (unsigned)fnx;
+            float fx0 = flane;                                           // (float)ix0, advanced by exact float adds
+            for (unsigned ix0 = (unsigned)lane; ix0 < (unsigned)fnx; ix0 += 32u * U, fx0 += (float)(32 * U)) {
+                // ---- phase 1: cells of the U samples, all loads issued ----
+                unsigned idx[U];
+                float wxs[U], wys[U], wzs[U];
+                bool ok[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    // voxels past the row end get coordinates too (just numbers) and are marked invalid
+                    const float fx = fx0 + (float)(32 * u);              // exact: small integers
+                    const float cx = __fmaf_rn(m[0], fx, rx), cy = __fmaf_rn(m[4], fx, ry), cz = __fmaf_rn(m[8], fx, rz);
+                    // CANON-4: region [-0.5, n-0.5), edge clamp (via the padded copy)
+                    bool v = cx >= -0.5f && cx < hx && cy >= -0.5f && cy < hy && cz >= -0.5f && cz < hz &&
+                             (ix0 + 32u * u < (unsigned)fnx);
+                    if (MASK) {
+                        const unsigned vi = row * (unsigned)fnx + min(ix0 + 32u * u, (unsigned)fnx - 1u);
+                        v = v && ((__ldg(a.mask_bits + (vi >> 5)) >> (vi & 31u)) & 1u);
+                    }
+                    const float tx = __fadd_rd(cx, kFloorMagic), ty2 = __fadd_rd(cy, kFloorMagic), tz2 = __fadd_rd(cz, kFloorMagic);
+                    wxs[u] = __fsub_rn(cx, __fsub_rn(tx, kFloorMagic));
+                    wys[u] = __fsub_rn(cy, __fsub_rn(ty2, kFloorMagic));
+                    wzs[u] = __fsub_rn(cz, __fsub_rn(tz2, kFloorMagic));
+                    const unsigned i = (__float_as_uint(tz2) * pny + __float_as_uint(ty2)) * pnx + __float_as_uint(tx) - fold;
+                    idx[u] = v ? i : 0u;
+                    ok[u] = v;
+                }
+                float4 q0[U], q1[U];
+                unsigned fa[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    q0[u] = __ldg(quad + idx[u]);
+                    q1[u] = __ldg(quad + idx[u] + 1);
+                    fa[u] = ok[u] ? (unsigned)__ldg(frow + ix0 + 32u * u) : 0u;
+                }
+                // ---- phase 2: x-, y-, z-lerps (CANON-4 order), binning (CANON-5), one update ----
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const float v00 = lerp_rn(q0[u].x, q1[u].x, wxs[u]);
+                    const float v10 = lerp_rn(q0[u].y, q1[u].y, wxs[u]);
+                    const float v01 = lerp_rn(q0[u].z, q1[u].z, wxs[u]);
+                    const float v11 = lerp_rn(q0[u].w, q1[u].w, wxs[u]);
+                    const float w0 = lerp_rn(v00, v10, wys[u]);
+                    const float w1 = lerp_rn(v01, v11, wys[u]);
+                    const float v = lerp_rn(w0, w1, wzs[u]);
+                    const float tt = __fmul_rn(__fsub_rn(v, mlo), mscale);
+                    const unsigned b = (unsigned)min(max(__float2int_rd(tt), 0), top);
+                    const unsigned cell = fa[u] * (unsigned)pitch + b;
+                    if (!HIST) {
+                        if (ok[u]) probe_acc += cell;
+                    } else if (!RARE) {
+                        if (ok[u]) red_shared_inc32(sbase + cell * 4u);
+                    } else {
+                        const bool in_smem = (int)fa[u] < rows_smem;
+                        if (ok[u] && in_smem) red_shared_inc32(sbase + cell * 4u);
+                        if (ok[u] && !in_smem) atomicAdd(&gh[__ldg(a.rank_inv + fa[u]) * nb + b], 1u);
+                    }
+                }
+            }
+        }
+        if (!HIST) continue;
+        __syncthreads();
+        // merge the CTA-private rows into the transform's global histogram (un-ranking the fixed bin) and
+        // re-zero them for the next item
+        for (int r = warp; r < rows_smem; r += NW) {
+            uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
+            for (int b = lane; b < nb; b += 32) {
+                const uint32_t v = sh_hist[r * pitch + b];
+                if (v) {
+                    sh_hist[r * pitch + b] = 0u;
+                    atomicAdd(&grow[b], v);
+                }
+            }
+        }
+        __syncthreads();
+    }
+    if (!HIST) {
+        probe_acc = warp_sum(probe_acc);
+        if (lane == 0) atomicAdd(a.sink, probe_acc);
+    }
+}
+
+template <int THREADS, int U, bool HIST, bool MASK, bool RARE>
+static cudaError_t launch_quad_t(const ResampleArgs& a, int num_sms, cudaStream_t s) {
+    const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
+    auto kern = resample_quad_kernel<THREADS, U, HIST, MASK, RARE>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int carve = (int)((smem + 1024) * 100 / (228 * 1024));
+    if (carve > 100) carve = 100;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+    if (e != cudaSuccess) return e;
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    long long grid = nitems < num_sms ? nitems : num_sms;
+    if (grid < 1) return cudaSuccess;
+    kern<<<(unsigned)grid, THREADS, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+template <int THREADS>
+static cudaError_t launch_quad_threads(const ResampleArgs& a, int unroll, int num_sms, cudaStream_t s) {
+    const bool probe = a.sink != nullptr, mask = a.mask_bits != nullptr;
+    // RARE: some populated fixed-bin rank has no shared row (its updates go to the global histogram)
+#define MI_QUAD(UU)                                                                                   \
+    do {                                                                                              \
+        if (probe) return launch_quad_t<THREADS, UU, false, false, false>(a, num_sms, s);             \
+        if (mask) return launch_quad_t<THREADS, UU, true, true, true>(a, num_sms, s);                 \
+        if (a.has_rare) return launch_quad_t<THREADS, UU, true, false, true>(a, num_sms, s);          \
+        return launch_quad_t<THREADS, UU, true, false, false>(a, num_sms, s);                         \
+    } while (0)
+    if (unroll == 1) MI_QUAD(1);
+    if (unroll == 2) MI_QUAD(2);
+    if (unroll == 3) MI_QUAD(3);
+    MI_QUAD(4);
+#undef MI_QUAD
+}
+
 int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes) {
     const size_t reserve = 1024;  // static shared memory + alignment slack
     size_t rows = (smem_bytes > reserve ? smem_bytes - reserve : 0) / ((size_t)pitch * sizeof(uint32_t));
@@ -477,12 +662,12 @@ cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms,
         if (unroll == 3) return launch_resample_t<MI_INTERP_TRILINEAR, 3, G, H>(a, num_sms, s);       \
         return launch_resample_t<MI_INTERP_TRILINEAR, 4, G, H>(a, num_sms, s);                        \
     } while (0)
-    const bool quad = a.gather == kGatherQuad && a.moving_quad != nullptr;
-    if (a.sink != nullptr) {   // roofline probe: no histogram
-        if (quad) MI_TRI(kGatherQuad, false);
-        MI_TRI(kGatherScalar, false);
+    if (a.gather == kGatherQuad && a.moving_quad != nullptr) {
+        if (a.threads == 512) return launch_quad_threads<512>(a, unroll, num_sms, s);
+        if (a.threads == 768) return launch_quad_threads<768>(a, unroll, num_sms, s);
+        return launch_quad_threads<1024>(a, unroll, num_sms, s);
     }
-    if (quad) MI_TRI(kGatherQuad, true);
+    if (a.sink != nullptr) MI_TRI(kGatherScalar, false);   // roofline probe: no histogram
     MI_TRI(kGatherScalar, true);
 #undef MI_TRI
 }

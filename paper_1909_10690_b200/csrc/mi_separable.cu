@@ -388,6 +388,8 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
     double* sh_red = reinterpret_cast<double*>(sh_pb + kEntropyPb);
     uint32_t* sh_hist = sh_raw + zhist_table_words(a.planes);
     __shared__ int s_lo, s_hi;
+    __shared__ unsigned long long s_issued;   // histogram updates this CTA issued (a.red_count)
+    if (threadIdx.x == 0) s_issued = 0ull;
     const unsigned nb = (unsigned)a.nb;
     const unsigned pitch = (unsigned)a.pitch;
     const int rows_smem = a.rows_smem;   // includes the dump row
@@ -404,7 +406,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
     const unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
     const unsigned cbase = sbase - 4u * (unsigned)kMagicBits;   // modulo 2^32
     const float mlo = a.mlo, mscale = a.mscale;
-    unsigned long long issued = 0ull;   // histogram updates this thread issued (a.red_count)
 
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int pair = (int)(item / a.n2);
@@ -448,7 +449,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                     dump.w[j] = (~keep.w[j]) & ((uint32_t)a.rows_real * 0x01010101u);
                 }
                 if (any == 0u) continue;
-                issued += (unsigned long long)(kZCols * (iz_hi - iz_lo));
                 const uint8_t* __restrict__ fbq = a.fb + (size_t)iz_lo * colpitch + col0;
                 Bins fa_next;
                 ld_bins(fa_next, fbq);
@@ -528,6 +528,23 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                 }
             }
         }
+        if (a.red_count != nullptr && iz_lo < iz_hi) {
+            // updates issued for this item, recounted from the column flags outside the hot loop (a counter
+            // carried through it costs registers the z kernel does not have: 1024 threads x 64)
+            unsigned mine = 0u;
+            for (int tile = 0; tile < ntiles; ++tile) {
+                const int wcol = (tile * kHistThreads + warp * 32) * kZCols;
+                if (wcol >= colpitch) break;
+                Bins cv;
+                ld_bins(cv, a.colvalid + (size_t)pair * colpitch + wcol + lane * 4);
+                uint32_t any = 0u;
+#pragma unroll
+                for (int j = 0; j < kZCols / 4; ++j) any |= cv.w[j];
+                mine += any != 0u;
+            }
+            mine = warp_sum_u(mine);
+            if (lane == 0 && mine) atomicAdd(&s_issued, (unsigned long long)mine * (unsigned)(kZCols * (iz_hi - iz_lo)));
+        }
         __syncthreads();
         if (!NN && MODE != kBinGeneral) {   // pad column nb (v == moving_hi) belongs to the last bin
             for (int r = threadIdx.x; r < rows_smem; r += blockDim.x) {
@@ -564,11 +581,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
             for (unsigned b = threadIdx.x; b <= nb; b += blockDim.x) sh_hist[a.rows_real * pitch + b] = 0u;
         __syncthreads();
     }
-    if (a.red_count != nullptr) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) issued += __shfl_xor_sync(0xffffffffu, issued, o);
-        if (lane == 0 && issued) atomicAdd(a.red_count, issued);
-    }
+    if (a.red_count != nullptr && threadIdx.x == 0 && s_issued) atomicAdd(a.red_count, s_issued);
 }
 
 // fixed ranked bins -> [fnz][colpitch] (plane pitch padded to a multiple of 4 so that four adjacent

@@ -255,6 +255,22 @@ def config_c5(res=1.0, grid_n=41, seed=303) -> Config:
     return Config("C5", fixed, moving, fsp, msp, 256, 0, (-10,) * 3, (10,) * 3, (grid_n,) * 3, (), d)
 
 
+def config_c5all(res=1.0, grid_n=41, seed=303, salt=0.02) -> Config:
+    """C5 with EVERY fixed bin populated, as real MR data at 256 bins is (the label phantom leaves the bins
+    between its tissue means empty, so at most 192 of 256 fixed bins hold voxels): a seeded 2 % of the fixed
+    voxels are replaced by uniform values in [0, 1].  The z kernel's shared histogram holds 209 rows at 256
+    bins, so the rarest fixed bins take the rare-voxel kernel, the histograms are written to global memory and a
+    separate entropy launch follows -- the path real data takes.  Stress input for bench.py --config C5ALL."""
+    c = config_c5(res, grid_n, seed)
+    idx = np.arange(c.fixed.size, dtype=_U64)
+    pick = keyed_uniform(seed + 7, idx, 0) < salt
+    vals = keyed_uniform(seed + 7, idx, 1).astype(np.float32)
+    fixed = c.fixed.copy().reshape(-1)
+    fixed[pick] = vals[pick]
+    return Config("C5ALL", fixed.reshape(c.fixed.shape), c.moving, c.fixed_spacing, c.moving_spacing, c.nbins, c.family,
+                  c.lo, c.hi, c.n, c.q, c.truth)
+
+
 def config_paper51(res=1.0, grid_n=51, seed=303) -> Config:
     """Paper-shaped context run (not one of BASELINE.json's configs): the paper maps "the same image on
     both fixed and moving" and gives 51 positions over +-25 mm per axis as its example
@@ -271,7 +287,7 @@ def config_paper51(res=1.0, grid_n=51, seed=303) -> Config:
 def get_config(name: str, **kw) -> Config:
     """Cached access: get_config('C5'), get_config('C3', res=0.25, grid_n=5) ..."""
     return {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4,
-            "C5": config_c5, "PAPER51": config_paper51}[name](**kw)
+            "C5": config_c5, "C5ALL": config_c5all, "PAPER51": config_paper51}[name](**kw)
 
 
 def ramp_volume(dims, coeffs) -> np.ndarray:

@@ -99,6 +99,18 @@ def test_compose_matrix_bit_for_bit_against_oracle(lib):
         lib.mi_compose_matrix([0, 0, 0, 0, np.nan, 0, 1, 1, 1])
 
 
+def test_seed_from_map_equals_oracle(lib):
+    from oracle import multimetric as mm
+    lo, hi, n = (-0.3, -0.2, -0.25), (0.3, 0.25, 0.2), (5, 4, 3)
+    for fam in range(5):
+        for index in range(0, 60, 7):
+            a, b = lib.mi_seed_from_map(fam, lo, hi, n, index), mm.seed_from_map(fam, lo, hi, n, index)
+            assert np.array_equal(a, b) if fam != 2 else np.max(np.abs(a - b)) <= 1e-12, (fam, index)
+    for bad in (-1, 60):
+        with pytest.raises(lib.MIError):
+            lib.mi_seed_from_map(0, lo, hi, n, bad)
+
+
 def test_create_validates_arguments(lib):
     v = np.zeros((4, 4, 4), dtype=np.float32)
     sp = (1.0, 1.0, 1.0)

@@ -171,3 +171,46 @@ def test_register_follows_the_oracle_trajectory(mi):
             assert np.array_equal(got["p"], got["trace"][-1])
         r0 = mi.mi_register(ctx, p0, runs[0][0], (0, 0, 0), (1, 1, 1), 5, 0.5, 1)     # nothing may move
         assert r0["iterations"] == 1 and np.array_equal(r0["p"], p0)
+
+
+def test_coarse_map_seeds_the_registration(mi):
+    """SURVEY 8(f)-2's hand-off end to end on the GPU: a coarse exhaustive map (the exhaustive
+    search as the robust start) -> mi_seed_from_map at its arg max -> mi_register (multi-metric ascent,
+    PAPER.md:199, 210).  Translation on the C1 pair: coarse 5^3 map on integer voxels, Tsallis q = 0.5 channel
+    for the translation group as the paper recommends; the ascent must end within one FINE step (0.5 voxel) of
+    the maximum of the fine 0.5-voxel map, and equal the oracle's trajectory from the same seed.  Rotation on
+    the quarter-resolution C3 pair: coarse 5^3 Euler map over +-6 deg (Shannon), ascent over the rotation group
+    ends within one fine step (1 deg) of the fine map's maximum."""
+    import oracle as orc
+    from oracle import multimetric as mm
+    cfg = ph.get_config("C1")
+    with mi.mi_create(cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        coarse, am = mi.mi_map(ctx, 0, cfg.lo, cfg.hi, cfg.n, (0.5,), 1)
+        p0 = mi.mi_seed_from_map(0, cfg.lo, cfg.hi, cfg.n, am[1])           # arg max of the Tsallis channel
+        assert np.array_equal(p0, mm.seed_from_map(0, cfg.lo, cfg.hi, cfg.n, int(am[1])))
+        delta = np.array([0.5, 0.5, 0.5, 0, 0, 0, 0, 0, 0.0])
+        got = mi.mi_register(ctx, p0, delta, (0.5, 0, 0), (0.05, 1, 1), 40, 0.5, 1)
+        fine, fam = mi.mi_map(ctx, 0, (-1, -4, -2), (4, 1, 3), (11, 11, 11), (0.5,), 1)
+    ref = mm.register(cfg.fixed, cfg.fixed_spacing, cfg.moving, cfg.moving_spacing, cfg.nbins, cfg.ranges, p0, delta,
+                      (0.5, 0, 0), (0.05, 1, 1), 40, 0.5, interp=1)
+    assert got["iterations"] == ref["iterations"] and np.max(np.abs(got["trace"] - ref["trace"])) <= 1e-6
+    k2, k1, k0 = np.unravel_index(int(fam[1]), (11, 11, 11))
+    peak = np.array([-1 + 0.5 * k0, -4 + 0.5 * k1, -2 + 0.5 * k2])
+    assert np.max(np.abs(got["p"][:3] - peak)) <= 0.5 + 1e-9, (got["p"][:3], peak)
+    assert got["values"][1] >= coarse[1].max() - 1e-9                       # it did not fall below its seed
+
+    c3 = ph.get_config("C3", res=0.25, grid_n=5)
+    lo, hi, n = (-6.0,) * 3, (6.0,) * 3, (5, 5, 5)
+    with mi.mi_create(c3.fixed, c3.moving, c3.fixed_spacing, c3.moving_spacing, c3.nbins) as ctx:
+        coarse, am = mi.mi_map(ctx, 1, lo, hi, n, (), 1)
+        p0 = mi.mi_seed_from_map(1, lo, hi, n, am[0])
+        assert np.array_equal(p0[:3], [0, 0, 0]) and np.array_equal(p0[6:], [1, 1, 1])
+        delta = np.array([0, 0, 0, 1.0, 1.0, 1.0, 0, 0, 0])
+        got = mi.mi_register(ctx, p0, delta, (0, 1.0, 0), (1, 0.1, 1), 30, 0.5, 1)
+        centre = p0[3:6]
+        flo, fhi = tuple(centre - 3.0), tuple(centre + 3.0)
+        fine, fam = mi.mi_map(ctx, 1, flo, fhi, (7, 7, 7), (), 1)
+    k2, k1, k0 = np.unravel_index(int(fam[0]), (7, 7, 7))
+    peak = np.array([flo[0] + k0, flo[1] + k1, flo[2] + k2])
+    assert np.max(np.abs(got["p"][3:6] - peak)) <= 1.0 + 1e-9, (got["p"][3:6], peak)
+    assert got["values"][0] >= coarse[0].max() - 1e-9

@@ -100,3 +100,23 @@ def test_register_follows_its_rule_and_reaches_the_map_maximum():
     # and it climbed: the Tsallis value at the end exceeds the one at the start
     _, v0 = mm.multimetric_gradient(*args, p0, delta, 0.5, interp=1)
     assert r["values"][1] > v0[1]
+
+
+def test_seed_from_map_reproduces_the_nodes_transform():
+    """The hand-off map -> register (reading A22): for every family the nine parameters of a node compose to the
+    very transform the map evaluated at that node (compose_matrix(seed) == family_matrix(node)): exactly for
+    translation / Euler / scale, to rounding for log-scale and for the versor -> Euler conversion."""
+    lo, hi, n = (-0.3, -0.2, -0.25), (0.3, 0.25, 0.2), (5, 4, 3)
+    for fam in range(5):
+        for index in (0, 7, 23, 59):
+            p = mm.seed_from_map(fam, lo, hi, n, index)
+            k = (index % 5, (index // 5) % 4, index // 20)
+            node = [lo[d] + k[d] * (hi[d] - lo[d]) / (n[d] - 1) for d in range(3)]
+            want = orc.family_matrix(fam, node)
+            got = mm.compose_matrix(p)
+            if fam in (0, 1, 3):
+                assert np.array_equal(got, want), (fam, index)
+            else:
+                assert np.max(np.abs(got - want)) <= 1e-14, (fam, index)
+    assert np.array_equal(mm.seed_from_map(0, lo, hi, n, 59), [0.3, 0.25, 0.2, 0, 0, 0, 1, 1, 1])
+    assert np.array_equal(mm.seed_from_map(3, (1, 1, 1), (1, 1, 1), (1, 1, 1), 0), [0, 0, 0, 0, 0, 0, 1, 1, 1])
