@@ -105,7 +105,8 @@ def test_seed_from_map_equals_oracle(lib):
     for fam in range(5):
         for index in range(0, 60, 7):
             a, b = lib.mi_seed_from_map(fam, lo, hi, n, index), mm.seed_from_map(fam, lo, hi, n, index)
-            assert np.array_equal(a, b) if fam != 2 else np.max(np.abs(a - b)) <= 1e-12, (fam, index)
+            # exp / asin / atan2 come from two maths libraries (libm, numpy's SIMD loops): an ulp, not a bit pattern
+            assert np.array_equal(a, b) if fam not in (2, 4) else np.max(np.abs(a - b)) <= 1e-12, (fam, index)
     for bad in (-1, 60):
         with pytest.raises(lib.MIError):
             lib.mi_seed_from_map(0, lo, hi, n, bad)
