@@ -40,13 +40,14 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # DRAM traffic of the dominant kernel from the committed `ncu --set full` captures of this command
-# (profiles/r2_ncu_*.md): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch and the evaluations
+# (profiles/r2b_ncu.md): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch and the evaluations
 # that launch performed; bench.py scales it to a step (bytes per evaluation x evaluations per step).
 # Keyed by (config, grid, interpolation).
 NCU_DRAM = {
-    # C5, zhist_kernel, launch = 5 of the 41 p0 slabs = 8405 transforms (profiles/r1k_ncu_zhist_final.md)
-    ("C5", (41, 41, 41), 1): {"bytes_per_launch": 16264608000 + 553361408, "evals_per_launch": 8405 * 21023600,
-                               "source": "profiles/r1k_ncu_zhist_final.md"},
+    # C5, zhist_kernel, launch = 5 of the 41 p0 slabs = 8405 transforms (profiles/r2b_ncu.md section 2:
+    # dram__bytes_read.sum 16.283806 GB + dram__bytes_write.sum 553.878528 MB)
+    ("C5", (41, 41, 41), 1): {"bytes_per_launch": 16283806000 + 553878528, "evals_per_launch": 8405 * 21023600,
+                               "source": "profiles/r2b_ncu.md"},
 }
 
 METRIC = "voxel-transform evaluations per second (MI map, 260x311x260 fixed, 256 bins)"
@@ -251,6 +252,8 @@ def run_ours(rt, args, cfg, interp, cpu_budget_s):
     am_dev = torch.empty(nch, dtype=torch.int64, device=rt.dev)
     ctx = mi.mi_create(fixed_dev, moving_dev, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins, *cfg.ranges,
                        device=rt.local, cuda_stream=rt.stream)
+    for name, val in args.opt:                           # experiments only: the default run sets none
+        mi.mi_set_option(ctx, getattr(mi, "MI_OPT_" + name.upper()), val)
     slab = sh.slab_range(cfg.n, rt.rank, rt.world) if shard else None
     if shard and slab is not None:
         slab_dev = torch.empty((nch, slab[1][2] - slab[0][2]) + shape[2:], dtype=torch.float64, device=rt.dev)
@@ -446,7 +449,8 @@ def run_ours(rt, args, cfg, interp, cpu_budget_s):
                 "l2": "flushed between timed steps (256 MiB write)",
                 "parallelism": ("one grid sharded x%d (p2 slabs, NCCL all-gather)" if shard else "replicas x%d") % rt.world,
                 "mi_evals_per_s": mi_evals,
-                "paper_table1_mi_evals_per_s_gtx1060": PAPER_TABLE1.get(cfg.family)}),
+                "paper_table1_mi_evals_per_s_gtx1060": PAPER_TABLE1.get(cfg.family),
+                **({"options": dict(args.opt)} if args.opt else {})}),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps, "ms_per_step": e2e_s / e2e_steps * 1e3, "mi_create_ms": create_ms},
             "gpu_launches": launches, "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
@@ -484,9 +488,12 @@ def main():
     ap.add_argument("--grid", type=int, default=0, help="development only: grid nodes per axis")
     ap.add_argument("--interp", default="trilinear", choices=["trilinear", "nearest", "pv"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="experiments only: mi_set_option(MI_OPT_<NAME>, VALUE) on the context, e.g. zhist_match_any=1")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3  # timing rule: W >= 3
+    args.opt = [(kv.split("=")[0], int(kv.split("=")[1])) for kv in args.opt]
     if args.impl == "ours" and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         respawn_under_torchrun(args)
 

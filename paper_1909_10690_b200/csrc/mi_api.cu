@@ -484,6 +484,27 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
     return MI_OK;
 }
 
+// CTAs per transform of the generic kernels: one when there are many transforms; otherwise the volume is split
+// into slabs of 32-row tiles so that about 16 waves of CTAs exist (each slab keeps >= 2 tiles).  The quad-gather
+// kernel orders its items slab-major, so for it the slabs are also made small enough that a slab's share of the
+// 16-byte-per-voxel quad volume (plus the margin a rotation adds) stays in L2 while all SMs work on it.
+int generic_nslabs(const mi_ctx* c, int64_t cnt, int interp) {
+    const int rows_total = c->fd[1] * c->fd[2];
+    const int cap = rows_total / 64 > 1 ? rows_total / 64 : 1;
+    int nslabs = 1;
+    const int64_t want = 16LL * c->num_sms;
+    if (cnt < want) {
+        nslabs = (int)((want + cnt - 1) / cnt);
+        if (nslabs > cap) nslabs = cap;
+    }
+    if (interp == MI_INTERP_TRILINEAR && !c->wide && c->opt_gather == 1 && c->opt_slab_mb > 0) {
+        const size_t quad_bytes = (size_t)(c->md[0] + 2) * (c->md[1] + 2) * (c->md[2] + 2) * sizeof(float4);
+        const int by_l2 = (int)((quad_bytes + ((size_t)c->opt_slab_mb << 20) - 1) / ((size_t)c->opt_slab_mb << 20));
+        if (by_l2 > nslabs) nslabs = by_l2 < cap ? by_l2 : cap;
+    }
+    return nslabs;
+}
+
 // The shared core of mi_eval_batch and mi_map.  hM: N x 12 index-space fp32 transforms in host
 // memory.  If map_out != NULL the result is assembled channel-major (step a6) instead of being
 // returned transform-major.  If sep != NULL the histograms are built by the separable path.
@@ -539,8 +560,6 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
                        (size_t)chunk * nbins2 * helem)) != MI_OK)
             return st;
     }
-    const int rows_total = c->fd[1] * c->fd[2];
-
     for (int64_t off = 0; sep == nullptr && off < N; off += chunk) {
         const int64_t cnt = (N - off < chunk) ? (N - off) : chunk;
         uint32_t* hist = hist_to_user_dev
@@ -571,23 +590,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
         a.mlo = c->mlo;
         a.mscale = c->mscale;
         a.n_transforms = (int)cnt;
-        // CTAs per transform: one when there are many transforms; otherwise split the volume into
-        // slabs of 32-row tiles so that about 16 waves of CTAs exist (each slab keeps >= 2 tiles).
-        int nslabs = 1;
-        const int64_t want = 16LL * c->num_sms;
-        if (cnt < want) {
-            nslabs = (int)((want + cnt - 1) / cnt);
-            const int cap = rows_total / 64 > 1 ? rows_total / 64 : 1;
-            if (nslabs > cap) nslabs = cap;
-        }
-        if (interp == MI_INTERP_TRILINEAR && !c->wide && c->opt_gather == 1 && c->opt_slab_mb > 0) {
-            // z slabs small enough that the slab's share of the 16-byte-per-voxel quad volume (plus the margin a
-            // rotation adds) stays in L2 while all SMs work on it (items are ordered slab-major)
-            const size_t quad_bytes = (size_t)(c->md[0] + 2) * (c->md[1] + 2) * (c->md[2] + 2) * sizeof(float4);
-            const int by_l2 = (int)((quad_bytes + ((size_t)c->opt_slab_mb << 20) - 1) / ((size_t)c->opt_slab_mb << 20));
-            const int cap = rows_total / 64 > 1 ? rows_total / 64 : 1;
-            if (by_l2 > nslabs) nslabs = by_l2 < cap ? by_l2 : cap;
-        }
+        const int nslabs = generic_nslabs(c, cnt, interp);
         a.nslabs = nslabs;
         timer.begin(4);
         if (pv) {
@@ -1307,7 +1310,7 @@ mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms,
     a.mlo = c->mlo;
     a.mscale = c->mscale;
     a.n_transforms = n_transforms;
-    a.nslabs = 1;
+    a.nslabs = generic_nslabs(c, n_transforms, MI_INTERP_TRILINEAR);   // the launch shape mi_eval_batch / mi_map use
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     MI_CUDA(c, cudaEventCreate(&e0));
     MI_CUDA(c, cudaEventCreate(&e1));

@@ -445,9 +445,9 @@ static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStr
 
 // ------------------------------------------------------------------------------------------------
 // a3 + a4, trilinear, yz-quad gathers: the kernel rotations (and every other non-diagonal transform) take.
-// Same arithmetic as resample_hist_kernel<TRILINEAR> (CANON-2, CANON-4, CANON-5), organised around what the
-// first ncu capture of the quad gathers showed (profiles/r2_ncu_generic.md): the kernel waits on memory, not
-// on the load/store pipe --
+// Same arithmetic as resample_hist_kernel<TRILINEAR> (CANON-2, CANON-4, CANON-5), organised so that the loads
+// of several samples are in flight per lane (the first version waited on memory with one pair in flight; as
+// committed the L1TEX data pipe is 91 % busy and the issue slots 82 %, profiles/r2b_ncu.md section 5) --
 //   * every trip first resolves the cells of its U samples per lane and issues all 2U 16-byte loads (and the
 //     U fixed-bin loads), then lerps, bins and counts: U independent load pairs are in flight per lane (the
 //     64-register budget of a 1024-thread CTA made the compiler reuse one register set for all samples, i.e.
