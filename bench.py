@@ -426,6 +426,26 @@ def run_ours(rt, args, cfg, interp, cpu_budget_s):
                          "frac_of_gathers_plus_updates": achieved * (1.0 / g_rate + 1.0 / r_rand),
                          "t_lsu_gather_nominal_ms": t_lsu * 1e3})
 
+    eval_batch = None
+    if path == 0 and interp == 1:
+        # latency of mi_eval_batch (the engine of mi_multimetric_gradient / mi_register) on the same context:
+        # N = 1, 19 (one finite-difference step of a nine-parameter registration) and one transform per SM;
+        # Shannon + one Tsallis order, outputs to the host, median host wall-clock of 7 calls after 2 warm-ups
+        eval_batch = {}
+        allT = np.stack([mi.mi_family_matrix(cfg.family, [cfg.lo[d] + k * (cfg.hi[d] - cfg.lo[d]) / max(cfg.n[d] - 1, 1)
+                                                          for d, k in enumerate((t % cfg.n[0], (t // cfg.n[0]) % cfg.n[1], t // (cfg.n[0] * cfg.n[1])))])
+                         for t in sample_nodes(cfg, min(cfg.n_transforms, rt.num_sms))])
+        for nt in (1, 19, rt.num_sms):
+            if nt > len(allT):
+                continue
+            ts = []
+            for i in range(9):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                mi.mi_eval_batch(ctx, allT[:nt], (0.5,), interp)
+                ts.append((time.perf_counter() - t0) * 1e3)
+            eval_batch["n%d_ms" % nt] = float(np.median(ts[2:]))
+
     cpu_baseline = None
     if cpu_budget_s > 0:
         cpu_baseline, _ = time_oracle(cfg, interp, cpu_budget_s)
@@ -460,6 +480,8 @@ def run_ours(rt, args, cfg, interp, cpu_budget_s):
             "path": {0: "generic", 1: "separable", 2: "wide", 3: "partial-volume"}[path],
             "rare_voxels": mi.mi_get_option(ctx, mi.MI_INFO_RARE_VOXELS),
             "capture_analysis": analysis, "wall_s_timed_region": wall}
+    if eval_batch:
+        line["eval_batch_latency"] = eval_batch
     mi.mi_destroy(ctx)
     return line
 
