@@ -323,8 +323,11 @@ mi_status mi_last_timing(const mi_ctx *ctx, float ms[5], int64_t launches[5]);
 
 /* Shared-memory atomic rate probe for the roofline: runs `iters` rounds of
  * atomicAdd(u32) into an nbins x nbins table in shared memory on every SM and reports
- * lane-updates per second.  pattern: 0 conflict-free (lane-distinct banks), 1 uniform random bins,
- * 2 all lanes on one address.  Host pointers. */
+ * lane-updates per second.  pattern: 0 conflict-free (lane-distinct banks); 1 uniform random bins,
+ * independent between the lanes of a warp (a hash of thread and update number) -- the roofline's
+ * denominator; 2 all lanes on one address; 3 one linear congruential generator per thread seeded linearly in
+ * the thread index (round 1's pattern: random in time, but the lanes of a warp form an arithmetic
+ * progression, which spreads them over the banks more evenly than chance).  Host pointers. */
 mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
                                       double *updates_per_s);
 

@@ -986,7 +986,8 @@ atomic_probe_kernel(int words_log2, int pattern, int iters, unsigned* __restrict
     __syncthreads();
     const unsigned lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned mask = (unsigned)words - 1u;
-    unsigned state = (blockIdx.x * 1024u + threadIdx.x) * 2654435761u + 12345u;
+    const unsigned tid = blockIdx.x * 1024u + threadIdx.x;
+    unsigned state = tid * 2654435761u + 12345u;
     const unsigned same = (sink[0] & 1u) + 2u;  // one address, not provably uniform at compile time
     for (int it = 0; it < iters; it += 4) {
 #pragma unroll
@@ -995,8 +996,19 @@ atomic_probe_kernel(int words_log2, int pattern, int iters, unsigned* __restrict
             if (pattern == 0) {
                 idx = (((warp * 37u + (unsigned)(it + u) * 11u) << 5) + lane) & mask;  // lane-distinct banks
             } else if (pattern == 1) {
+                // uniform random bins, INDEPENDENT between the lanes of a warp: a 32-bit integer hash of
+                // (thread, update number).  32 independent lanes over 32 banks load the fullest bank with
+                // 3.53 addresses on average -- the cost of a histogram update whose bin is data.
+                unsigned x = tid * 0x9E3779B9u + (unsigned)(it + u) * 0x85EBCA6Bu;
+                x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;
+                idx = x & mask;
+            } else if (pattern == 3) {
+                // round 1's "random" pattern, kept for the record: one LCG per thread seeded linearly in the
+                // thread index, so the 32 lanes of a warp form an arithmetic progression modulo 2^32 in every
+                // round -- bins that look random in time but are evenly spread ACROSS the lanes (2.70
+                // wavefronts per update instead of 3.53)
                 state = state * 1664525u + 1013904223u;
-                idx = (state >> 10) & mask;                                            // uniform random bins
+                idx = (state >> 10) & mask;
             } else {
                 idx = same;
             }

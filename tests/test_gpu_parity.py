@@ -730,3 +730,17 @@ def test_separable_many_moving_rows_exceeds_grid_y_limit(mi):
                   (2.0,), (0, 0, 0))
     for interp in (0, 1):
         check_map(mi, c, interp)
+
+
+def test_roofline_probes_order_and_random_bank_cost(mi):
+    """The roofline's denominators: the shared-memory update rate with lane-distinct banks, with
+    uniform random bins drawn INDEPENDENTLY per lane, with round 1's per-thread LCG (lanes in arithmetic
+    progression: fewer bank collisions than chance) and with every lane on one address (merged by the hardware).
+    32 independent lanes over 32 banks load the fullest bank with 3.53 addresses on average
+    (tests/test_oracle_pins.py::test_expected_bank_load_of_independent_uniform_lanes), so the random rate must sit
+    near 1/3.53 of one warp-wide update per clock and clearly below the LCG pattern's."""
+    free, rand, same, lcg = (mi.mi_probe_shared_atomic_rate(0, 256, p, 4096) for p in (0, 1, 2, 3))
+    assert free > lcg > rand > 0
+    assert same > rand
+    assert 0.25 < rand / free < 0.45, rand / free
+    assert 1.15 < lcg / rand < 1.5, lcg / rand

@@ -425,3 +425,22 @@ def test_map_range_helper_equals_orc_map():
     full = orc.mi_map(*args, q=(0.5,))["map"]
     assert np.array_equal(orc.mi_map_range(*args, (0, 0, 0), cfg.n, q=(0.5,)), full)
     assert np.array_equal(orc.mi_map_range(*args, (1, 0, 2), (3, 4, 4), q=(0.5,)), full[:, 2:4, 0:4, 1:3])
+
+
+def test_expected_bank_load_of_independent_uniform_lanes():
+    """Roofline arithmetic, not oracle arithmetic: a warp-wide shared-memory update takes as many passes as the
+    fullest of the 32 banks holds distinct addresses.  For 32 lanes with independent uniform bins that is 3.53 on
+    average (the denominator of the headline roofline fraction); an arithmetic progression of
+    bins across the lanes -- what one linear congruential generator per thread, seeded linearly in the thread
+    index, produces -- is spread more evenly (about 2.7)."""
+    rng = np.random.default_rng(7)
+    x = rng.integers(0, 1 << 16, size=(20000, 32))
+    load = np.array([np.bincount(r & 31, minlength=32).max() for r in x])
+    assert abs(load.mean() - 3.53) < 0.03
+    lane = np.arange(32, dtype=np.uint64)
+    loads = []
+    for _ in range(4000):
+        a, d = (int(v) for v in rng.integers(0, 1 << 32, size=2))
+        s = (np.uint64(a) + lane * np.uint64(d | 1)) & np.uint64(0xFFFFFFFF)
+        loads.append(np.bincount(((s >> np.uint64(10)) & np.uint64(31)).astype(np.int64), minlength=32).max())
+    assert 2.4 < np.mean(loads) < 3.0, np.mean(loads)
