@@ -29,7 +29,7 @@ struct mi_ctx {
     float* d_moving_pad = nullptr;      // replicate-padded moving volume (mx+2, my+2, mz+2)
     float4* d_moving_quad = nullptr;    // its yz-quads (generic kernel, trilinear): 16 bytes per padded voxel
     uint8_t* d_mbins = nullptr;
-    uint8_t* d_mbins_pad = nullptr;     // replicate-padded moving bins (partial-volume interpolation)
+    uint32_t* d_mbins_quad = nullptr;   // yz-quads of the replicate-padded moving bins (partial-volume interpolation)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
     unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
     unsigned rare_alloc = 0;            // entries d_rare was allocated for
@@ -598,7 +598,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             pa.fbins_ranked = c->d_fbins_ranked;
             pa.rank_inv = c->d_rank_inv;
             pa.mask_bits = c->d_mask_bits;
-            pa.mbins_pad = c->d_mbins_pad;
+            pa.mbins_quad = c->d_mbins_quad;
             pa.M = a.M;
             pa.hist = reinterpret_cast<unsigned long long*>(hist);
             pa.rows_smem = c->rows_smem;
@@ -608,6 +608,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             pa.nb = c->nb;
             pa.n_transforms = (int)cnt;
             pa.nchunks = 0;
+            pa.rows_per_chunk = 0;
             MI_CUDA(c, mi::launch_resample_hist_pv(pa, c->num_sms, s));
         } else if (c->wide) {
             mi::WideArgs w;
@@ -830,8 +831,8 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         }
         if ((st = plan_layout(c)) != MI_OK) { mi::set_thread_error(c->err); break; }
         if (!c->wide) {
-            if ((e = dev_alloc((void**)&c->d_mbins_pad, (size_t)npad, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving bins"); break; }
-            if ((e = mi::launch_pad_replicate_u8(c->d_mbins, c->d_mbins_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving bins"); break; }
+            if ((e = dev_alloc((void**)&c->d_mbins_quad, (size_t)npad * sizeof(uint32_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bin quads"); break; }
+            if ((e = mi::launch_bins_quad_build(c->d_mbins, c->d_mbins_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving bin quads"); break; }
         }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if (!c->wide) {
@@ -856,7 +857,7 @@ void mi_destroy(mi_ctx* c) {
     DeviceGuard guard(c->device);
     if (guard.ok) {
         void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mask_bits, c->d_fbins16, c->d_mbins16, c->d_mbins,
-                        c->d_mbins_pad, c->d_moving_quad, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
+                        c->d_mbins_quad, c->d_moving_quad, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);

@@ -109,15 +109,15 @@ struct PvArgs {
     const uint8_t* fbins_ranked;  // fixed bins replaced by their population rank, flat voxel order
     const int* rank_inv;          // rank -> fixed bin
     const uint32_t* mask_bits;    // NULL, or one bit per fixed voxel
-    const uint8_t* mbins_pad;     // replicate-padded moving BIN volume, dims (mx+2, my+2, mz+2)
+    const uint32_t* mbins_quad;   // yz-quads of the replicate-padded moving BIN volume, dims (mx+2, my+2, mz+2)
     const float* M;               // n_transforms x 12 (device)
     unsigned long long* hist;     // n_transforms x nb x nb in units of 2^-15 voxel, zero on entry
     int rows_smem, pitch;         // shared histogram rows (ranked) and words per row
     VolumeDesc f, m;
     int nb, n_transforms;
-    int nchunks;                  // set by the launcher: voxel chunks per transform
+    int nchunks, rows_per_chunk;  // set by the launcher: chunks of whole fixed rows per transform
 };
-cudaError_t launch_pad_replicate_u8(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, cudaStream_t s);
+cudaError_t launch_bins_quad_build(const uint8_t* src, uint32_t* dst, int nx, int ny, int nz, cudaStream_t s);
 cudaError_t launch_resample_hist_pv(PvArgs a, int num_sms, cudaStream_t s);
 cudaError_t launch_entropy_pv(const unsigned long long* hist, int nb, int n_transforms, const double* q_dev, int nq,
                               int q_off, int form, double* mi_out, int64_t* nvalid, OutMap om, cudaStream_t s);

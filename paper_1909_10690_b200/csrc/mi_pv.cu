@@ -6,10 +6,10 @@
 // Arithmetic (reading A21): coordinates, validity, floor / fraction and edge clamp are CANON-2 / CANON-4;
 // the fraction of each axis is rounded to 1/32 voxel, u = floor(32 f + 0.5), and a neighbour's weight is the
 // integer product of (u or 32 - u) over the axes, so a sample adds exactly 2^15 units and every histogram is an
-// integer table that does not depend on the order of the updates.  Neighbour bins come from the pre-binned,
-// replicate-padded moving volume (eight byte gathers, no lerps).
+// integer table that does not depend on the order of the updates.  Neighbour bins come from the yz-quads of the
+// pre-binned, replicate-padded moving volume (two 4-byte gathers, no lerps).
 //
-//   resample_hist_pv_kernel   CTA-private u32 histogram in shared memory, one (transform, voxel chunk) item
+//   resample_hist_pv_kernel   CTA-private u32 histogram in shared memory, one (transform, chunk of rows) item
 //                             at a time; a chunk holds at most 131040 voxels so that no counter can pass
 //                             2^32 (131040 * 2^15 < 2^32); merged into the transform's uint64 histogram
 //   entropy_pv_kernel         step a5 on uint64 counts (unit 2^-15 voxel; probabilities are unit-free)
@@ -25,30 +25,38 @@ namespace {
 
 constexpr int kPvChunkVoxels = 131040;   // multiple of 32; 131040 * 32768 = 4293918720 < 2^32
 
-__global__ void __launch_bounds__(256) pad_replicate_u8_kernel(const uint8_t* __restrict__ src,
-                                                               uint8_t* __restrict__ dst, int nx, int ny, int nz) {
+// yz-quads of the replicate-padded moving BIN volume: entry (x,y,z) of the padded grid holds the bins of the padded
+// voxels (x,y,z), (x,y+1,z), (x,y,z+1), (x,y+1,z+1) in bytes 0..3 -- the entries x and x+1 are the eight neighbours of
+// a sample, two 4-byte loads instead of eight 1-byte gathers (the load/store unit writes 4 bytes per lane into the
+// register file whatever the access size, profiles/r2b_ncu.md section 5).
+__global__ void __launch_bounds__(256) bins_quad_build_kernel(const uint8_t* __restrict__ src, uint32_t* __restrict__ dst,
+                                                              int nx, int ny, int nz) {
     const int px = nx + 2, py = ny + 2, pz = nz + 2;
     const int64_t total = (int64_t)px * py * pz;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (int64_t)gridDim.x * blockDim.x) {
         const int x = (int)(i % px);
         const int64_t r = i / px;
         const int y = (int)(r % py), z = (int)(r / py);
-        const int sx = min(max(x - 1, 0), nx - 1), sy = min(max(y - 1, 0), ny - 1), sz = min(max(z - 1, 0), nz - 1);
-        dst[i] = src[((int64_t)sz * ny + sy) * nx + sx];
+        const int sx = min(max(x - 1, 0), nx - 1);
+        const int sy0 = min(max(y - 1, 0), ny - 1), sy1 = min(max(y, 0), ny - 1);   // padded y and y+1
+        const int sz0 = min(max(z - 1, 0), nz - 1), sz1 = min(max(z, 0), nz - 1);   // padded z and z+1
+        const uint32_t b00 = src[((int64_t)sz0 * ny + sy0) * nx + sx], b10 = src[((int64_t)sz0 * ny + sy1) * nx + sx];
+        const uint32_t b01 = src[((int64_t)sz1 * ny + sy0) * nx + sx], b11 = src[((int64_t)sz1 * ny + sy1) * nx + sx];
+        dst[i] = b00 | (b10 << 8) | (b01 << 16) | (b11 << 24);
     }
 }
 
-// One axis: validity (CANON-4 region), padded lower index floor(c) + 1 and the weight pair (32 - u, u).
+// One axis: validity (CANON-4 region), the raw float bits of magic + floor(c) and the weight pair (32 - u, u).
 struct PvAxis {
     bool ok;
-    int lower;
+    unsigned tbits;
     unsigned w0, w1;
 };
 __device__ __forceinline__ PvAxis pv_axis(float c, float half_hi) {
     PvAxis a;
     a.ok = c >= -0.5f && c < half_hi;
     const float t = __fadd_rd(c, kFloorMagic);
-    a.lower = __float_as_int(t) - kFloorMagicBits + 1;
+    a.tbits = __float_as_uint(t);
     const float f = __fsub_rn(c, __fsub_rn(t, kFloorMagic));
     const int u = __float2int_rd(__fadd_rn(__fmul_rn(f, 32.0f), 0.5f));
     a.w1 = (unsigned)u;
@@ -56,6 +64,11 @@ __device__ __forceinline__ PvAxis pv_axis(float c, float half_hi) {
     return a;
 }
 
+// One (transform, chunk of fixed rows) item per CTA at a time; a warp takes whole rows, a lane the voxels
+// ix = lane + 32 j of its row, kPvUnroll of them per trip with all their loads issued first.
+constexpr int kPvUnroll = 2;
+
+template <bool MASK>
 __global__ void __launch_bounds__(kHistThreads, 1) resample_hist_pv_kernel(const __grid_constant__ PvArgs a) {
     extern __shared__ __align__(16) uint32_t sh_hist[];
     const int nb = a.nb, pitch = a.pitch, rows_smem = a.rows_smem;
@@ -64,52 +77,81 @@ __global__ void __launch_bounds__(kHistThreads, 1) resample_hist_pv_kernel(const
     __syncthreads();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
     const int fnx = a.f.nx, fny = a.f.ny;
-    const long long nf = (long long)a.f.nx * a.f.ny * a.f.nz;
-    const int pnx = a.m.nx + 2, pny = a.m.ny + 2;
+    const int rows_total = a.f.ny * a.f.nz;
+    const unsigned pnx = (unsigned)a.m.nx + 2u, pny = (unsigned)a.m.ny + 2u;
+    // padded index of cell (jx+1, jy+1, jz+1) from the raw float bits T_k = magic + j_k (as in resample_quad_kernel)
+    const unsigned fold = (unsigned)(kFloorMagicBits - 1) * (pny * pnx + pnx + 1u);
     const float hx = __fsub_rn((float)a.m.nx, 0.5f), hy = __fsub_rn((float)a.m.ny, 0.5f), hz = __fsub_rn((float)a.m.nz, 0.5f);
+    const uint32_t* __restrict__ quad = a.mbins_quad;
+    const float flane = (float)lane;
     const long long nitems = (long long)a.n_transforms * a.nchunks;
     for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
         const int t = (int)(item / a.nchunks);
         const int chunk = (int)(item - (long long)t * a.nchunks);
-        const long long v_lo = (long long)chunk * kPvChunkVoxels;
-        const long long v_hi = v_lo + kPvChunkVoxels < nf ? v_lo + kPvChunkVoxels : nf;
+        const int row_lo = chunk * a.rows_per_chunk;
+        const int row_hi = min(row_lo + a.rows_per_chunk, rows_total);
         float m[12];
 #pragma unroll
         for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
         unsigned long long* gh = a.hist + (size_t)t * nb * nb;
-        for (long long v0 = v_lo + warp * 32; v0 < v_hi; v0 += nwarps * 32) {
-            const long long v = v0 + lane;
-            if (v >= v_hi) continue;
-            const int ix = (int)(v % fnx);
-            const long long row = v / fnx;
-            const int iy = (int)(row % fny), iz = (int)(row / fny);
-            if (a.mask_bits != nullptr && ((__ldg(a.mask_bits + (v >> 5)) >> (v & 31)) & 1u) == 0u) continue;
-            const float fx = (float)ix, fy = (float)iy, fz = (float)iz;
-            // CANON-2
-            const float cx = __fmaf_rn(m[0], fx, __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3])));
-            const float cy = __fmaf_rn(m[4], fx, __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7])));
-            const float cz = __fmaf_rn(m[8], fx, __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11])));
-            const PvAxis ax = pv_axis(cx, hx), ay = pv_axis(cy, hy), az = pv_axis(cz, hz);
-            if (!(ax.ok && ay.ok && az.ok)) continue;
-            const int fa = __ldg(a.fbins_ranked + v);
-            const uint8_t* __restrict__ p = a.mbins_pad + ((size_t)az.lower * pny + ay.lower) * pnx + ax.lower;
-            const uint8_t* __restrict__ pz = p + (size_t)pnx * pny;
-            const unsigned b000 = __ldg(p), b100 = __ldg(p + 1), b010 = __ldg(p + pnx), b110 = __ldg(p + pnx + 1);
-            const unsigned b001 = __ldg(pz), b101 = __ldg(pz + 1), b011 = __ldg(pz + pnx), b111 = __ldg(pz + pnx + 1);
-            const unsigned wy0z0 = ay.w0 * az.w0, wy1z0 = ay.w1 * az.w0, wy0z1 = ay.w0 * az.w1, wy1z1 = ay.w1 * az.w1;
-            const unsigned bins[8] = {b000, b100, b010, b110, b001, b101, b011, b111};
-            const unsigned wts[8] = {ax.w0 * wy0z0, ax.w1 * wy0z0, ax.w0 * wy1z0, ax.w1 * wy1z0,
-                                     ax.w0 * wy0z1, ax.w1 * wy0z1, ax.w0 * wy1z1, ax.w1 * wy1z1};
-            if (fa < rows_smem) {
-                uint32_t* row_ptr = sh_hist + fa * pitch;
+        for (int row = row_lo + warp; row < row_hi; row += nwarps) {
+            const int iz = row / fny, iy = row - iz * fny;
+            const float fy = (float)iy, fz = (float)iz;
+            // CANON-2: row terms, then one fma per voxel and axis
+            const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
+            const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
+            const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
+            const uint8_t* __restrict__ frow = a.fbins_ranked + (size_t)row * (unsigned)fnx;
+            float fx0 = flane;
+            for (unsigned ix0 = (unsigned)lane; ix0 < (unsigned)fnx; ix0 += 32u * kPvUnroll, fx0 += (float)(32 * kPvUnroll)) {
+                PvAxis ax[kPvUnroll], ay[kPvUnroll], az[kPvUnroll];
+                unsigned idx[kPvUnroll];
+                bool ok[kPvUnroll];
 #pragma unroll
-                for (int k = 0; k < 8; ++k)
-                    if (wts[k]) atomicAdd(row_ptr + bins[k], wts[k]);
-            } else {
-                unsigned long long* grow = gh + (size_t)__ldg(a.rank_inv + fa) * nb;
+                for (int u = 0; u < kPvUnroll; ++u) {
+                    const float fx = fx0 + (float)(32 * u);
+                    ax[u] = pv_axis(__fmaf_rn(m[0], fx, rx), hx);
+                    ay[u] = pv_axis(__fmaf_rn(m[4], fx, ry), hy);
+                    az[u] = pv_axis(__fmaf_rn(m[8], fx, rz), hz);
+                    bool v = ax[u].ok && ay[u].ok && az[u].ok && (ix0 + 32u * u < (unsigned)fnx);
+                    if (MASK) {
+                        const unsigned vi = (unsigned)row * (unsigned)fnx + min(ix0 + 32u * u, (unsigned)fnx - 1u);
+                        v = v && ((__ldg(a.mask_bits + (vi >> 5)) >> (vi & 31u)) & 1u);
+                    }
+                    const unsigned i = (az[u].tbits * pny + ay[u].tbits) * pnx + ax[u].tbits - fold;
+                    idx[u] = v ? i : 0u;
+                    ok[u] = v;
+                }
+                uint32_t q0[kPvUnroll], q1[kPvUnroll];
+                unsigned fa[kPvUnroll];
 #pragma unroll
-                for (int k = 0; k < 8; ++k)
-                    if (wts[k]) atomicAdd(grow + bins[k], (unsigned long long)wts[k]);
+                for (int u = 0; u < kPvUnroll; ++u) {
+                    q0[u] = __ldg(quad + idx[u]);
+                    q1[u] = __ldg(quad + idx[u] + 1);
+                    fa[u] = ok[u] ? (unsigned)__ldg(frow + ix0 + 32u * u) : 0u;
+                }
+#pragma unroll
+                for (int u = 0; u < kPvUnroll; ++u) {
+                    if (!ok[u]) continue;
+                    const unsigned wy0z0 = ay[u].w0 * az[u].w0, wy1z0 = ay[u].w1 * az[u].w0;
+                    const unsigned wy0z1 = ay[u].w0 * az[u].w1, wy1z1 = ay[u].w1 * az[u].w1;
+                    // neighbour (dx,dy,dz): byte dy + 2 dz of entry x + dx; same order as the oracle's loops
+                    const unsigned bins[8] = {q0[u] & 0xFFu, q1[u] & 0xFFu, (q0[u] >> 8) & 0xFFu, (q1[u] >> 8) & 0xFFu,
+                                              (q0[u] >> 16) & 0xFFu, (q1[u] >> 16) & 0xFFu, q0[u] >> 24, q1[u] >> 24};
+                    const unsigned wts[8] = {ax[u].w0 * wy0z0, ax[u].w1 * wy0z0, ax[u].w0 * wy1z0, ax[u].w1 * wy1z0,
+                                             ax[u].w0 * wy0z1, ax[u].w1 * wy0z1, ax[u].w0 * wy1z1, ax[u].w1 * wy1z1};
+                    if ((int)fa[u] < rows_smem) {
+                        uint32_t* row_ptr = sh_hist + fa[u] * pitch;
+#pragma unroll
+                        for (int k = 0; k < 8; ++k)
+                            if (wts[k]) atomicAdd(row_ptr + bins[k], wts[k]);
+                    } else {
+                        unsigned long long* grow = gh + (size_t)__ldg(a.rank_inv + fa[u]) * nb;
+#pragma unroll
+                        for (int k = 0; k < 8; ++k)
+                            if (wts[k]) atomicAdd(grow + bins[k], (unsigned long long)wts[k]);
+                    }
+                }
             }
         }
         __syncthreads();
@@ -204,26 +246,34 @@ entropy_pv_kernel(const unsigned long long* __restrict__ hist, int nb, const dou
 
 }  // namespace
 
-cudaError_t launch_pad_replicate_u8(const uint8_t* src, uint8_t* dst, int nx, int ny, int nz, cudaStream_t s) {
+cudaError_t launch_bins_quad_build(const uint8_t* src, uint32_t* dst, int nx, int ny, int nz, cudaStream_t s) {
     const int64_t total = (int64_t)(nx + 2) * (ny + 2) * (nz + 2);
     int64_t blocks = (total + 255) / 256;
     if (blocks > sm_count() * 16) blocks = sm_count() * 16;
-    pad_replicate_u8_kernel<<<(unsigned)blocks, 256, 0, s>>>(src, dst, nx, ny, nz);
+    bins_quad_build_kernel<<<(unsigned)blocks, 256, 0, s>>>(src, dst, nx, ny, nz);
     return cudaGetLastError();
 }
 
 cudaError_t launch_resample_hist_pv(PvArgs a, int num_sms, cudaStream_t s) {
     if (a.rows_smem < 1 || a.pitch < a.nb || a.nb > 256) return cudaErrorInvalidConfiguration;
-    const long long nf = (long long)a.f.nx * a.f.ny * a.f.nz;
-    a.nchunks = (int)((nf + kPvChunkVoxels - 1) / kPvChunkVoxels);
+    // a chunk holds whole fixed rows and at most kPvChunkVoxels voxels: no u32 counter of the shared histogram can
+    // pass 2^32 before the chunk is merged (a row longer than that is split by the voxel count of one row only
+    // when fnx > kPvChunkVoxels, which mi_create's 2^31-voxel limit and this check exclude)
+    if (a.f.nx > kPvChunkVoxels) return cudaErrorInvalidConfiguration;
+    const int rows_total = a.f.ny * a.f.nz;
+    a.rows_per_chunk = kPvChunkVoxels / a.f.nx;
+    a.nchunks = (rows_total + a.rows_per_chunk - 1) / a.rows_per_chunk;
     const long long nitems = (long long)a.n_transforms * a.nchunks;
     if (nitems < 1) return cudaSuccess;
     const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
-    cudaError_t e = cudaFuncSetAttribute(resample_hist_pv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    const long long grid = nitems < num_sms ? nitems : num_sms;
-    resample_hist_pv_kernel<<<(unsigned)grid, kHistThreads, smem, s>>>(a);
-    return cudaGetLastError();
+    auto launch = [&](auto kern) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        const long long grid = nitems < num_sms ? nitems : num_sms;
+        kern<<<(unsigned)grid, kHistThreads, smem, s>>>(a);
+        return cudaGetLastError();
+    };
+    return a.mask_bits != nullptr ? launch(resample_hist_pv_kernel<true>) : launch(resample_hist_pv_kernel<false>);
 }
 
 cudaError_t launch_entropy_pv(const unsigned long long* hist, int nb, int n_transforms, const double* q_dev, int nq,
