@@ -327,7 +327,8 @@ mi_status mi_last_timing(const mi_ctx *ctx, float ms[5], int64_t launches[5]);
  * independent between the lanes of a warp (a hash of thread and update number) -- the roofline's
  * denominator; 2 all lanes on one address; 3 one linear congruential generator per thread seeded linearly in
  * the thread index (round 1's pattern: random in time, but the lanes of a warp form an arithmetic
- * progression, which spreads them over the banks more evenly than chance).  Host pointers. */
+ * progression, which spreads them over the banks more evenly than chance); 4 and 5 are patterns 2 and 1 with a
+ * per-lane VALUE added instead of 1 (the weighted update of partial-volume interpolation).  Host pointers. */
 mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
                                       double *updates_per_s);
 

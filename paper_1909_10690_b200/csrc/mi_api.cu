@@ -30,6 +30,7 @@ struct mi_ctx {
     float4* d_moving_quad = nullptr;    // its yz-quads (generic kernel, trilinear): 16 bytes per padded voxel
     uint8_t* d_mbins = nullptr;
     uint32_t* d_mbins_quad = nullptr;   // yz-quads of the replicate-padded moving bins (partial-volume interpolation)
+    int hot_mbin = 0;                   // most populated moving bin (partial-volume kernel's register-summed cell)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
     unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
     unsigned rare_alloc = 0;            // entries d_rare was allocated for
@@ -609,6 +610,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             pa.n_transforms = (int)cnt;
             pa.nchunks = 0;
             pa.rows_per_chunk = 0;
+            pa.hot_b = c->hot_mbin;
             MI_CUDA(c, mi::launch_resample_hist_pv(pa, c->num_sms, s));
         } else if (c->wide) {
             mi::WideArgs w;
@@ -833,6 +835,15 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if (!c->wide) {
             if ((e = dev_alloc((void**)&c->d_mbins_quad, (size_t)npad * sizeof(uint32_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bin quads"); break; }
             if ((e = mi::launch_bins_quad_build(c->d_mbins, c->d_mbins_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving bin quads"); break; }
+            {   // the most populated moving bin (d_counts is free again: the fixed counts are on the host)
+                unsigned long long h_mcounts[256];
+                if ((e = mi::launch_bin_count(c->d_mbins, nm, d_counts, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "count moving bins"); break; }
+                if ((e = cudaMemcpyAsync(h_mcounts, d_counts, sizeof(h_mcounts), cudaMemcpyDeviceToHost, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "copy moving counts"); break; }
+                if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "sync moving counts"); break; }
+                c->hot_mbin = 0;
+                for (int b = 1; b < nbins; ++b)
+                    if (h_mcounts[b] > h_mcounts[c->hot_mbin]) c->hot_mbin = b;
+            }
         }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
         if (!c->wide) {
@@ -1335,7 +1346,7 @@ mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms,
 
 mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
                                       double* updates_per_s) {
-    if (!updates_per_s || nbins < 8 || nbins > 256 || pattern < 0 || pattern > 3 || iters < 1)
+    if (!updates_per_s || nbins < 8 || nbins > 256 || pattern < 0 || pattern > 5 || iters < 1)
         return MI_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }

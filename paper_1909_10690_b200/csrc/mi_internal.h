@@ -116,7 +116,9 @@ struct PvArgs {
     VolumeDesc f, m;
     int nb, n_transforms;
     int nchunks, rows_per_chunk;  // set by the launcher: chunks of whole fixed rows per transform
+    int hot_b;                    // most populated moving bin: cell (fixed rank 0, hot_b) is summed in registers
 };
+cudaError_t launch_bin_count(const uint8_t* bins, int64_t n, unsigned long long* counts, cudaStream_t s);
 cudaError_t launch_bins_quad_build(const uint8_t* src, uint32_t* dst, int nx, int ny, int nz, cudaStream_t s);
 cudaError_t launch_resample_hist_pv(PvArgs a, int num_sms, cudaStream_t s);
 cudaError_t launch_entropy_pv(const unsigned long long* hist, int nb, int n_transforms, const double* q_dev, int nq,

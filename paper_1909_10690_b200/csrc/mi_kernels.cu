@@ -205,6 +205,16 @@ __global__ void __launch_bounds__(256) remap_bins_kernel(const uint8_t* __restri
     if (j < n) out[j] = lut[in[j]];
 }
 
+cudaError_t launch_bin_count(const uint8_t* bins, int64_t n, unsigned long long* counts, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(counts, 0, 256 * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return e;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks < 1) blocks = 1;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
+    bin_count_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, n, counts);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_rank_fixed_bins(const uint8_t* bins, int64_t n, unsigned long long* counts_scratch,
                                    uint8_t* rank, int* inv, uint8_t* ranked_bins, cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(counts_scratch, 0, 256 * sizeof(unsigned long long), s);
@@ -1009,10 +1019,17 @@ atomic_probe_kernel(int words_log2, int pattern, int iters, unsigned* __restrict
                 // wavefronts per update instead of 3.53)
                 state = state * 1664525u + 1013904223u;
                 idx = (state >> 10) & mask;
+            } else if (pattern == 5) {
+                unsigned x = tid * 0x9E3779B9u + (unsigned)(it + u) * 0x85EBCA6Bu;      // as pattern 1
+                x ^= x >> 16; x *= 0x7FEB352Du; x ^= x >> 15; x *= 0x846CA68Bu; x ^= x >> 16;
+                idx = x & mask;
             } else {
                 idx = same;
             }
-            atomicAdd(&sh_tab[idx], 1u);
+            // patterns 4 and 5 add a per-lane VALUE (the partial-volume kernel's weighted update, SASS ATOMS.ADD
+            // instead of ATOMS.POPC.INC)
+            if (pattern >= 4) atomicAdd(&sh_tab[idx], lane | 1u);
+            else atomicAdd(&sh_tab[idx], 1u);
         }
     }
     __syncthreads();

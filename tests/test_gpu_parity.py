@@ -744,3 +744,17 @@ def test_roofline_probes_order_and_random_bank_cost(mi):
     assert same > rand
     assert 0.25 < rand / free < 0.45, rand / free
     assert 1.15 < lcg / rand < 1.5, lcg / rand
+
+
+def test_fixed_volume_with_more_than_65535_slices(mi):
+    """mi.h: a fixed volume with nz > 65535 is accepted and its translation / scale maps take the generic kernel
+    (the separable kernels index z slices with 16 bits)."""
+    fixed = ph.random_volume((3, 2, 70000), 51)
+    moving = ph.random_volume((4, 3, 40), 52)
+    c = ph.Config("tall", fixed, moving, (1.0, 1.0, 0.001), (1.0, 1.0, 1.0), 32, 0, (-0.5, -0.5, -3.0), (0.5, 0.5, 3.0),
+                  (2, 1, 3), (0.5,), (0, 0, 0))
+    for interp in (0, 1):
+        check_map(mi, c, interp)
+    with make_ctx(mi, c.fixed, c.moving, c.fixed_spacing, c.moving_spacing, c.nbins, c.ranges) as ctx:
+        mi.mi_map(ctx, c.family, c.lo, c.hi, c.n, c.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 0
