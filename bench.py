@@ -40,14 +40,17 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # DRAM traffic of the dominant kernel from the committed `ncu --set full` captures of this command
-# (profiles/r2b_ncu.md): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch and the evaluations
+# (profiles/r2c_ncu.md): dram__bytes_read.sum + dram__bytes_write.sum of ONE launch and the evaluations
 # that launch performed; bench.py scales it to a step (bytes per evaluation x evaluations per step).
 # Keyed by (config, grid, interpolation).
 NCU_DRAM = {
-    # C5, zhist_kernel, launch = 5 of the 41 p0 slabs = 8405 transforms (profiles/r2b_ncu.md section 2:
-    # dram__bytes_read.sum 16.283806 GB + dram__bytes_write.sum 553.878528 MB)
-    ("C5", (41, 41, 41), 1): {"bytes_per_launch": 16283806000 + 553878528, "evals_per_launch": 8405 * 21023600,
-                               "source": "profiles/r2b_ncu.md"},
+    # C5, zhist_kernel, launch = 5 of the 41 p0 slabs = 8405 transforms (profiles/r2c_ncu.md section 3:
+    # dram__bytes_read.sum 16.282388 GB + dram__bytes_write.sum 553.706496 MB)
+    ("C5", (41, 41, 41), 1): {"bytes_per_launch": 16282388000 + 553706496, "evals_per_launch": 8405 * 21023600,
+                               "source": "profiles/r2c_ncu.md section 3"},
+    # C3, resample_quad_kernel, launch = the whole 15^3 map (profiles/r2c_ncu.md section 6: 9.950978 + 4.473929 GB)
+    ("C3", (15, 15, 15), 1): {"bytes_per_launch": 9950978000 + 4473929000, "evals_per_launch": 3375 * 21023600,
+                               "source": "profiles/r2c_ncu.md section 6"},
 }
 
 METRIC = "voxel-transform evaluations per second (MI map, 260x311x260 fixed, 256 bins)"

@@ -457,7 +457,7 @@ static cudaError_t launch_resample_t(const ResampleArgs& a, int num_sms, cudaStr
 // a3 + a4, trilinear, yz-quad gathers: the kernel rotations (and every other non-diagonal transform) take.
 // Same arithmetic as resample_hist_kernel<TRILINEAR> (CANON-2, CANON-4, CANON-5), organised so that the loads
 // of several samples are in flight per lane (the first version waited on memory with one pair in flight; as
-// committed the L1TEX data pipe is 91 % busy and the issue slots 82 %, profiles/r2b_ncu.md section 5) --
+// committed the L1TEX data pipe is 92 % busy and the issue slots 83 %, profiles/r2c_ncu.md section 6) --
 //   * every trip first resolves the cells of its U samples per lane and issues all 2U 16-byte loads (and the
 //     U fixed-bin loads), then lerps, bins and counts: U independent load pairs are in flight per lane (the
 //     64-register budget of a 1024-thread CTA made the compiler reuse one register set for all samples, i.e.

@@ -28,7 +28,7 @@ constexpr int kPvChunkVoxels = 131040;   // multiple of 32; 131040 * 32768 = 429
 // yz-quads of the replicate-padded moving BIN volume: entry (x,y,z) of the padded grid holds the bins of the padded
 // voxels (x,y,z), (x,y+1,z), (x,y,z+1), (x,y+1,z+1) in bytes 0..3 -- the entries x and x+1 are the eight neighbours of
 // a sample, two 4-byte loads instead of eight 1-byte gathers (the load/store unit writes 4 bytes per lane into the
-// register file whatever the access size, profiles/r2b_ncu.md section 5).
+// register file whatever the access size, profiles/r2c_ncu.md section 6).
 __global__ void __launch_bounds__(256) bins_quad_build_kernel(const uint8_t* __restrict__ src, uint32_t* __restrict__ dst,
                                                               int nx, int ny, int nz) {
     const int px = nx + 2, py = ny + 2, pz = nz + 2;

@@ -704,7 +704,7 @@ def test_separable_binning_variants_and_range_edges(mi):
             mg, _ = gpu_map(mi, c, interp, SEPARABLE=0)
             assert np.array_equal(ms, mg)
             # north_star's "__match_any_sync warp aggregation before shared atomics": the optional variant of
-            # the z kernel (profiles/r2b_ncu.md section 3 is why it is not the default) counts the same histograms
+            # the z kernel (profiles/r2c_ncu.md section 4 is why it is not the default) counts the same histograms
             ma, _ = gpu_map(mi, c, interp, FUSE_ENTROPY=0, ZHIST_MATCH_ANY=1)
             assert np.array_equal(ma, mg)
 
