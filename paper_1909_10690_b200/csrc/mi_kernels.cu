@@ -637,6 +637,146 @@ static cudaError_t launch_quad_threads(const ResampleArgs& a, int unroll, int nu
 #undef MI_QUAD
 }
 
+// ------------------------------------------------------------------------------------------------
+// a3 + a4, nearest neighbour, arbitrary 3x4: resample_quad_kernel's organisation (cells of the U samples of a lane
+// resolved first, all loads issued, then the updates through a 32-bit shared address) with CANON-3 sampling: the
+// moving bin is one byte of the pre-binned volume.  Same tiles, same slab-major item order.
+// ------------------------------------------------------------------------------------------------
+template <int U, bool MASK, bool RARE>
+__global__ void __launch_bounds__(kHistThreads, 1) resample_nn_kernel(const __grid_constant__ ResampleArgs a) {
+    extern __shared__ __align__(16) uint32_t sh_hist[];
+    constexpr int NW = kHistThreads / 32;
+    constexpr int TZ = NW / 8;
+    const int nb = a.nb, pitch = a.pitch, rows_smem = a.rows_smem;
+    const int words = rows_smem * pitch;
+    for (int w = threadIdx.x; w < words; w += kHistThreads) sh_hist[w] = 0u;
+    __syncthreads();
+    unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
+    asm volatile("" : "+r"(sbase));
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wy = warp & 7, wz = warp >> 3;
+    const int fnx = a.f.nx, fny = a.f.ny, fnz = a.f.nz;
+    const int tiles_y = (fny + 7) >> 3;
+    const int tiles_total = tiles_y * ((fnz + TZ - 1) / TZ);
+    const unsigned mnx = (unsigned)a.m.nx, mny = (unsigned)a.m.ny;
+    const float fmx = (float)a.m.nx, fmy = (float)a.m.ny, fmz = (float)a.m.nz;
+    // voxel index (jz*ny + jy)*nx + jx from the raw float bits T_k = magic + j_k, modulo 2^32
+    const unsigned fold = (unsigned)kFloorMagicBits * (mny * mnx + mnx + 1u);
+    const uint8_t* __restrict__ mbins = a.mbins;
+    const float flane = (float)lane;
+
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        const int slab = (int)(item / a.n_transforms);
+        const int t = (int)(item - (long long)slab * a.n_transforms);
+        const int tile_lo = (int)((long long)tiles_total * slab / a.nslabs);
+        const int tile_hi = (int)((long long)tiles_total * (slab + 1) / a.nslabs);
+        float m[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
+        uint32_t* gh = a.hist + (size_t)t * nb * nb;
+
+        int tz = tile_lo / tiles_y, ty = tile_lo - tz * tiles_y;
+        for (int tile = tile_lo; tile < tile_hi; ++tile, ++ty) {
+            if (ty == tiles_y) { ty = 0; ++tz; }
+            const int iy = (ty << 3) + wy, iz = tz * TZ + wz;
+            if (iy >= fny || iz >= fnz) continue;
+            const unsigned row = (unsigned)(iz * fny + iy);
+            const float fy = (float)iy, fz = (float)iz;
+            // CANON-2: row terms, then one fma per voxel and axis
+            const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
+            const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
+            const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
+            const uint8_t* __restrict__ frow = a.fbins_ranked + (size_t)row * (unsigned)fnx;
+            float fx0 = flane;
+            for (unsigned ix0 = (unsigned)lane; ix0 < (unsigned)fnx; ix0 += 32u * U, fx0 += (float)(32 * U)) {
+                unsigned idx[U];
+                bool ok[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const float fx = fx0 + (float)(32 * u);
+                    const float cx = __fmaf_rn(m[0], fx, rx), cy = __fmaf_rn(m[4], fx, ry), cz = __fmaf_rn(m[8], fx, rz);
+                    // CANON-3: r = floor(c + 0.5) (round half up), validity tested on r in float
+                    const float tx = __fadd_rd(__fadd_rn(cx, 0.5f), kFloorMagic);
+                    const float ty2 = __fadd_rd(__fadd_rn(cy, 0.5f), kFloorMagic);
+                    const float tz2 = __fadd_rd(__fadd_rn(cz, 0.5f), kFloorMagic);
+                    const float qx = __fsub_rn(tx, kFloorMagic), qy = __fsub_rn(ty2, kFloorMagic), qz = __fsub_rn(tz2, kFloorMagic);
+                    bool v = qx >= 0.0f && qx < fmx && qy >= 0.0f && qy < fmy && qz >= 0.0f && qz < fmz &&
+                             (ix0 + 32u * u < (unsigned)fnx);
+                    if (MASK) {
+                        const unsigned vi = row * (unsigned)fnx + min(ix0 + 32u * u, (unsigned)fnx - 1u);
+                        v = v && ((__ldg(a.mask_bits + (vi >> 5)) >> (vi & 31u)) & 1u);
+                    }
+                    const unsigned i = (__float_as_uint(tz2) * mny + __float_as_uint(ty2)) * mnx + __float_as_uint(tx) - fold;
+                    idx[u] = v ? i : 0u;
+                    ok[u] = v;
+                }
+                unsigned mb[U], fa[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    mb[u] = (unsigned)__ldg(mbins + idx[u]);
+                    fa[u] = ok[u] ? (unsigned)__ldg(frow + ix0 + 32u * u) : 0u;
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const unsigned cell = fa[u] * (unsigned)pitch + mb[u];
+                    if (!RARE) {
+                        if (ok[u]) red_shared_inc32(sbase + cell * 4u);
+                    } else {
+                        const bool in_smem = (int)fa[u] < rows_smem;
+                        if (ok[u] && in_smem) red_shared_inc32(sbase + cell * 4u);
+                        if (ok[u] && !in_smem) atomicAdd(&gh[__ldg(a.rank_inv + fa[u]) * nb + mb[u]], 1u);
+                    }
+                }
+            }
+        }
+        __syncthreads();
+        for (int r = warp; r < rows_smem; r += NW) {
+            uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
+            for (int b = lane; b < nb; b += 32) {
+                const uint32_t v = sh_hist[r * pitch + b];
+                if (v) {
+                    sh_hist[r * pitch + b] = 0u;
+                    atomicAdd(&grow[b], v);
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <int U, bool MASK, bool RARE>
+static cudaError_t launch_nn_t(const ResampleArgs& a, int num_sms, cudaStream_t s) {
+    const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
+    auto kern = resample_nn_kernel<U, MASK, RARE>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int carve = (int)((smem + 1024) * 100 / (228 * 1024));
+    if (carve > 100) carve = 100;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+    if (e != cudaSuccess) return e;
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    long long grid = nitems < num_sms ? nitems : num_sms;
+    if (grid < 1) return cudaSuccess;
+    kern<<<(unsigned)grid, kHistThreads, smem, s>>>(a);
+    return cudaGetLastError();
+}
+
+static cudaError_t launch_nn(const ResampleArgs& a, int unroll, int num_sms, cudaStream_t s) {
+    const bool mask = a.mask_bits != nullptr;
+#define MI_NN(UU)                                                                          \
+    do {                                                                                   \
+        if (mask) return launch_nn_t<UU, true, true>(a, num_sms, s);                       \
+        if (a.has_rare) return launch_nn_t<UU, false, true>(a, num_sms, s);                \
+        return launch_nn_t<UU, false, false>(a, num_sms, s);                               \
+    } while (0)
+    if (unroll == 1) MI_NN(1);
+    if (unroll == 2) MI_NN(2);
+    if (unroll == 3) MI_NN(3);
+    MI_NN(4);
+#undef MI_NN
+}
+
 int hist_rows_in_smem(int nb, int pitch, size_t smem_bytes) {
     const size_t reserve = 1024;  // static shared memory + alignment slack
     size_t rows = (smem_bytes > reserve ? smem_bytes - reserve : 0) / ((size_t)pitch * sizeof(uint32_t));
@@ -660,6 +800,7 @@ cudaError_t launch_resample_hist(const ResampleArgs& a, int interp, int num_sms,
     }
     if (interp == MI_INTERP_NEAREST) {
         if (a.sink != nullptr) return cudaErrorInvalidConfiguration;
+        if (a.gather == kGatherQuad) return launch_nn(a, unroll, num_sms, s);   // MI_OPT_GENERIC_GATHER = 0: round 1's kernel
         if (unroll == 1) return launch_resample_t<MI_INTERP_NEAREST, 1, kGatherScalar, true>(a, num_sms, s);
         if (unroll == 2) return launch_resample_t<MI_INTERP_NEAREST, 2, kGatherScalar, true>(a, num_sms, s);
         if (unroll == 3) return launch_resample_t<MI_INTERP_NEAREST, 3, kGatherScalar, true>(a, num_sms, s);

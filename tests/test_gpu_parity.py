@@ -758,3 +758,29 @@ def test_fixed_volume_with_more_than_65535_slices(mi):
     with make_ctx(mi, c.fixed, c.moving, c.fixed_spacing, c.moving_spacing, c.nbins, c.ranges) as ctx:
         mi.mi_map(ctx, c.family, c.lo, c.hi, c.n, c.q, 1)
         assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 0
+
+
+def test_generic_kernel_variants_count_the_same_histograms(mi):
+    """Every selectable variant of the generic (arbitrary 3x4) path -- yz-quad or scalar gathers, the reorganised or
+    round 1's nearest-neighbour kernel (MI_OPT_GENERIC_GATHER), CTA sizes, samples in flight per lane, slab sizes --
+    against the oracle's histograms, on a ragged multimodal pair with 256 bins (some fixed-bin ranks have no shared
+    row) and on random volumes that fill every bin."""
+    cfg = ph.get_config("C5", res=0.25, grid_n=3)
+    rng = np.random.default_rng(11)
+    T = np.concatenate([rand_physical(rng, 4, shift=8.0), np.stack([orc.family_matrix(0, (3.2, -4.7, 1.1))])])
+    pairs = [(cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing),
+             (ph.random_volume((37, 21, 13), 61), ph.random_volume((30, 25, 17), 62), (1.0, 1.2, 0.9), (1.1, 1.0, 1.3))]
+    variants = [dict(GENERIC_GATHER=0), dict(GENERIC_GATHER=0, GENERIC_UNROLL=1), dict(GENERIC_THREADS=512),
+                dict(GENERIC_THREADS=768, GENERIC_UNROLL=2), dict(GENERIC_UNROLL=1), dict(GENERIC_UNROLL=4),
+                dict(GENERIC_SLAB_MB=1), dict(GENERIC_SMEM_KB=64), dict(GENERIC_TY_LOG2=2, GENERIC_GATHER=0)]
+    for fixed, moving, fs, ms in pairs:
+        M = orc.physical_to_index(T, fixed.shape[::-1], fs, moving.shape[::-1], ms)
+        ref = {interp: orc.eval_batch(fixed, moving, M, 256, 0, 1, 0, 1, interp, q=(0.5,), want_hist=True) for interp in (0, 1)}
+        for opts in variants:
+            with make_ctx(mi, fixed, moving, fs, ms, 256) as ctx:
+                set_options(mi, ctx, **opts)
+                for interp in (0, 1):
+                    vals, hist, nvalid = mi.mi_eval_batch(ctx, T, (0.5,), interp, hist_out=True, nvalid_out=True)
+                    assert np.array_equal(hist, ref[interp]["hist"]), (opts, interp)
+                    assert np.array_equal(nvalid, ref[interp]["nvalid"]), (opts, interp)
+                    assert np.max(np.abs(vals - ref[interp]["mi"])) <= MI_TOL
