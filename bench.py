@@ -438,6 +438,15 @@ def run_ours(rt, args, cfg, interp, cpu_budget_s):
                          "peak_gathers_plus_updates": 1.0 / (1.0 / g_rate + 1.0 / r_rand) / 1e9,
                          "frac_of_gathers_plus_updates": achieved * (1.0 / g_rate + 1.0 / r_rand),
                          "t_lsu_gather_nominal_ms": t_lsu * 1e3})
+        # hardware floor of ANY kernel that brings eight fp32 neighbours per sample into registers: the load/store
+        # unit writes 64 B per clock per SM into the register file (profiles/r2c_ncu.md section 6), a warp-wide
+        # sample needs 32 x 32 B of neighbours + 128 B of fixed bins = 18 beats, + 2.41 crossbar wavefronts for its update
+        clk_per_warp_sample = (32 * 32 + 128) / 64.0 + 2.41
+        floor_rate = rt.num_sms * sm_hz * 32.0 / clk_per_warp_sample
+        roofline["writeback_floor"] = {"clocks_per_warp_sample": clk_per_warp_sample, "rate": floor_rate / 1e9,
+                                       "unit": "G trilinear samples/s", "frac": achieved / floor_rate,
+                                       "source": "64 B/clk/SM register-file writeback (ncu: l1tex__lsu_writeback_active), "
+                                                 "148 SMs at the sampled SM clock"}
 
     eval_batch = None
     if path == 0 and interp == 1:
