@@ -525,6 +525,19 @@ def test_partial_volume_interpolation_against_oracle(mi):
         assert ei.value.status == mi.MI_ERR_UNSUPPORTED
 
 
+def test_partial_volume_full_size_histograms(mi):
+    """Partial-volume interpolation at the full C3 and C5 sizes (161 row chunks per transform, the register-summed
+    background cell at scale): uint64 histograms bit-exact against the oracle at three grid nodes each."""
+    for name, nodes in (("C3", [(0, 0, 0), (11, 4, 9), (14, 14, 14)]), ("C5", [(0, 0, 0), (26, 11, 22), (40, 40, 40)])):
+        cfg = ph.get_config(name)
+        T = np.stack([orc.family_matrix(cfg.family, node_param(cfg, node)) for node in nodes])
+        ref = oracle_nodes(cfg, nodes, orc.INTERP_PARTIAL_VOLUME, q=(0.5,), want_hist=True)
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 256) as ctx:
+            vals, hist, nvalid = mi.mi_eval_batch_pv(ctx, T, (0.5,), hist_out=True, nvalid_out=True)
+        assert np.array_equal(hist, ref["hist"]) and np.array_equal(nvalid, ref["nvalid"])
+        assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
+
+
 def test_affine12_composite_grid_full_3_to_the_12(mi):
     """The paper's 12-dimensional exhaustive idea: all 3^12 = 531441 combinations of a minus,
     zero and plus step on the 12 entries of [A|t], evaluated in full on the C1 pair through
