@@ -469,6 +469,28 @@ def test_wide_histograms_above_256_bins(mi):
         check_map(mi, c, interp)
 
 
+def test_wide_histograms_full_size_4096_bins(mi):
+    """The "full histogram" of PAPER.md:212 at one bin per level of 12-bit data: 4096 bins at the full C3 size
+    (64 MB of counters per transform in global memory), two rotation nodes, nearest neighbour bit-exact and
+    trilinear within the flip allowance, MI within 1e-4 nats."""
+    c3 = ph.get_config("C3")
+    cfg = ph.Config("C3w", c3.fixed, c3.moving, c3.fixed_spacing, c3.moving_spacing, 4096, c3.family, c3.lo, c3.hi, c3.n,
+                    (0.5,), c3.truth)
+    nodes = [(3, 12, 7), (11, 4, 9)]
+    T = np.stack([orc.family_matrix(cfg.family, node_param(cfg, node)) for node in nodes])
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 4096) as ctx:
+        for interp in (0, 1):
+            ref = oracle_nodes(cfg, nodes, interp, want_hist=True)
+            vals, hist, nvalid = mi.mi_eval_batch(ctx, T, cfg.q, interp, hist_out=True, nvalid_out=True)
+            assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 2
+            if interp == 0:
+                assert np.array_equal(hist, ref["hist"]) and np.array_equal(nvalid, ref["nvalid"])
+            else:
+                moved = np.abs(hist.astype(np.int64) - ref["hist"].astype(np.int64)).sum(axis=(1, 2)) / 2
+                assert np.all(moved <= FLIP_FRAC * cfg.fixed.size), moved
+            assert np.max(np.abs(vals - ref["mi"])) <= MI_TOL
+
+
 def test_partial_volume_interpolation_against_oracle(mi):
     """MI_INTERP_PARTIAL_VOLUME (reading A21): integer histograms in units of 2^-15 voxel, bit-exact against the
     oracle for random affines (ragged sizes, several voxel chunks per transform, rare fixed-bin rows, a
