@@ -532,6 +532,7 @@ def main():
     ap.add_argument("--res", type=float, default=1.0, help="development only: reduced-resolution phantom")
     ap.add_argument("--grid", type=int, default=0, help="development only: grid nodes per axis")
     ap.add_argument("--interp", default="trilinear", choices=["trilinear", "nearest", "pv"])
+    ap.add_argument("--nbins", type=int, default=0, help="development only: override the config's bin count (e.g. 4096)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="experiments only: mi_set_option(MI_OPT_<NAME>, VALUE) on the context, e.g. zhist_match_any=1")
@@ -552,7 +553,11 @@ def main():
             kw["res"] = args.res
         if args.grid:
             kw["grid_n"] = args.grid
-        return ph.get_config(name, **kw)
+        cfg = ph.get_config(name, **kw)
+        if args.nbins:
+            import dataclasses
+            cfg = dataclasses.replace(cfg, nbins=args.nbins)
+        return cfg
 
     if args.impl == "reference":
         for name in names:

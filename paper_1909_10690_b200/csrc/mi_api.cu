@@ -31,6 +31,7 @@ struct mi_ctx {
     uint8_t* d_mbins = nullptr;
     uint32_t* d_mbins_quad = nullptr;   // yz-quads of the replicate-padded moving bins (partial-volume interpolation)
     int hot_mbin = 0;                   // most populated moving bin (partial-volume kernel's register-summed cell)
+    unsigned wide_hot_key = 0xFFFFFFFFu; // nbins > 256: (most populated fixed bin) * nb + (most populated moving bin)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
     unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
     unsigned rare_alloc = 0;            // entries d_rare was allocated for
@@ -498,7 +499,7 @@ int generic_nslabs(const mi_ctx* c, int64_t cnt, int interp) {
         nslabs = (int)((want + cnt - 1) / cnt);
         if (nslabs > cap) nslabs = cap;
     }
-    if (interp == MI_INTERP_TRILINEAR && !c->wide && c->opt_gather == 1 && c->opt_slab_mb > 0) {
+    if (interp == MI_INTERP_TRILINEAR && c->opt_gather == 1 && c->opt_slab_mb > 0) {
         const size_t quad_bytes = (size_t)(c->md[0] + 2) * (c->md[1] + 2) * (c->md[2] + 2) * sizeof(float4);
         const int by_l2 = (int)((quad_bytes + ((size_t)c->opt_slab_mb << 20) - 1) / ((size_t)c->opt_slab_mb << 20));
         if (by_l2 > nslabs) nslabs = by_l2 < cap ? by_l2 : cap;
@@ -627,6 +628,10 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             w.mscale = c->mscale;
             w.n_transforms = (int)cnt;
             w.nslabs = nslabs;
+            w.moving_quad = c->d_moving_quad;
+            w.hot_key = c->wide_hot_key;
+            w.version = c->opt_gather == 1 ? 2 : 1;
+            w.unroll = c->opt_unroll;
             MI_CUDA(c, mi::launch_resample_hist_wide(w, interp, c->num_sms, s));
         } else {
             MI_CUDA(c, mi::launch_resample_hist(a, interp, c->num_sms, s));
@@ -794,7 +799,7 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         if ((e = dev_alloc((void**)&c->d_fbins_ranked, (size_t)nf + 16, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc ranked bins"); break; }
         if ((e = dev_alloc((void**)&c->d_rank, 256, device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank"); break; }
         if ((e = dev_alloc((void**)&c->d_rank_inv, 256 * sizeof(int), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc rank_inv"); break; }
-        if ((e = dev_alloc((void**)&d_counts, 256 * sizeof(unsigned long long), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc counts"); break; }
+        if ((e = dev_alloc((void**)&d_counts, mi::kMaxBinsWide * sizeof(unsigned long long), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc counts"); break; }
         if ((e = dev_alloc((void**)&c->d_moving_pad, (size_t)npad * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc padded moving"); break; }
         if ((e = dev_alloc((void**)&d_mov, (size_t)nm * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving"); break; }
         if ((e = dev_alloc((void**)&d_tmp, (size_t)nf * sizeof(float), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc staging"); break; }
@@ -813,6 +818,20 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             if ((e = dev_alloc((void**)&c->d_mbins16, (size_t)nm * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide moving bins"); break; }
             if ((e = mi::launch_prebin16(d_tmp, c->d_fbins16, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed (wide)"); break; }
             if ((e = mi::launch_prebin16(d_mov, c->d_mbins16, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving (wide)"); break; }
+            {   // the most populated fixed and moving bins: the cell resample_wide_kernel counts in registers
+                std::vector<unsigned long long> h_c(mi::kMaxBinsWide);
+                int hot[2] = {0, 0};
+                bool failed = false;
+                for (int which = 0; which < 2 && !failed; ++which) {
+                    if ((e = mi::launch_bin_count16(which == 0 ? c->d_fbins16 : c->d_mbins16, which == 0 ? nf : nm, d_counts, s)) != cudaSuccess ||
+                        (e = cudaMemcpyAsync(h_c.data(), d_counts, h_c.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s)) != cudaSuccess ||
+                        (e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "count wide bins"); failed = true; break; }
+                    for (int b = 1; b < nbins; ++b)
+                        if (h_c[b] > h_c[hot[which]]) hot[which] = b;
+                }
+                if (failed) break;
+                c->wide_hot_key = (unsigned)hot[0] * (unsigned)nbins + (unsigned)hot[1];
+            }
         } else {
             if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, nullptr, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
             if ((e = mi::launch_prebin(d_mov, c->d_mbins, nm, c->mlo, c->mscale, nbins, reinterpret_cast<unsigned*>(d_counts), s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving"); break; }
@@ -846,10 +865,8 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             }
         }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
-        if (!c->wide) {
-            if ((e = dev_alloc((void**)&c->d_moving_quad, (size_t)npad * sizeof(float4), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving quads"); break; }
-            if ((e = mi::launch_quad_build(c->d_moving_pad, c->d_moving_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving quads"); break; }
-        }
+        if ((e = dev_alloc((void**)&c->d_moving_quad, (size_t)npad * sizeof(float4), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving quads"); break; }
+        if ((e = mi::launch_quad_build(c->d_moving_pad, c->d_moving_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving quads"); break; }
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
     dev_free(d_tmp, c->stream);

@@ -1300,7 +1300,199 @@ __global__ void __launch_bounds__(512) resample_hist_wide_kernel(const __grid_co
     }
 }
 
+// 4096-bin population count of a uint16 volume (CTA-private shared histogram, merged with atomics): finds the
+// most populated fixed and moving bins of a wide context (resample_wide_kernel's register-summed cell).
+__global__ void __launch_bounds__(256) bin_count16_kernel(const uint16_t* __restrict__ bins, int64_t n,
+                                                          unsigned long long* __restrict__ counts) {
+    __shared__ unsigned sh[kMaxBinsWide];
+    for (int i = threadIdx.x; i < kMaxBinsWide; i += 256) sh[i] = 0u;
+    __syncthreads();
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        atomicAdd(&sh[bins[i] & (kMaxBinsWide - 1)], 1u);
+    __syncthreads();
+    for (int i = threadIdx.x; i < kMaxBinsWide; i += 256)
+        if (sh[i]) atomicAdd(&counts[i], (unsigned long long)sh[i]);
+}
+
+cudaError_t launch_bin_count16(const uint16_t* bins, int64_t n, unsigned long long* counts, cudaStream_t s) {
+    cudaError_t e = cudaMemsetAsync(counts, 0, kMaxBinsWide * sizeof(unsigned long long), s);
+    if (e != cudaSuccess) return e;
+    int64_t blocks = (n + 255) / 256;
+    if (blocks < 1) blocks = 1;
+    if (blocks > sm_count() * 8) blocks = sm_count() * 8;
+    bin_count16_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, n, counts);
+    return cudaGetLastError();
+}
+
+// Wide histograms, second version: resample_quad_kernel's organisation (rows of an 8 x 4 tile per CTA pass, the cells
+// of U samples per lane resolved first, all loads issued -- two 16-byte yz-quad loads per trilinear sample, one
+// 2-byte load per nearest-neighbour sample -- slab-major items) with the counters in global memory.  Instead of
+// __match_any_sync before every update (about 50 clocks per warp-wide update), the ONE cell that serialises in L2 --
+// (most populated fixed bin, most populated moving bin): the background, a quarter of all updates -- is counted in a
+// register per lane and added once per item; every other update is a plain L2 reduction.
+template <int INTERP, int U, bool MASK>
+__global__ void __launch_bounds__(kHistThreads, 1) resample_wide_kernel(const __grid_constant__ WideArgs a) {
+    constexpr int NW = kHistThreads / 32;
+    constexpr int TZ = NW / 8;
+    const int nb = a.nb;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int wy = warp & 7, wz = warp >> 3;
+    const int fnx = a.f.nx, fny = a.f.ny, fnz = a.f.nz;
+    const int tiles_y = (fny + 7) >> 3;
+    const int tiles_total = tiles_y * ((fnz + TZ - 1) / TZ);
+    const unsigned pnx = (unsigned)a.m.nx + 2u, pny = (unsigned)a.m.ny + 2u;
+    const unsigned mnx = (unsigned)a.m.nx, mny = (unsigned)a.m.ny;
+    const unsigned fold_pad = (unsigned)(kFloorMagicBits - 1) * (pny * pnx + pnx + 1u);   // see MovingView::fold
+    const unsigned fold_nn = (unsigned)kFloorMagicBits * (mny * mnx + mnx + 1u);
+    const float fmx = (float)a.m.nx, fmy = (float)a.m.ny, fmz = (float)a.m.nz;
+    const float hx = __fsub_rn(fmx, 0.5f), hy = __fsub_rn(fmy, 0.5f), hz = __fsub_rn(fmz, 0.5f);
+    const float mlo = a.mlo, mscale = a.mscale;
+    const int top = nb - 1;
+    const float4* __restrict__ quad = a.moving_quad;
+    const uint16_t* __restrict__ mbins = a.mbins;
+    const unsigned hot_key = a.hot_key;
+    const float flane = (float)lane;
+
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    for (long long item = blockIdx.x; item < nitems; item += gridDim.x) {
+        // slab-major: the SMs spread over the counters of ALL transforms of the call.  Grouping the transforms so
+        // that one group's counters stay L2-resident (16 transforms at 1024 bins, one at 4096) measured 35 / 92 ms
+        // against 24 / 45 ms on a 125-transform call at the C3 size: contention on the counters costs more than
+        // their L2 misses.
+        const int slab = (int)(item / a.n_transforms);
+        const int t = (int)(item - (long long)slab * a.n_transforms);
+        const int tile_lo = (int)((long long)tiles_total * slab / a.nslabs);
+        const int tile_hi = (int)((long long)tiles_total * (slab + 1) / a.nslabs);
+        float m[12];
+#pragma unroll
+        for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
+        uint32_t* gh = a.hist + (size_t)t * nb * nb;
+        unsigned hot_acc = 0u;
+
+        int tz = tile_lo / tiles_y, ty = tile_lo - tz * tiles_y;
+        for (int tile = tile_lo; tile < tile_hi; ++tile, ++ty) {
+            if (ty == tiles_y) { ty = 0; ++tz; }
+            const int iy = (ty << 3) + wy, iz = tz * TZ + wz;
+            if (iy >= fny || iz >= fnz) continue;
+            const unsigned row = (unsigned)(iz * fny + iy);
+            const float fy = (float)iy, fz = (float)iz;
+            // CANON-2: row terms, then one fma per voxel and axis
+            const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
+            const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
+            const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
+            const uint16_t* __restrict__ frow = a.fbins + (size_t)row * (unsigned)fnx;
+            float fx0 = flane;
+            for (unsigned ix0 = (unsigned)lane; ix0 < (unsigned)fnx; ix0 += 32u * U, fx0 += (float)(32 * U)) {
+                unsigned idx[U];
+                float wxs[U], wys[U], wzs[U];
+                bool ok[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const float fx = fx0 + (float)(32 * u);
+                    const float cx = __fmaf_rn(m[0], fx, rx), cy = __fmaf_rn(m[4], fx, ry), cz = __fmaf_rn(m[8], fx, rz);
+                    bool v;
+                    unsigned i;
+                    if (INTERP == MI_INTERP_NEAREST) {
+                        // CANON-3: r = floor(c + 0.5) (round half up), validity tested on r in float
+                        const float tx = __fadd_rd(__fadd_rn(cx, 0.5f), kFloorMagic);
+                        const float ty2 = __fadd_rd(__fadd_rn(cy, 0.5f), kFloorMagic);
+                        const float tz2 = __fadd_rd(__fadd_rn(cz, 0.5f), kFloorMagic);
+                        const float qx = __fsub_rn(tx, kFloorMagic), qy = __fsub_rn(ty2, kFloorMagic), qz = __fsub_rn(tz2, kFloorMagic);
+                        v = qx >= 0.0f && qx < fmx && qy >= 0.0f && qy < fmy && qz >= 0.0f && qz < fmz;
+                        i = (__float_as_uint(tz2) * mny + __float_as_uint(ty2)) * mnx + __float_as_uint(tx) - fold_nn;
+                        wxs[u] = wys[u] = wzs[u] = 0.0f;
+                    } else {
+                        // CANON-4: region [-0.5, n-0.5), edge clamp (via the padded copy)
+                        v = cx >= -0.5f && cx < hx && cy >= -0.5f && cy < hy && cz >= -0.5f && cz < hz;
+                        const float tx = __fadd_rd(cx, kFloorMagic), ty2 = __fadd_rd(cy, kFloorMagic), tz2 = __fadd_rd(cz, kFloorMagic);
+                        wxs[u] = __fsub_rn(cx, __fsub_rn(tx, kFloorMagic));
+                        wys[u] = __fsub_rn(cy, __fsub_rn(ty2, kFloorMagic));
+                        wzs[u] = __fsub_rn(cz, __fsub_rn(tz2, kFloorMagic));
+                        i = (__float_as_uint(tz2) * pny + __float_as_uint(ty2)) * pnx + __float_as_uint(tx) - fold_pad;
+                    }
+                    v = v && (ix0 + 32u * u < (unsigned)fnx);
+                    if (MASK) {
+                        const unsigned vi = row * (unsigned)fnx + min(ix0 + 32u * u, (unsigned)fnx - 1u);
+                        v = v && ((__ldg(a.mask_bits + (vi >> 5)) >> (vi & 31u)) & 1u);
+                    }
+                    idx[u] = v ? i : 0u;
+                    ok[u] = v;
+                }
+                float4 q0[U], q1[U];
+                unsigned mb[U], fa[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    if (INTERP == MI_INTERP_NEAREST) {
+                        mb[u] = (unsigned)__ldg(mbins + idx[u]);
+                    } else {
+                        q0[u] = __ldg(quad + idx[u]);
+                        q1[u] = __ldg(quad + idx[u] + 1);
+                    }
+                    fa[u] = ok[u] ? (unsigned)__ldg(frow + ix0 + 32u * u) : 0u;
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    unsigned b;
+                    if (INTERP == MI_INTERP_NEAREST) {
+                        b = mb[u];
+                    } else {
+                        // x-, y-, z-lerps (CANON-4 order), binning (CANON-5)
+                        const float v00 = lerp_rn(q0[u].x, q1[u].x, wxs[u]);
+                        const float v10 = lerp_rn(q0[u].y, q1[u].y, wxs[u]);
+                        const float v01 = lerp_rn(q0[u].z, q1[u].z, wxs[u]);
+                        const float v11 = lerp_rn(q0[u].w, q1[u].w, wxs[u]);
+                        const float w0 = lerp_rn(v00, v10, wys[u]);
+                        const float w1 = lerp_rn(v01, v11, wys[u]);
+                        const float v = lerp_rn(w0, w1, wzs[u]);
+                        const float tt = __fmul_rn(__fsub_rn(v, mlo), mscale);
+                        b = (unsigned)min(max(__float2int_rd(tt), 0), top);
+                    }
+                    const unsigned key = fa[u] * (unsigned)nb + b;
+                    const bool hot = key == hot_key;
+                    hot_acc += (ok[u] && hot) ? 1u : 0u;
+                    if (ok[u] && !hot) atomicAdd(&gh[key], 1u);
+                }
+            }
+        }
+        hot_acc = warp_sum(hot_acc);
+        if (lane == 0 && hot_acc) atomicAdd(&gh[hot_key], hot_acc);
+    }
+}
+
+template <int INTERP>
+static cudaError_t launch_wide2(const WideArgs& a, int unroll, int num_sms, cudaStream_t s) {
+    const long long nitems = (long long)a.n_transforms * a.nslabs;
+    long long grid = nitems < num_sms ? nitems : num_sms;
+    if (grid < 1) return cudaSuccess;
+    const bool mask = a.mask_bits != nullptr;
+#define MI_WIDE(UU)                                                                                              \
+    do {                                                                                                         \
+        if (mask) resample_wide_kernel<INTERP, UU, true><<<(unsigned)grid, kHistThreads, 0, s>>>(a);             \
+        else resample_wide_kernel<INTERP, UU, false><<<(unsigned)grid, kHistThreads, 0, s>>>(a);                 \
+        return cudaGetLastError();                                                                               \
+    } while (0)
+    if (unroll == 1) MI_WIDE(1);
+    if (unroll == 2) MI_WIDE(2);
+    if (unroll == 3) MI_WIDE(3);
+    MI_WIDE(4);
+#undef MI_WIDE
+}
+
 cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s) {
+    if (a.version == 2 && a.moving_quad != nullptr) {
+        // samples in flight per lane: as in launch_resample_hist (fewest idle chunks in the last trip of a row)
+        int unroll = a.unroll;
+        if (unroll < 1 || unroll > 4) {
+            const int chunks = (a.f.nx + 31) / 32;
+            int best_waste = 1 << 30;
+            for (int u = 1; u <= 4; ++u) {
+                const int waste = (chunks + u - 1) / u * u - chunks;
+                if (waste <= best_waste) { best_waste = waste; unroll = u; }
+            }
+        }
+        return interp == MI_INTERP_NEAREST ? launch_wide2<MI_INTERP_NEAREST>(a, unroll, num_sms, s)
+                                           : launch_wide2<MI_INTERP_TRILINEAR>(a, unroll, num_sms, s);
+    }
     const long long nitems = (long long)a.n_transforms * a.nslabs;
     long long grid = nitems < 4LL * num_sms ? nitems : 4LL * num_sms;
     if (grid < 1) return cudaSuccess;
