@@ -3,6 +3,7 @@
 // No step of the path runs on the CPU except a2 (12 numbers per transform, in double).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -31,7 +32,8 @@ struct mi_ctx {
     uint8_t* d_mbins = nullptr;
     uint32_t* d_mbins_quad = nullptr;   // yz-quads of the replicate-padded moving bins (partial-volume interpolation)
     int hot_mbin = 0;                   // most populated moving bin (partial-volume kernel's register-summed cell)
-    unsigned wide_hot_key = 0xFFFFFFFFu; // nbins > 256: (most populated fixed bin) * nb + (most populated moving bin)
+    uint16_t* d_fbins16_ranked = nullptr; // nbins > 256: fixed bins replaced by their population rank
+    int* d_wrank_inv = nullptr;          // nbins > 256: rank -> fixed bin (kMaxBinsWide entries)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
     unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
     unsigned rare_alloc = 0;            // entries d_rare was allocated for
@@ -629,7 +631,10 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
             w.n_transforms = (int)cnt;
             w.nslabs = nslabs;
             w.moving_quad = c->d_moving_quad;
-            w.hot_key = c->wide_hot_key;
+            w.fbins_ranked = c->d_fbins16_ranked;
+            w.rank_inv = c->d_wrank_inv;
+            w.rows_smem = c->rows_smem;
+            w.pitch = c->gpitch;
             w.version = c->opt_gather == 1 ? 2 : 1;
             w.unroll = c->opt_unroll;
             MI_CUDA(c, mi::launch_resample_hist_wide(w, interp, c->num_sms, s));
@@ -818,19 +823,28 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             if ((e = dev_alloc((void**)&c->d_mbins16, (size_t)nm * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide moving bins"); break; }
             if ((e = mi::launch_prebin16(d_tmp, c->d_fbins16, nf, c->flo, c->fscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed (wide)"); break; }
             if ((e = mi::launch_prebin16(d_mov, c->d_mbins16, nm, c->mlo, c->mscale, nbins, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin moving (wide)"); break; }
-            {   // the most populated fixed and moving bins: the cell resample_wide_kernel counts in registers
+            {   // rank the fixed bins by population (host: 4096 counts) and remap them: the most populated fixed
+                // bins get resample_wide_kernel's shared-memory rows
                 std::vector<unsigned long long> h_c(mi::kMaxBinsWide);
-                int hot[2] = {0, 0};
+                if ((e = mi::launch_bin_count16(c->d_fbins16, nf, d_counts, s)) != cudaSuccess ||
+                    (e = cudaMemcpyAsync(h_c.data(), d_counts, h_c.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s)) != cudaSuccess ||
+                    (e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "count wide bins"); break; }
+                std::vector<int> order(mi::kMaxBinsWide);
+                for (int b = 0; b < mi::kMaxBinsWide; ++b) order[b] = b;
+                std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return h_c[x] > h_c[y]; });
+                std::vector<uint16_t> h_rank(mi::kMaxBinsWide);
+                for (int r = 0; r < mi::kMaxBinsWide; ++r) h_rank[order[r]] = (uint16_t)r;
+                uint16_t* d_wrank = nullptr;
+                if ((e = dev_alloc((void**)&d_wrank, mi::kMaxBinsWide * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide ranks"); break; }
                 bool failed = false;
-                for (int which = 0; which < 2 && !failed; ++which) {
-                    if ((e = mi::launch_bin_count16(which == 0 ? c->d_fbins16 : c->d_mbins16, which == 0 ? nf : nm, d_counts, s)) != cudaSuccess ||
-                        (e = cudaMemcpyAsync(h_c.data(), d_counts, h_c.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s)) != cudaSuccess ||
-                        (e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "count wide bins"); failed = true; break; }
-                    for (int b = 1; b < nbins; ++b)
-                        if (h_c[b] > h_c[hot[which]]) hot[which] = b;
-                }
+                if ((e = dev_alloc((void**)&c->d_wrank_inv, mi::kMaxBinsWide * sizeof(int), device, c->stream)) != cudaSuccess ||
+                    (e = dev_alloc((void**)&c->d_fbins16_ranked, (size_t)nf * sizeof(uint16_t), device, c->stream)) != cudaSuccess ||
+                    (e = cudaMemcpyAsync(d_wrank, h_rank.data(), h_rank.size() * sizeof(uint16_t), cudaMemcpyHostToDevice, s)) != cudaSuccess ||
+                    (e = cudaMemcpyAsync(c->d_wrank_inv, order.data(), order.size() * sizeof(int), cudaMemcpyHostToDevice, s)) != cudaSuccess ||
+                    (e = mi::launch_remap16(c->d_fbins16, c->d_fbins16_ranked, nf, d_wrank, s)) != cudaSuccess ||
+                    (e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank wide fixed bins"); failed = true; }
+                dev_free(d_wrank, c->stream);
                 if (failed) break;
-                c->wide_hot_key = (unsigned)hot[0] * (unsigned)nbins + (unsigned)hot[1];
             }
         } else {
             if ((e = mi::launch_prebin(d_tmp, c->d_fbins, nf, c->flo, c->fscale, nbins, nullptr, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "prebin fixed"); break; }
@@ -885,7 +899,7 @@ void mi_destroy(mi_ctx* c) {
     DeviceGuard guard(c->device);
     if (guard.ok) {
         void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mask_bits, c->d_fbins16, c->d_mbins16, c->d_mbins,
-                        c->d_mbins_quad, c->d_moving_quad, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
+                        c->d_mbins_quad, c->d_moving_quad, c->d_fbins16_ranked, c->d_wrank_inv, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);

@@ -81,10 +81,13 @@ struct WideArgs {
     float mlo, mscale;
     int n_transforms, nslabs;
     const float4* moving_quad;    // yz-quads of the padded moving volume (version 2, trilinear)
-    unsigned hot_key;             // version 2: fixed bin * nb + moving bin of the register-summed cell
+    const uint16_t* fbins_ranked; // version 2: fixed bins replaced by their population rank
+    const int* rank_inv;          // version 2: rank -> fixed bin
+    int rows_smem, pitch;         // version 2: ranked rows counted in shared memory, words per row
     int version, unroll;          // 2: resample_wide_kernel; 1: round 1's resample_hist_wide_kernel (MI_OPT_GENERIC_GATHER = 0)
 };
 cudaError_t launch_bin_count16(const uint16_t* bins, int64_t n, unsigned long long* counts, cudaStream_t s);
+cudaError_t launch_remap16(const uint16_t* bins, uint16_t* ranked, int64_t n, const uint16_t* rank, cudaStream_t s);
 cudaError_t launch_mask_bits(const uint8_t* mask, int64_t n, uint32_t* bits, cudaStream_t s);
 cudaError_t launch_prebin16(const float* vol, uint16_t* bins, int64_t n, float lo, float scale, int nb, cudaStream_t s);
 cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s);

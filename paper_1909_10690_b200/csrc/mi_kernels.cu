@@ -1324,17 +1324,39 @@ cudaError_t launch_bin_count16(const uint16_t* bins, int64_t n, unsigned long lo
     return cudaGetLastError();
 }
 
+// fixed bins -> population ranks (uint16): the most populated fixed bins get the shared-memory rows of
+// resample_wide_kernel
+__global__ void __launch_bounds__(256) remap16_kernel(const uint16_t* __restrict__ bins, uint16_t* __restrict__ ranked,
+                                                      int64_t n, const uint16_t* __restrict__ rank) {
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x)
+        ranked[i] = __ldg(rank + (bins[i] & (kMaxBinsWide - 1)));
+}
+
+cudaError_t launch_remap16(const uint16_t* bins, uint16_t* ranked, int64_t n, const uint16_t* rank, cudaStream_t s) {
+    int64_t blocks = (n + 255) / 256;
+    if (blocks < 1) blocks = 1;
+    if (blocks > sm_count() * 16) blocks = sm_count() * 16;
+    remap16_kernel<<<(unsigned)blocks, 256, 0, s>>>(bins, ranked, n, rank);
+    return cudaGetLastError();
+}
+
 // Wide histograms, second version: resample_quad_kernel's organisation (rows of an 8 x 4 tile per CTA pass, the cells
 // of U samples per lane resolved first, all loads issued -- two 16-byte yz-quad loads per trilinear sample, one
-// 2-byte load per nearest-neighbour sample -- slab-major items) with the counters in global memory.  Instead of
-// __match_any_sync before every update (about 50 clocks per warp-wide update), the ONE cell that serialises in L2 --
-// (most populated fixed bin, most populated moving bin): the background, a quarter of all updates -- is counted in a
-// register per lane and added once per item; every other update is a plain L2 reduction.
+// 2-byte load per nearest-neighbour sample -- slab-major items) with the counters in global memory.  Fixed bins
+// arrive RANKED by population: the rows of the a.rows_smem most populated fixed bins (48 rows at 1024 bins, 12 at 4096:
+// the background and the most common tissue levels) are counted in shared memory and added to the global histogram
+// once per item; every other update is a plain L2 reduction (round 1 ran __match_any_sync before every update,
+// about 50 clocks per warp-wide update).
 template <int INTERP, int U, bool MASK>
 __global__ void __launch_bounds__(kHistThreads, 1) resample_wide_kernel(const __grid_constant__ WideArgs a) {
+    extern __shared__ __align__(16) uint32_t sh_hist[];
     constexpr int NW = kHistThreads / 32;
     constexpr int TZ = NW / 8;
-    const int nb = a.nb;
+    const int nb = a.nb, pitch = a.pitch, rows_smem = a.rows_smem;
+    for (int w = threadIdx.x; w < rows_smem * pitch; w += kHistThreads) sh_hist[w] = 0u;
+    __syncthreads();
+    unsigned sbase = (unsigned)__cvta_generic_to_shared(sh_hist);
+    asm volatile("" : "+r"(sbase));
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int wy = warp & 7, wz = warp >> 3;
     const int fnx = a.f.nx, fny = a.f.ny, fnz = a.f.nz;
@@ -1350,7 +1372,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) resample_wide_kernel(const __
     const int top = nb - 1;
     const float4* __restrict__ quad = a.moving_quad;
     const uint16_t* __restrict__ mbins = a.mbins;
-    const unsigned hot_key = a.hot_key;
     const float flane = (float)lane;
 
     const long long nitems = (long long)a.n_transforms * a.nslabs;
@@ -1367,7 +1388,6 @@ __global__ void __launch_bounds__(kHistThreads, 1) resample_wide_kernel(const __
 #pragma unroll
         for (int i = 0; i < 12; ++i) m[i] = __ldg(a.M + (size_t)t * 12 + i);
         uint32_t* gh = a.hist + (size_t)t * nb * nb;
-        unsigned hot_acc = 0u;
 
         int tz = tile_lo / tiles_y, ty = tile_lo - tz * tiles_y;
         for (int tile = tile_lo; tile < tile_hi; ++tile, ++ty) {
@@ -1380,7 +1400,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) resample_wide_kernel(const __
             const float rx = __fmaf_rn(m[1], fy, __fmaf_rn(m[2], fz, m[3]));
             const float ry = __fmaf_rn(m[5], fy, __fmaf_rn(m[6], fz, m[7]));
             const float rz = __fmaf_rn(m[9], fy, __fmaf_rn(m[10], fz, m[11]));
-            const uint16_t* __restrict__ frow = a.fbins + (size_t)row * (unsigned)fnx;
+            const uint16_t* __restrict__ frow = a.fbins_ranked + (size_t)row * (unsigned)fnx;
             float fx0 = flane;
             for (unsigned ix0 = (unsigned)lane; ix0 < (unsigned)fnx; ix0 += 32u * U, fx0 += (float)(32 * U)) {
                 unsigned idx[U];
@@ -1447,15 +1467,25 @@ __global__ void __launch_bounds__(kHistThreads, 1) resample_wide_kernel(const __
                         const float tt = __fmul_rn(__fsub_rn(v, mlo), mscale);
                         b = (unsigned)min(max(__float2int_rd(tt), 0), top);
                     }
-                    const unsigned key = fa[u] * (unsigned)nb + b;
-                    const bool hot = key == hot_key;
-                    hot_acc += (ok[u] && hot) ? 1u : 0u;
-                    if (ok[u] && !hot) atomicAdd(&gh[key], 1u);
+                    const bool in_smem = (int)fa[u] < rows_smem;
+                    if (ok[u] && in_smem) red_shared_inc32(sbase + (fa[u] * (unsigned)pitch + b) * 4u);
+                    if (ok[u] && !in_smem) atomicAdd(&gh[(unsigned)__ldg(a.rank_inv + fa[u]) * (unsigned)nb + b], 1u);
                 }
             }
         }
-        hot_acc = warp_sum(hot_acc);
-        if (lane == 0 && hot_acc) atomicAdd(&gh[hot_key], hot_acc);
+        __syncthreads();
+        // the shared rows go to the transform's global histogram (un-ranking the fixed bin) and are zeroed again
+        for (int r = warp; r < rows_smem; r += NW) {
+            uint32_t* grow = gh + (size_t)__ldg(a.rank_inv + r) * nb;
+            for (int b = lane; b < nb; b += 32) {
+                const uint32_t v = sh_hist[r * pitch + b];
+                if (v) {
+                    sh_hist[r * pitch + b] = 0u;
+                    atomicAdd(&grow[b], v);
+                }
+            }
+        }
+        __syncthreads();
     }
 }
 
@@ -1465,21 +1495,33 @@ static cudaError_t launch_wide2(const WideArgs& a, int unroll, int num_sms, cuda
     long long grid = nitems < num_sms ? nitems : num_sms;
     if (grid < 1) return cudaSuccess;
     const bool mask = a.mask_bits != nullptr;
+    const size_t smem = (size_t)a.rows_smem * a.pitch * sizeof(uint32_t);
+    int carve = (int)((smem + 1024) * 100 / (228 * 1024));
+    if (carve > 100) carve = 100;
+#define MI_WIDE_K(KERN)                                                                                          \
+    do {                                                                                                         \
+        cudaError_t e = cudaFuncSetAttribute(KERN, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);      \
+        if (e != cudaSuccess) return e;                                                                          \
+        e = cudaFuncSetAttribute(KERN, cudaFuncAttributePreferredSharedMemoryCarveout, carve);                   \
+        if (e != cudaSuccess) return e;                                                                          \
+        KERN<<<(unsigned)grid, kHistThreads, smem, s>>>(a);                                                      \
+        return cudaGetLastError();                                                                               \
+    } while (0)
 #define MI_WIDE(UU)                                                                                              \
     do {                                                                                                         \
-        if (mask) resample_wide_kernel<INTERP, UU, true><<<(unsigned)grid, kHistThreads, 0, s>>>(a);             \
-        else resample_wide_kernel<INTERP, UU, false><<<(unsigned)grid, kHistThreads, 0, s>>>(a);                 \
-        return cudaGetLastError();                                                                               \
+        if (mask) MI_WIDE_K((resample_wide_kernel<INTERP, UU, true>));                                           \
+        else MI_WIDE_K((resample_wide_kernel<INTERP, UU, false>));                                               \
     } while (0)
     if (unroll == 1) MI_WIDE(1);
     if (unroll == 2) MI_WIDE(2);
     if (unroll == 3) MI_WIDE(3);
     MI_WIDE(4);
 #undef MI_WIDE
+#undef MI_WIDE_K
 }
 
 cudaError_t launch_resample_hist_wide(const WideArgs& a, int interp, int num_sms, cudaStream_t s) {
-    if (a.version == 2 && a.moving_quad != nullptr) {
+    if (a.version == 2 && a.moving_quad != nullptr && a.fbins_ranked != nullptr && a.rows_smem >= 1) {
         // samples in flight per lane: as in launch_resample_hist (fewest idle chunks in the last trip of a row)
         int unroll = a.unroll;
         if (unroll < 1 || unroll > 4) {
