@@ -34,6 +34,7 @@ struct mi_ctx {
     int hot_mbin = 0;                   // most populated moving bin (partial-volume kernel's register-summed cell)
     uint16_t* d_fbins16_ranked = nullptr; // nbins > 256: fixed bins replaced by their population rank
     int* d_wrank_inv = nullptr;          // nbins > 256: rank -> fixed bin (kMaxBinsWide entries)
+    uint8_t* d_wrow_used = nullptr;      // nbins > 256: 1 where a fixed bin holds voxels (rows the entropy pass reads)
     uint32_t* d_mask_bits = nullptr;    // NULL, or one bit per fixed voxel (mi_set_fixed_mask)
     unsigned rare_cap = 0;              // rare voxels without a mask (upper bound of n_rare)
     unsigned rare_alloc = 0;            // entries d_rare was allocated for
@@ -655,7 +656,8 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
                                                  mi::OutMap{0, 0, 0, 0, 0, 0, 0}, s));
             else
             MI_CUDA(c, mi::launch_entropy(hist, c->nb, (int)cnt, c->d_q, nq, q_off, c->tsallis_form,
-                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, mi::OutMap{0, 0, 0, 0, 0, 0, 0}, s));
+                                          c->d_mi + (size_t)off * nch, c->d_nvalid + off, mi::OutMap{0, 0, 0, 0, 0, 0, 0}, s,
+                                          c->d_wrow_used));
             c->last_launches[2] += 1;
             q_off += mi::kMaxQPerPass;
         } while (q_off < nq);
@@ -834,6 +836,8 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
                 std::stable_sort(order.begin(), order.end(), [&](int x, int y) { return h_c[x] > h_c[y]; });
                 std::vector<uint16_t> h_rank(mi::kMaxBinsWide);
                 for (int r = 0; r < mi::kMaxBinsWide; ++r) h_rank[order[r]] = (uint16_t)r;
+                std::vector<uint8_t> h_used(mi::kMaxBinsWide);
+                for (int b = 0; b < mi::kMaxBinsWide; ++b) h_used[b] = h_c[b] > 0 ? 1 : 0;
                 uint16_t* d_wrank = nullptr;
                 if ((e = dev_alloc((void**)&d_wrank, mi::kMaxBinsWide * sizeof(uint16_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc wide ranks"); break; }
                 bool failed = false;
@@ -841,6 +845,8 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
                     (e = dev_alloc((void**)&c->d_fbins16_ranked, (size_t)nf * sizeof(uint16_t), device, c->stream)) != cudaSuccess ||
                     (e = cudaMemcpyAsync(d_wrank, h_rank.data(), h_rank.size() * sizeof(uint16_t), cudaMemcpyHostToDevice, s)) != cudaSuccess ||
                     (e = cudaMemcpyAsync(c->d_wrank_inv, order.data(), order.size() * sizeof(int), cudaMemcpyHostToDevice, s)) != cudaSuccess ||
+                    (e = dev_alloc((void**)&c->d_wrow_used, mi::kMaxBinsWide, device, c->stream)) != cudaSuccess ||
+                    (e = cudaMemcpyAsync(c->d_wrow_used, h_used.data(), h_used.size(), cudaMemcpyHostToDevice, s)) != cudaSuccess ||
                     (e = mi::launch_remap16(c->d_fbins16, c->d_fbins16_ranked, nf, d_wrank, s)) != cudaSuccess ||
                     (e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "rank wide fixed bins"); failed = true; }
                 dev_free(d_wrank, c->stream);
@@ -899,7 +905,7 @@ void mi_destroy(mi_ctx* c) {
     DeviceGuard guard(c->device);
     if (guard.ok) {
         void* bufs[] = {c->d_fbins, c->d_fbins_ranked, c->d_rank, c->d_rank_inv, c->d_moving_pad, c->d_mask_bits, c->d_fbins16, c->d_mbins16, c->d_mbins,
-                        c->d_mbins_quad, c->d_moving_quad, c->d_fbins16_ranked, c->d_wrank_inv, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
+                        c->d_mbins_quad, c->d_moving_quad, c->d_fbins16_ranked, c->d_wrank_inv, c->d_wrow_used, c->d_red_count, c->d_fb_pitched, c->d_rare, c->d_X, c->d_XY, c->d_colvalid, c->d_axis, c->d_M, c->d_hist,
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);

@@ -109,7 +109,8 @@ struct OutMap {
 };
 cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const double* q_dev, int nq,
                            int q_off, int form, double* mi_out /* n x (1+nq) */, int64_t* nvalid,
-                           OutMap om, cudaStream_t s);
+                           OutMap om, cudaStream_t s,
+                           const uint8_t* row_used = nullptr /* nb > 256: flags of the populated fixed bins */);
 
 // ---- partial-volume interpolation (mi_pv.cu) ---------------------------------------------------
 struct PvArgs {

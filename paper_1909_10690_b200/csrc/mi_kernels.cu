@@ -926,10 +926,12 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
 // per-CTA partial sums, row sums (fixed marginal) stored, column sums (moving marginal) added to pb
 // with integer atomics (order-free, so the result is reproducible).  Pass 2: one CTA per transform
 // adds the marginal terms and the partial sums in a fixed order and finishes.
+constexpr int kWideLoads = 4;    // loads in flight per lane (16 measured 4x slower: the double-precision terms of a non-zero cell are then inlined 16 times)
 __global__ void __launch_bounds__(kEntropyThreads)
 entropy_wide_partial_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restrict__ q, int q_off,
                             int nq_pass, unsigned* __restrict__ pa, unsigned* __restrict__ pb,
-                            double* __restrict__ partial /* [t][split][1 + kMaxQPerPass] */) {
+                            double* __restrict__ partial /* [t][split][1 + kMaxQPerPass] */,
+                            const uint8_t* __restrict__ row_used /* NULL, or nb flags: fixed bin holds voxels */) {
     constexpr int NW = kEntropyThreads / 32;
     constexpr int NA = 1 + kMaxQPerPass;
     __shared__ unsigned sh_pb[kMaxBinsWide];
@@ -947,14 +949,16 @@ entropy_wide_partial_kernel(const uint32_t* __restrict__ hist, int nb, const dou
 #pragma unroll
     for (int i = 0; i < NA; ++i) acc[i] = 0.0;
     for (int r = r0 + warp; r < r1; r += NW) {
+        // a fixed bin without voxels has an all-zero row (pa is zero on entry): at 4096 bins most rows
+        if (row_used != nullptr && __ldg(row_used + r) == 0) continue;
         const uint32_t* __restrict__ row = h + (size_t)r * nb;
         unsigned rowsum = 0;
-        for (int c0 = lane; c0 < nb; c0 += 128) {          // four loads in flight per lane
-            unsigned v[4];
+        for (int c0 = lane; c0 < nb; c0 += 32 * kWideLoads) {   // kWideLoads loads in flight per lane
+            unsigned v[kWideLoads];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) v[u] = c0 + 32 * u < nb ? __ldg(row + c0 + 32 * u) : 0u;
+            for (int u = 0; u < kWideLoads; ++u) v[u] = c0 + 32 * u < nb ? __ldg(row + c0 + 32 * u) : 0u;
 #pragma unroll
-            for (int u = 0; u < 4; ++u)
+            for (int u = 0; u < kWideLoads; ++u)
                 if (v[u]) {
                     rowsum += v[u];
                     atomicAdd(&sh_pb[c0 + 32 * u], v[u]);
@@ -1043,7 +1047,8 @@ entropy_wide_final_kernel(int nb, const double* __restrict__ q, int nq_total, in
 }
 
 cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const double* q_dev, int nq,
-                           int q_off, int form, double* mi_out, int64_t* nvalid, OutMap om, cudaStream_t s) {
+                           int q_off, int form, double* mi_out, int64_t* nvalid, OutMap om, cudaStream_t s,
+                           const uint8_t* row_used) {
     if (n_transforms <= 0) return cudaSuccess;
     int nq_pass = nq - q_off;
     if (nq_pass > kMaxQPerPass) nq_pass = kMaxQPerPass;
@@ -1075,7 +1080,7 @@ cudaError_t launch_entropy(const uint32_t* hist, int nb, int n_transforms, const
     e = cudaMemsetAsync(pab, 0, cnt_words * sizeof(unsigned), s);
     if (e == cudaSuccess) {
         entropy_wide_partial_kernel<<<dim3(nsplit, n_transforms), kEntropyThreads, 0, s>>>(hist, nb, q_dev, q_off, nq_pass,
-                                                                                         pa, pb, partial);
+                                                                                         pa, pb, partial, row_used);
         entropy_wide_final_kernel<<<n_transforms, kEntropyThreads, 0, s>>>(nb, q_dev, nq, q_off, nq_pass, form, pa, pb,
                                                                           partial, nsplit, mi_out, nvalid, om);
         e = cudaGetLastError();
