@@ -573,7 +573,7 @@ __global__ void __launch_bounds__(kHistThreads, 1) zhist_kernel(const __grid_con
                         v = sh_hist[r * pitch + b];
                         if (v) sh_hist[r * pitch + b] = 0u;
                     }
-                    grow[b] = v;
+                    __stcs(grow + b, v);   // streaming: 256 KB per item must not push the xy planes out of L2
                 }
             }
         }
