@@ -854,21 +854,35 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
 #pragma unroll
     for (int i = 0; i < NACC; ++i) acc[i] = 0.0;
 
-    // joint terms + marginal counts
+    // joint terms + marginal counts.  The table is mostly zeros and streams from DRAM: all MAXB/32 loads of a lane's
+    // share of a row are issued first, then the non-zero ones are visited one by one so that the double-precision
+    // terms are compiled once (inlined per load they spill; one load at a time the kernel waits on memory).
+    constexpr int NV = MAXB / 32;
     for (int r = warp; r < nb; r += NW) {
         unsigned rowsum = 0;
-        for (int c = lane; c < nb; c += 32) {
-            const unsigned v = h[r * nb + c];
-            if (v) {
-                rowsum += v;
-                atomicAdd(&sh_pb[c], v);
-                const double dv = (double)v;
-                const double lc = log(dv);
-                acc[2] += dv * lc;
+        unsigned v[NV];
+        unsigned nz = 0u;
 #pragma unroll
-                for (int k = 0; k < kMaxQPerPass; ++k)
-                    if (k < nq_pass) acc[3 + 3 * k + 2] += exp(qv[k] * lc);
-            }
+        for (int u = 0; u < NV; ++u) {
+            const int c = lane + 32 * u;
+            v[u] = c < nb ? __ldg(h + (size_t)r * nb + c) : 0u;
+        }
+#pragma unroll
+        for (int u = 0; u < NV; ++u) nz |= (v[u] != 0u ? 1u : 0u) << u;
+        while (nz) {
+            const int u = __ffs(nz) - 1;
+            nz &= nz - 1u;
+            unsigned val = v[0];
+#pragma unroll
+            for (int k = 1; k < NV; ++k) val = u == k ? v[k] : val;
+            rowsum += val;
+            atomicAdd(&sh_pb[lane + 32 * u], val);
+            const double dv = (double)val;
+            const double lc = log(dv);
+            acc[2] += dv * lc;
+#pragma unroll
+            for (int k = 0; k < kMaxQPerPass; ++k)
+                if (k < nq_pass) acc[3 + 3 * k + 2] += exp(qv[k] * lc);
         }
         rowsum = warp_sum(rowsum);
         if (lane == 0) sh_pa[r] = rowsum;
