@@ -96,6 +96,12 @@ class ClockSampler:
     def stop(self):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        late = False
+        if not self.rows:       # a timed region shorter than nvidia-smi's start-up (C1): wait for its first line
+            late = True
+            deadline = time.perf_counter() + 2.0
+            while not self.rows and time.perf_counter() < deadline:
+                time.sleep(0.02)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
@@ -112,9 +118,12 @@ class ClockSampler:
                 if len(r) > 3 + k and r[3 + k].lower().startswith("active"):
                     reasons.add(nm)
         busy = [c for c, p in zip(sm, power) if p > 250.0] or sm
-        return {"sm_mhz": float(np.median(busy)) if busy else None,
-                "sm_max_mhz": max(smax) if smax else None, "reasons": sorted(reasons),
-                "samples": len(sm), "power_w_max": max(power) if power else None}
+        out = {"sm_mhz": float(np.median(busy)) if busy else None,
+               "sm_max_mhz": max(smax) if smax else None, "reasons": sorted(reasons),
+               "samples": len(sm), "power_w_max": max(power) if power else None}
+        if late:
+            out["note"] = "timed region shorter than one sampling period: sampled right after it"
+        return out
 
 
 def sample_nodes(cfg, count):
