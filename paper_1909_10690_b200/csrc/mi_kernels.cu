@@ -940,7 +940,7 @@ entropy_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restri
 // per-CTA partial sums, row sums (fixed marginal) stored, column sums (moving marginal) added to pb
 // with integer atomics (order-free, so the result is reproducible).  Pass 2: one CTA per transform
 // adds the marginal terms and the partial sums in a fixed order and finishes.
-constexpr int kWideLoads = 4;    // loads in flight per lane (16 measured 4x slower: the double-precision terms of a non-zero cell are then inlined 16 times)
+constexpr int kWideLoads = 16;   // loads in flight per lane
 __global__ void __launch_bounds__(kEntropyThreads)
 entropy_wide_partial_kernel(const uint32_t* __restrict__ hist, int nb, const double* __restrict__ q, int q_off,
                             int nq_pass, unsigned* __restrict__ pa, unsigned* __restrict__ pb,
@@ -971,17 +971,23 @@ entropy_wide_partial_kernel(const uint32_t* __restrict__ hist, int nb, const dou
             unsigned v[kWideLoads];
 #pragma unroll
             for (int u = 0; u < kWideLoads; ++u) v[u] = c0 + 32 * u < nb ? __ldg(row + c0 + 32 * u) : 0u;
+            unsigned nz = 0u;
 #pragma unroll
-            for (int u = 0; u < kWideLoads; ++u)
-                if (v[u]) {
-                    rowsum += v[u];
-                    atomicAdd(&sh_pb[c0 + 32 * u], v[u]);
-                    const double dv = (double)v[u], lc = log(dv);
-                    acc[0] += dv * lc;
+            for (int u = 0; u < kWideLoads; ++u) nz |= (v[u] != 0u ? 1u : 0u) << u;
+            while (nz) {                                      // the non-zero ones, one by one: the terms are compiled once
+                const int u = __ffs(nz) - 1;
+                nz &= nz - 1u;
+                unsigned val = v[0];
 #pragma unroll
-                    for (int k = 0; k < kMaxQPerPass; ++k)
-                        if (k < nq_pass) acc[1 + k] += exp(qv[k] * lc);
-                }
+                for (int k = 1; k < kWideLoads; ++k) val = u == k ? v[k] : val;
+                rowsum += val;
+                atomicAdd(&sh_pb[c0 + 32 * u], val);
+                const double dv = (double)val, lc = log(dv);
+                acc[0] += dv * lc;
+#pragma unroll
+                for (int k = 0; k < kMaxQPerPass; ++k)
+                    if (k < nq_pass) acc[1 + k] += exp(qv[k] * lc);
+            }
         }
         rowsum = warp_sum(rowsum);
         if (lane == 0) pa[(size_t)t * nb + r] = rowsum;
