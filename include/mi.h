@@ -129,6 +129,45 @@ mi_status mi_eval_batch(mi_ctx *ctx, const double *T, int64_t N, const double *q
 mi_status mi_eval_batch_pv(mi_ctx *ctx, const double *T, int64_t N, const double *q, int32_t nq,
                            double *mi_out, uint64_t *hist_out, int64_t *nvalid_out);
 
+/* mi_eval_noalloc -- steps a3-a5 (resample, joint histogram, entropies: eq. 1-2
+ * PAPER.md:25-32) for ONE transform, without a context and without allocating any device memory.
+ *
+ * Why it exists.  mi_create and the calls on a context take device memory from the library's pool.  A
+ * caller whose process has given the whole GPU to another allocator (a tensor framework's caching
+ * allocator, a renderer, a fixed MPS/MIG memory limit), or who sits in a latency-critical loop where the
+ * device-wide synchronisation of cudaMalloc / cudaFree is not acceptable, cannot use them.  This call makes
+ * no cudaMalloc, cudaFree or other allocating call: its only scratch, the nbins x nbins joint histogram
+ * (plus the q list), lives in a static __device__ array inside the library.
+ *
+ * Cost and limits.  The array is 256 KB + 256 B; every GPU on which the library is loaded holds it until
+ * the process exits.  nbins <= 256, nq <= 8, NEAREST or TRILINEAR, one transform per call; larger requests
+ * return MI_ERR_UNSUPPORTED with a message in mi_last_error(NULL) -- nothing is truncated.
+ *
+ * Arguments.  fixed_dev, moving_dev: float32 volumes in DEVICE memory the caller owns (layout, dims,
+ * spacing, ranges, nbins as in mi_create; read in place, not copied, so they must stay valid until the
+ * work queued on cuda_stream has run).  T: one row-major 3x4 [A|t] (host); q, nq, interp as in
+ * mi_eval_batch (host); form as in mi_set_tsallis_form.  Outputs are DEVICE pointers the caller owns:
+ * mi_out_dev 1+nq doubles; hist_out_dev NULL or nbins x nbins uint32; nvalid_out_dev NULL or one int64.
+ * A host pointer for a volume or an output is MI_ERR_INVALID_ARG (staging it would need a device buffer).
+ * device, cuda_stream as in mi_create.  The call only queues work on cuda_stream and returns; the outputs
+ * are complete when that stream has run, and a kernel fault shows up at the caller's next synchronisation.
+ * Results are bit-identical to mi_eval_batch's for the same volumes and transform.
+ *
+ * One array, shared by every call:
+ *   - it still holds the previous call's histogram; each call clears the cells it uses, on cuda_stream,
+ *     before counting -- callers need not (and cannot) clear it themselves;
+ *   - two calls whose GPU work overlaps in time on one device (different streams, threads or contexts)
+ *     count into the same cells and spoil each other: serialise them on one stream or with events;
+ *   - the FIRST call on each device looks up the array's device address (cudaGetSymbolAddress with that
+ *     device current) and opts the kernel into large shared memory.  Make that first call during set-up,
+ *     before any stream capture begins; later calls only launch kernels. */
+mi_status mi_eval_noalloc(const float *fixed_dev, const int32_t fixed_dims[3], const double fixed_spacing[3],
+                          const float *moving_dev, const int32_t moving_dims[3], const double moving_spacing[3],
+                          int32_t nbins, float fixed_lo, float fixed_hi, float moving_lo, float moving_hi,
+                          const double T[12], const double *q, int32_t nq, mi_interp interp, mi_tsallis_form form,
+                          double *mi_out_dev, uint32_t *hist_out_dev, int64_t *nvalid_out_dev,
+                          int32_t device, void *cuda_stream);
+
 /* mi_map -- the exhaustive map of one family: "map with the MI function all
  * the space in a finite range and build a 3D image".
  *   lo, hi, n   inclusive grid per parameter axis: value k on axis d is

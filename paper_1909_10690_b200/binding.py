@@ -33,7 +33,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 (MI_INFO_NUM_SMS, MI_INFO_BIN_MODE, MI_INFO_ZHIST_ROWS, MI_INFO_RARE_VOXELS, MI_INFO_GENERIC_ROWS,
  MI_INFO_LAST_PATH, MI_INFO_LAST_UPDATES_ISSUED) = range(100, 107)
 
-EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_map", "mi_map_range", "mi_set_option",
+EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_eval_noalloc", "mi_map", "mi_map_range", "mi_set_option",
            "mi_get_option", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
            "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_seed_from_map", "mi_multimetric_gradient", "mi_register",
@@ -56,6 +56,9 @@ _lib.mi_eval_batch.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, C.c_int, _vp
 _lib.mi_eval_batch.restype = C.c_int
 _lib.mi_eval_batch_pv.argtypes = [_vp, _vp, C.c_int64, _vp, C.c_int32, _vp, _vp, _vp]
 _lib.mi_eval_batch_pv.restype = C.c_int
+_lib.mi_eval_noalloc.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_float, C.c_float, C.c_float, C.c_float,
+                                 _vp, _vp, C.c_int32, C.c_int, C.c_int, _vp, _vp, _vp, C.c_int32, _vp]
+_lib.mi_eval_noalloc.restype = C.c_int
 _lib.mi_map.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp]
 _lib.mi_map.restype = C.c_int
 _lib.mi_map_range.argtypes = [_vp, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_int, _vp, _vp, _vp]
@@ -256,6 +259,37 @@ def mi_eval_batch_pv(ctx, T, q=(), mi_out=None, hist_out=None, nvalid_out=None):
     st = _lib.mi_eval_batch_pv(ctx.handle, _ptr(T), N, _ptr(q) if nq else None, nq, _ptr(mi_out), _ptr(hist_out),
                                _ptr(nvalid_out))
     _check(ctx, st)
+    return mi_out, hist_out, nvalid_out
+
+
+def mi_eval_noalloc(fixed, moving, fixed_spacing, moving_spacing, nbins, T, q=(), interp=MI_INTERP_TRILINEAR,
+                    form=0, mi_out=None, hist_out=None, nvalid_out=None, fixed_lo=0.0, fixed_hi=1.0, moving_lo=0.0,
+                    moving_hi=1.0, device=0, cuda_stream=None):
+    """One transform's MI (and optionally its joint histogram) for callers that must not let the library
+    allocate device memory -- the GPU is owned by another allocator, or cudaMalloc's device-wide sync is
+    not acceptable in their loop.  The histogram scratch is a 256 KB static array inside the library, so
+    nbins <= 256 and nq <= 8, and calls overlapping on one GPU would race (see include/mi.h).
+
+    fixed, moving: float32 CUDA tensors (z, y, x).  mi_out (1+nq float64), hist_out (nbins x nbins, uint32
+    stored in an int32 tensor) and nvalid_out (1 int64) are CUDA tensors the caller allocated; mi_out is
+    required, the others may be None.  Work is only queued on the stream: synchronise before reading."""
+    assert _is_torch(fixed) and _is_torch(moving) and fixed.is_cuda and moving.is_cuda, "device tensors only"
+    fixed, moving = _volume(fixed), _volume(moving)
+    assert mi_out is not None, "mi_out must be a caller-allocated CUDA tensor"
+    T = _f64(T, 12)
+    q = _f64(q)
+    fd = _i32(tuple(fixed.shape)[::-1], 3)
+    md = _i32(tuple(moving.shape)[::-1], 3)
+    fs, ms = _f64(fixed_spacing, 3), _f64(moving_spacing, 3)
+    if cuda_stream is None:
+        import torch
+        cuda_stream = torch.cuda.current_stream(device).cuda_stream
+    st = _lib.mi_eval_noalloc(_ptr(fixed), _ptr(fd), _ptr(fs), _ptr(moving), _ptr(md), _ptr(ms), int(nbins),
+                              float(fixed_lo), float(fixed_hi), float(moving_lo), float(moving_hi), _ptr(T),
+                              _ptr(q) if q.size else None, q.size, int(interp), int(form), _ptr(mi_out),
+                              _ptr(hist_out), _ptr(nvalid_out), int(device), cuda_stream)
+    if st != MI_OK:
+        raise MIError(st, mi_last_error(None))
     return mi_out, hist_out, nvalid_out
 
 
