@@ -367,7 +367,10 @@ mi_status mi_last_timing(const mi_ctx *ctx, float ms[5], int64_t launches[5]);
  * denominator; 2 all lanes on one address; 3 one linear congruential generator per thread seeded linearly in
  * the thread index (round 1's pattern: random in time, but the lanes of a warp form an arithmetic
  * progression, which spreads them over the banks more evenly than chance); 4 and 5 are patterns 2 and 1 with a
- * per-lane VALUE added instead of 1 (the weighted update of partial-volume interpolation).  Host pointers. */
+ * per-lane VALUE added instead of 1 (the weighted update of partial-volume interpolation); 6 is pattern 1's
+ * statistics with the bins hashed once per thread BEFORE the timed loop (eight per thread, reused), so that no
+ * integer arithmetic competes with the updates -- the probe that shows what the crossbar itself sustains
+ * (pattern 1's hash costs about 5 % of it).  iters is rounded up to a multiple of 8.  Host pointers. */
 mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
                                       double *updates_per_s);
 

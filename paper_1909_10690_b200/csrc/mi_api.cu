@@ -1383,7 +1383,7 @@ mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms,
 
 mi_status mi_probe_shared_atomic_rate(int32_t device, int32_t nbins, int32_t pattern, int32_t iters,
                                       double* updates_per_s) {
-    if (!updates_per_s || nbins < 8 || nbins > 256 || pattern < 0 || pattern > 5 || iters < 1)
+    if (!updates_per_s || nbins < 8 || nbins > 256 || pattern < 0 || pattern > 6 || iters < 1)
         return MI_ERR_INVALID_ARG;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
