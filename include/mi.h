@@ -276,9 +276,20 @@ mi_status mi_seed_from_map(mi_family family, const double lo[3], const double hi
                            int64_t index, double p_out[9]);
 
 /* delta[k] <= 0 skips component k (grad_out[k] = 0).  grad_out: 9 doubles; value_out: NULL or 2
- * doubles (Shannon, Tsallis_q at p).  Host pointers; q > 0 and finite. */
+ * doubles (Shannon, Tsallis_q at p).  Host pointers; q > 0 and finite.
+ * With MI_INTERP_PARTIAL_VOLUME the weights are quantised to 1/32 voxel per axis (A21), so MI is
+ * piecewise constant in the transform and a finite difference needs a step the quantisation resolves:
+ * every delta[k] > 0 must be at least mi_pv_min_delta's value for k, else MI_ERR_INVALID_ARG (the same
+ * holds for mi_register).  NEAREST and TRILINEAR have no such bound. */
 mi_status mi_multimetric_gradient(mi_ctx *ctx, const double p[9], const double delta[9], double q,
                                   mi_interp interp, double grad_out[9], double value_out[2]);
+
+/* Smallest central-difference steps partial-volume interpolation resolves on this context's geometry, in the
+ * units of p: [0..2] translation, moving spacing / 32 mm (one quantisation step of that moving axis);
+ * [3..5] rotation in degrees and [6..8] scale factor, the change that moves a point at the reference radius
+ * r = max(smallest fixed extent / 4, smallest fixed spacing) by one step of the coarsest moving axis, so that
+ * every voxel farther than r from the centre moves at least one step.  Host pointer, 9 doubles. */
+mi_status mi_pv_min_delta(const mi_ctx *ctx, double delta_min_out[9]);
 
 /* The loop of the paper's Fig. 1 (Transform -> Metric -> Optimizer) around the
  * multi-metric gradient.  The paper names "gradient descent" and the strategy but prints no step rule;

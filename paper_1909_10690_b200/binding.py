@@ -36,7 +36,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_eval_noalloc", "mi_map", "mi_map_range", "mi_set_option",
            "mi_get_option", "mi_destroy", "mi_last_error",
            "mi_family_matrix", "mi_index_affine", "mi_get_bins", "mi_last_timing", "mi_release_cached_memory",
-           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_seed_from_map", "mi_multimetric_gradient", "mi_register",
+           "mi_map_gradient", "mi_map_basins", "mi_compose_matrix", "mi_seed_from_map", "mi_multimetric_gradient", "mi_register", "mi_pv_min_delta",
            "mi_probe_shared_atomic_rate", "mi_probe_gather_rate", "mi_version")
 
 if not os.path.exists(LIB_PATH):
@@ -85,6 +85,8 @@ _lib.mi_compose_matrix.argtypes = [_vp, _vp]
 _lib.mi_compose_matrix.restype = C.c_int
 _lib.mi_multimetric_gradient.argtypes = [_vp, _vp, _vp, C.c_double, C.c_int, _vp, _vp]
 _lib.mi_multimetric_gradient.restype = C.c_int
+_lib.mi_pv_min_delta.argtypes = [_vp, _vp]
+_lib.mi_pv_min_delta.restype = C.c_int
 _lib.mi_register.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, C.c_double, C.c_int, _vp, _vp, _vp]
 _lib.mi_register.restype = C.c_int
 _lib.mi_map_gradient.argtypes = [_vp, _vp, _vp, _vp, _vp, C.c_int32, _vp]
@@ -471,6 +473,13 @@ def mi_multimetric_gradient(ctx, p, delta, q, interp=MI_INTERP_TRILINEAR):
 
 class _RegisterInfo(C.Structure):
     _fields_ = [("iterations", C.c_int32), ("steps", C.c_double * 3), ("values", C.c_double * 2)]
+
+
+def mi_pv_min_delta(ctx) -> np.ndarray:
+    """Smallest finite-difference steps (9 doubles, units of p) MI_INTERP_PARTIAL_VOLUME resolves on this context."""
+    out = np.empty(9, dtype=np.float64)
+    _check(ctx, _lib.mi_pv_min_delta(ctx.handle, _ptr(out)))
+    return out
 
 
 def mi_register(ctx, p0, delta, step0, step_min, max_iter, q, interp=MI_INTERP_TRILINEAR):

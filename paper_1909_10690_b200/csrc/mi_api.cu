@@ -380,7 +380,8 @@ mi_status run_separable(mi_ctx* c, const SeparablePlan& sp, int32_t nq, int inte
     // Batch = ga values of p0 x gb values of p1.  Whole p0 slabs (gb = n1) when the scratch budgets
     // allow, as many as minimise idle SM-waves; otherwise one p0 at a time in chunks of p1.
     size_t max_pairs = c->xy_budget / xy_bytes_per_pair;
-    if (c->sep_hist_budget / hist_bytes_per_pair < max_pairs) max_pairs = c->sep_hist_budget / hist_bytes_per_pair;
+    if (!fused && c->sep_hist_budget / hist_bytes_per_pair < max_pairs)   // fused: no histogram leaves the SM
+        max_pairs = c->sep_hist_budget / hist_bytes_per_pair;
     if (max_pairs > 65535) max_pairs = 65535;  // gridDim.y of the y-pass
     if (max_pairs < 1) return kSepFallback;
     int ga = 1, gb = n1;
@@ -552,6 +553,7 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     int64_t chunk = (int64_t)(c->hist_budget / (nbins2 * helem));
     if (chunk < 1) chunk = 1;
     if (chunk > N) chunk = N;
+    if (c->wide && chunk > 65535) chunk = 65535;   // the wide entropy pass puts the transform on gridDim.y
     c->last_reds = -1;   // -1: not counted (only the z kernel of the separable path counts its updates)
     if (sep != nullptr) {
         MI_CUDA(c, cudaMemsetAsync(c->d_red_count, 0, sizeof(unsigned long long), s));
@@ -964,6 +966,9 @@ mi_status mi_set_tsallis_form(mi_ctx* c, mi_tsallis_form form) {
 mi_status mi_set_option(mi_ctx* c, mi_option key, int64_t v) {
     if (!c) return MI_ERR_INVALID_ARG;
     bool relayout = false;
+    // the options plan_layout reads: restored if the new value gives a layout the device cannot hold
+    const int old_bin_mode_max = c->opt_bin_mode_max, old_zrows_max = c->opt_zrows_max, old_zpad = c->opt_zpad,
+              old_gpad = c->opt_gpad, old_gsmem_kb = c->opt_gsmem_kb;
     auto bad = [&]() { return fail(c, MI_ERR_INVALID_ARG, "mi_set_option: value out of range"); };
     switch (key) {
     case MI_OPT_SEPARABLE: c->use_separable = v != 0; break;
@@ -1014,7 +1019,16 @@ mi_status mi_set_option(mi_ctx* c, mi_option key, int64_t v) {
     if (!relayout) return MI_OK;
     DeviceGuard guard(c->device);
     if (!guard.ok) return fail(c, MI_ERR_CUDA, "cudaSetDevice failed");
-    return plan_layout(c);
+    const mi_status st = plan_layout(c);
+    if (st != MI_OK) {
+        // the context keeps working with the layout it had: put the old values back and plan again
+        const std::string why = c->err;
+        c->opt_bin_mode_max = old_bin_mode_max; c->opt_zrows_max = old_zrows_max; c->opt_zpad = old_zpad;
+        c->opt_gpad = old_gpad; c->opt_gsmem_kb = old_gsmem_kb;
+        if (plan_layout(c) != MI_OK) return st;
+        return fail(c, st, "mi_set_option: value rejected, option unchanged (" + why + ")");
+    }
+    return MI_OK;
 }
 
 mi_status mi_get_option(const mi_ctx* c, mi_option key, int64_t* out) {
@@ -1152,6 +1166,30 @@ mi_status gradient_core(mi_ctx* c, const double p[9], const double delta[9], dou
     return MI_OK;
 }
 
+// Smallest finite-difference steps under partial-volume interpolation.  PV rounds each axis' fraction to 1/32
+// voxel (reading A21), so MI is piecewise constant in the transform: a step must move the sample points by at
+// least one quantisation step or both arms of the central difference see the same histogram.
+//   translation k     one step of moving axis k: s_m[k] / 32 mm
+//   rotation, scale   a point at distance r from the centre moves r * angle (r * factor change); the reference
+//                     radius is a quarter of the smallest fixed extent (not below one fixed voxel), so that every
+//                     voxel farther out than that moves at least one step of the coarsest moving axis
+void pv_min_delta(const mi_ctx* c, double out[9]) {
+    double step_mm = 0.0, extent = 0.0, smin = c->fs[0];
+    for (int k = 0; k < 3; ++k) {
+        out[k] = c->ms[k] / 32.0;
+        if (out[k] > step_mm) step_mm = out[k];
+        const double e = c->fs[k] * (double)(c->fd[k] - 1);
+        if (k == 0 || e < extent) extent = e;
+        if (c->fs[k] < smin) smin = c->fs[k];
+    }
+    double r_ref = 0.25 * extent;
+    if (r_ref < smin) r_ref = smin;
+    for (int k = 0; k < 3; ++k) {
+        out[3 + k] = step_mm / r_ref * (180.0 / 3.14159265358979323846);
+        out[6 + k] = step_mm / r_ref;
+    }
+}
+
 mi_status validate_gradient_args(mi_ctx* c, const double* p, const double* delta, double q, int interp) {
     if (!p || !delta) return fail(c, MI_ERR_INVALID_ARG, "NULL argument");
     mi_status st = validate_interp(c, interp);
@@ -1160,12 +1198,28 @@ mi_status validate_gradient_args(mi_ctx* c, const double* p, const double* delta
     if (st != MI_OK) return st;
     for (int i = 0; i < 9; ++i)
         if (!std::isfinite(p[i]) || !std::isfinite(delta[i])) return fail(c, MI_ERR_INVALID_ARG, "non-finite parameter");
+    if (interp == MI_INTERP_PARTIAL_VOLUME) {
+        double dmin[9];
+        pv_min_delta(c, dmin);
+        for (int i = 0; i < 9; ++i)
+            if (delta[i] > 0.0 && delta[i] < dmin[i])
+                return fail(c, MI_ERR_INVALID_ARG,
+                            "delta[" + std::to_string(i) + "] = " + std::to_string(delta[i]) + " is below " +
+                                std::to_string(dmin[i]) + ", the smallest step partial-volume interpolation resolves "
+                                "(weights are quantised to 1/32 voxel; see mi_pv_min_delta)");
+    }
     return MI_OK;
 }
 
 }  // namespace
 
 extern "C" {
+
+mi_status mi_pv_min_delta(const mi_ctx* c, double delta_min_out[9]) {
+    if (!c || !delta_min_out) return MI_ERR_INVALID_ARG;
+    pv_min_delta(c, delta_min_out);
+    return MI_OK;
+}
 
 mi_status mi_multimetric_gradient(mi_ctx* c, const double p[9], const double delta[9], double q, mi_interp interp,
                                   double grad_out[9], double value_out[2]) {
@@ -1362,9 +1416,12 @@ mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms,
     a.nslabs = generic_nslabs(c, n_transforms, MI_INTERP_TRILINEAR);   // the launch shape mi_eval_batch / mi_map use
     cudaEvent_t e0 = nullptr, e1 = nullptr;
     MI_CUDA(c, cudaEventCreate(&e0));
-    MI_CUDA(c, cudaEventCreate(&e1));
+    cudaError_t e = cudaEventCreate(&e1);
+    if (e != cudaSuccess) {
+        cudaEventDestroy(e0);
+        return cuda_fail(c, e, "cudaEventCreate");
+    }
     float best = 1e30f;
-    cudaError_t e = cudaSuccess;
     for (int rep = 0; rep <= reps && e == cudaSuccess; ++rep) {   // the first run warms up
         cudaEventRecord(e0, s);
         e = mi::launch_resample_hist(a, MI_INTERP_TRILINEAR, c->num_sms, s);

@@ -214,3 +214,35 @@ def test_coarse_map_seeds_the_registration(mi):
     peak = np.array([flo[0] + k0, flo[1] + k1, flo[2] + k2])
     assert np.max(np.abs(got["p"][3:6] - peak)) <= 1.0 + 1e-9, (got["p"][3:6], peak)
     assert got["values"][0] >= coarse[0].max() - 1e-9
+
+
+def test_partial_volume_gradient_needs_a_step_its_quantisation_resolves(mi):
+    """Partial-volume weights are quantised to 1/32 voxel (reading A21), so PV MI is piecewise constant in the
+    transform.  mi_pv_min_delta names the smallest finite-difference steps that quantisation resolves;
+    mi_multimetric_gradient / mi_register refuse anything smaller instead of returning a silent zero, and at the
+    smallest accepted step the two arms really see different histograms and every gradient component is non-zero.
+    Trilinear has no bound."""
+    cfg = ph.get_config("C1")
+    p = np.array([0.7, -0.4, 0.3, 2.0, -1.0, 1.5, 1.02, 0.99, 1.01])
+    with mi.mi_create(cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        dmin = mi.mi_pv_min_delta(ctx)
+        ms = np.asarray(cfg.moving_spacing, dtype=np.float64)
+        assert np.array_equal(dmin[:3], ms / 32.0) and np.all(dmin[3:] > 0)
+        g, _ = mi.mi_multimetric_gradient(ctx, p, dmin, 0.5, mi.MI_INTERP_PARTIAL_VOLUME)
+        assert np.all(g != 0.0), g
+        for k in range(9):
+            e = np.zeros(9)
+            e[k] = dmin[k]
+            T = np.stack([mi.mi_compose_matrix(p), mi.mi_compose_matrix(p + e)])
+            _, h, _ = mi.mi_eval_batch_pv(ctx, T, (), hist_out=True)
+            assert not np.array_equal(h[0], h[1]), "PV histogram unchanged by the smallest accepted step of parameter %d" % k
+            small = np.zeros(9)
+            small[k] = 0.99 * dmin[k]
+            with pytest.raises(mi.MIError) as err:
+                mi.mi_multimetric_gradient(ctx, p, small, 0.5, mi.MI_INTERP_PARTIAL_VOLUME)
+            assert err.value.status == mi.MI_ERR_INVALID_ARG and "mi_pv_min_delta" in str(err.value)
+            mi.mi_multimetric_gradient(ctx, p, small, 0.5, mi.MI_INTERP_TRILINEAR)      # no bound without quantisation
+        with pytest.raises(mi.MIError):
+            mi.mi_register(ctx, p, 0.5 * dmin, (0.5, 0.5, 0.01), (0.1, 0.1, 0.002), 3, 0.5, mi.MI_INTERP_PARTIAL_VOLUME)
+        r = mi.mi_register(ctx, p, dmin, (0.5, 0.5, 0.01), (0.1, 0.1, 0.002), 3, 0.5, mi.MI_INTERP_PARTIAL_VOLUME)
+        assert r["iterations"] >= 1

@@ -423,6 +423,28 @@ def test_separable_scratch_smaller_than_one_slab(mi):
             mi.mi_set_option(ctx, mi.MI_OPT_ZHIST_PAD, 0)
         with pytest.raises(mi.MIError):
             mi.mi_set_option(ctx, mi.MI_INFO_NUM_SMS, 1)              # read-only
+        # the fused path writes no histogram, so a zero histogram budget must not push it to the generic kernel
+        set_options(mi, ctx, XY_BUDGET_MB=12288, FUSE_ENTROPY=1, SEP_HIST_BUDGET_MB=0)
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1
+        assert np.max(np.abs(m - ref)) <= 1e-9 and np.array_equal(am, aref)
+
+
+def test_rejected_option_leaves_the_context_as_it_was(mi):
+    """an option value whose layout the device cannot hold (8 KB of shared memory for rows of 4096
+    + 5 words) is refused AND not kept: the option reads back unchanged and the next call gives the same result."""
+    cfg = ph.get_config("C1")
+    T = rand_physical(np.random.default_rng(5), 3)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, 4096) as ctx:
+        before = mi.mi_eval_batch(ctx, T, (0.5,), 1, hist_out=True, nvalid_out=True)
+        kb = mi.mi_get_option(ctx, mi.MI_OPT_GENERIC_SMEM_KB)
+        with pytest.raises(mi.MIError) as e:
+            mi.mi_set_option(ctx, mi.MI_OPT_GENERIC_SMEM_KB, 8)
+        assert "option unchanged" in str(e.value)
+        assert mi.mi_get_option(ctx, mi.MI_OPT_GENERIC_SMEM_KB) == kb
+        after = mi.mi_eval_batch(ctx, T, (0.5,), 1, hist_out=True, nvalid_out=True)
+        for a, b in zip(before, after):
+            assert np.array_equal(a, b)
         assert mi.mi_get_option(ctx, mi.MI_INFO_NUM_SMS) >= 1
 
 
