@@ -97,7 +97,13 @@ typedef enum {
  *                  (nbins*nbins*4 bytes per transform) and every transform takes the generic kernel.
  *   *_lo, *_hi     intensity range of each volume, lo < hi, finite.
  *   device         CUDA device ordinal.   cuda_stream  a cudaStream_t (may be NULL = default).
- * Blocks until the context is ready. */
+ * Blocks until the context is ready.
+ * Device memory of a context (nbins <= 256), from the library's pool, each buffer rounded up to 2 MB: per FIXED
+ * voxel 3 B (bins, ranked bins, pitched ranked bins); per MOVING voxel 1 B (bins) + 4 B per padded voxel (the
+ * replicate-padded float copy, dims + 2).  Built only by the first call that needs them (MI_INFO_QUADS_BUILT):
+ * + 16 B per padded moving voxel for the generic trilinear kernels (any transform that is not a pure
+ * translation / scale grid), + 4 B per padded voxel for partial volume.  Map calls add their scratch on
+ * demand, bounded by the MI_OPT_*_BUDGET_MB options. */
 mi_status mi_create(mi_ctx **out,
                     const float *fixed, const int32_t fixed_dims[3], const double fixed_spacing[3],
                     const float *moving, const int32_t moving_dims[3], const double moving_spacing[3],
@@ -228,6 +234,10 @@ typedef enum {
     MI_INFO_LAST_UPDATES_ISSUED = 106, /* shared-memory histogram updates the z kernel issued in the last call
                                       (-1 if the call did not take the separable path): evaluations minus the z
                                       slices that fall outside the moving volume                               */
+    MI_INFO_QUADS_BUILT = 107,     /* bit 0: the float yz-quad copy of the moving volume exists (16 B per padded moving
+                                      voxel; built by the first generic trilinear call with GENERIC_GATHER = 1, freed by
+                                      GENERIC_GATHER = 0); bit 1: the bin-quad copy exists (4 B per padded voxel; first
+                                      partial-volume call)                                                       */
     MI_INFO_LAST_PATH = 105        /* path of the last call: 0 generic, 1 separable, 2 wide-histogram, 3 partial-volume kernels */
 } mi_option;
 mi_status mi_set_option(mi_ctx *ctx, mi_option key, int64_t value);

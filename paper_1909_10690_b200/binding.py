@@ -31,7 +31,7 @@ _STATUS = {0: "MI_OK", 1: "MI_ERR_INVALID_ARG", 2: "MI_ERR_UNSUPPORTED", 3: "MI_
  MI_OPT_GENERIC_UNROLL, MI_OPT_ZHIST_MATCH_ANY, MI_OPT_GENERIC_GATHER, MI_OPT_GENERIC_THREADS,
  MI_OPT_GENERIC_SLAB_MB) = range(16)
 (MI_INFO_NUM_SMS, MI_INFO_BIN_MODE, MI_INFO_ZHIST_ROWS, MI_INFO_RARE_VOXELS, MI_INFO_GENERIC_ROWS,
- MI_INFO_LAST_PATH, MI_INFO_LAST_UPDATES_ISSUED) = range(100, 107)
+ MI_INFO_LAST_PATH, MI_INFO_LAST_UPDATES_ISSUED, MI_INFO_QUADS_BUILT) = range(100, 108)
 
 EXPORTS = ("mi_create", "mi_set_tsallis_form", "mi_set_fixed_mask", "mi_eval_batch", "mi_eval_batch_pv", "mi_eval_noalloc", "mi_map", "mi_map_range", "mi_set_option",
            "mi_get_option", "mi_destroy", "mi_last_error",

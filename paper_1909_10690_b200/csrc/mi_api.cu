@@ -11,6 +11,7 @@
 #include <mutex>
 #include <new>
 #include <string>
+#include <unordered_map>
 #include <vector>
 
 #include "mi_internal.h"
@@ -130,16 +131,102 @@ cudaError_t device_pool(int dev, cudaMemPool_t* out) {
 // column flags) and its time depends on where they sit relative to each other -- one extra 8-byte allocation
 // early in mi_create, which shifted everything behind it by 512 bytes, cost 21 % of the headline step (773 ms
 // against 636 ms, the CTAs on three SMs running 8-22 % longer, round 2).
+//
+// In front of the pool sits an exact-size cache: a freed block is parked under (device, stream, bytes) and handed
+// back to the next request with the same key; only a miss goes to the pool.  Why: the pool keeps freed memory, but
+// it satisfies a request of a new size by splitting a bigger free block, and it rebuilds a big block later by
+// re-mapping physical memory into a fresh virtual range -- measured at about 250 ms for the 12 GB of a C5 map's
+// scratch, every create / map / destroy cycle, as soon as mi_create's allocation sequence no longer matched the
+// previous cycle's frees by luck (round 3).  A create / map / destroy loop asks for the same
+// sizes every time, so exact-size reuse never splits anything.  Reuse on the SAME stream needs no event: the
+// block's earlier uses precede its new ones in stream order.  A pool allocation that fails with out-of-memory
+// returns the parked blocks of that device to the pool and is retried; mi_release_cached_memory does the same.
+struct ParkedBlock { void* p; size_t bytes; cudaStream_t s; };
+struct LiveBlock { size_t bytes; int dev; };
+std::mutex g_cache_mutex;
+std::vector<ParkedBlock> g_parked[64];
+std::unordered_map<void*, LiveBlock> g_live;
+
+void unpark_all_locked(int dev) {   // g_cache_mutex held
+    for (const ParkedBlock& b : g_parked[dev]) {
+        if (cudaFreeAsync(b.p, b.s) != cudaSuccess) {   // the caller's stream may be gone by now
+            cudaGetLastError();
+            cudaFree(b.p);
+        }
+    }
+    g_parked[dev].clear();
+}
+void unpark_all(int dev) {
+    if (dev < 0 || dev >= 64) return;
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    unpark_all_locked(dev);
+}
+
+// Pinned staging buffers are parked the same way (by exact size): cudaMallocHost / cudaFreeHost map and unmap
+// the buffer on the device and synchronise it, which a create / map / destroy loop should not pay every cycle.
+// A buffer is parked only when no copy from it is in flight (mi_destroy synchronises the stream first).
+struct ParkedHost { void* p; size_t bytes; };
+std::vector<ParkedHost> g_parked_host;
+cudaError_t pinned_alloc(void** p, size_t bytes) {
+    {
+        std::lock_guard<std::mutex> lock(g_cache_mutex);
+        for (size_t i = g_parked_host.size(); i-- > 0;) {
+            if (g_parked_host[i].bytes == bytes) {
+                *p = g_parked_host[i].p;
+                g_parked_host.erase(g_parked_host.begin() + (long)i);
+                return cudaSuccess;
+            }
+        }
+    }
+    return cudaMallocHost(p, bytes);
+}
+void pinned_free(void* p, size_t bytes) {
+    if (!p) return;
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    g_parked_host.push_back(ParkedHost{p, bytes});
+}
+void unpark_pinned() {
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    for (const ParkedHost& b : g_parked_host) cudaFreeHost(b.p);
+    g_parked_host.clear();
+}
+
 cudaError_t dev_alloc(void** p, size_t bytes, int dev, cudaStream_t s) {
     cudaMemPool_t pool = nullptr;
     cudaError_t e = device_pool(dev, &pool);
     if (e != cudaSuccess) return e;
     constexpr size_t kGranule = (size_t)2 << 20;
     bytes = ((bytes ? bytes : 1) + kGranule - 1) / kGranule * kGranule;
-    return cudaMallocFromPoolAsync(p, bytes, pool, s);
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    std::vector<ParkedBlock>& parked = g_parked[dev];
+    for (size_t i = parked.size(); i-- > 0;) {
+        if (parked[i].bytes == bytes && parked[i].s == s) {
+            *p = parked[i].p;
+            parked.erase(parked.begin() + (long)i);
+            g_live[*p] = LiveBlock{bytes, dev};
+            return cudaSuccess;
+        }
+    }
+    e = cudaMallocFromPoolAsync(p, bytes, pool, s);
+    if (e == cudaErrorMemoryAllocation && !parked.empty()) {
+        cudaGetLastError();
+        unpark_all_locked(dev);
+        cudaDeviceSynchronize();   // the frees were queued on their own streams
+        e = cudaMallocFromPoolAsync(p, bytes, pool, s);
+    }
+    if (e == cudaSuccess) g_live[*p] = LiveBlock{bytes, dev};
+    return e;
 }
 void dev_free(void* p, cudaStream_t s) {
-    if (p) cudaFreeAsync(p, s);
+    if (!p) return;
+    std::lock_guard<std::mutex> lock(g_cache_mutex);
+    const auto it = g_live.find(p);
+    if (it == g_live.end()) {   // not from dev_alloc: cannot happen inside the library
+        cudaFreeAsync(p, s);
+        return;
+    }
+    g_parked[it->second.dev].push_back(ParkedBlock{p, it->second.bytes, s});
+    g_live.erase(it);
 }
 
 int sm_count() {
@@ -271,6 +358,27 @@ mi_status validate_q(mi_ctx* c, const double* q, int32_t nq) {
 // pitches of both histogram kernels, the z kernel's binning variant and -- for the separable path --
 // the pitched fixed bins with the rare-voxel list, which depend on the row count and on the
 // fixed-voxel mask.  Called by mi_create, mi_set_option and mi_set_fixed_mask; the device is current.
+// The quad copies of the moving side are big -- 16 B per padded voxel for the float yz-quads the generic trilinear
+// kernels gather from, 4 B for the bin quads of partial volume -- and a context that only ever runs separable
+// (translation / scale) maps or nearest-neighbour needs neither.  They are built on the first call that does.
+mi_status ensure_moving_quads(mi_ctx* c, bool float_quads, bool bin_quads) {
+    cudaStream_t s = c->stream;
+    const size_t npad = ((size_t)c->md[0] + 2) * ((size_t)c->md[1] + 2) * ((size_t)c->md[2] + 2);
+    if (float_quads && c->d_moving_quad == nullptr) {
+        cudaError_t e = dev_alloc((void**)&c->d_moving_quad, npad * sizeof(float4), c->device, s);
+        if (e != cudaSuccess) { c->d_moving_quad = nullptr; return cuda_fail(c, e, "cudaMalloc moving quads"); }
+        e = mi::launch_quad_build(c->d_moving_pad, c->d_moving_quad, c->md[0], c->md[1], c->md[2], s);
+        if (e != cudaSuccess) { dev_free(c->d_moving_quad, s); c->d_moving_quad = nullptr; return cuda_fail(c, e, "build moving quads"); }
+    }
+    if (bin_quads && c->d_mbins_quad == nullptr) {
+        cudaError_t e = dev_alloc((void**)&c->d_mbins_quad, npad * sizeof(uint32_t), c->device, s);
+        if (e != cudaSuccess) { c->d_mbins_quad = nullptr; return cuda_fail(c, e, "cudaMalloc moving bin quads"); }
+        e = mi::launch_bins_quad_build(c->d_mbins, c->d_mbins_quad, c->md[0], c->md[1], c->md[2], s);
+        if (e != cudaSuccess) { dev_free(c->d_mbins_quad, s); c->d_mbins_quad = nullptr; return cuda_fail(c, e, "build moving bin quads"); }
+    }
+    return MI_OK;
+}
+
 mi_status plan_layout(mi_ctx* c) {
     cudaStream_t s = c->stream;
     // generic kernel: the gathers live in L1, which is what the shared histogram leaves of the SM's
@@ -537,8 +645,11 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
     if ((st = grow(c, &c->d_q, &c->cap_q, (size_t)(nq > 0 ? nq : 1))) != MI_OK) return st;
     if (c->staging_busy) { MI_CUDA(c, cudaEventSynchronize(c->ev_staging)); c->staging_busy = false; }
     if ((size_t)N * 12 > c->cap_hM) {
-        if (c->h_M) { cudaFreeHost(c->h_M); c->h_M = nullptr; c->cap_hM = 0; }
-        MI_CUDA(c, cudaMallocHost(reinterpret_cast<void**>(&c->h_M), (size_t)N * 12 * sizeof(float)));
+        if (c->h_M) {
+            mi::pinned_free(c->h_M, c->cap_hM * sizeof(float));
+            c->h_M = nullptr; c->cap_hM = 0;
+        }
+        MI_CUDA(c, mi::pinned_alloc(reinterpret_cast<void**>(&c->h_M), (size_t)N * 12 * sizeof(float)));
         c->cap_hM = (size_t)N * 12;
     }
     std::memcpy(c->h_M, hM.data(), (size_t)N * 12 * sizeof(float));
@@ -567,6 +678,9 @@ mi_status eval_core(mi_ctx* c, const std::vector<float>& hM, int64_t N, const do
                        (size_t)chunk * nbins2 * helem)) != MI_OK)
             return st;
     }
+    if (sep == nullptr &&
+        (st = ensure_moving_quads(c, interp == MI_INTERP_TRILINEAR && c->opt_gather == 1, pv)) != MI_OK)
+        return st;
     for (int64_t off = 0; sep == nullptr && off < N; off += chunk) {
         const int64_t cnt = (N - off < chunk) ? (N - off) : chunk;
         uint32_t* hist = hist_to_user_dev
@@ -874,8 +988,6 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
         }
         if ((st = plan_layout(c)) != MI_OK) { mi::set_thread_error(c->err); break; }
         if (!c->wide) {
-            if ((e = dev_alloc((void**)&c->d_mbins_quad, (size_t)npad * sizeof(uint32_t), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving bin quads"); break; }
-            if ((e = mi::launch_bins_quad_build(c->d_mbins, c->d_mbins_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving bin quads"); break; }
             {   // the most populated moving bin (d_counts is free again: the fixed counts are on the host)
                 unsigned long long h_mcounts[256];
                 if ((e = mi::launch_bin_count(c->d_mbins, nm, d_counts, s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "count moving bins"); break; }
@@ -887,8 +999,7 @@ mi_status mi_create(mi_ctx** out, const float* fixed, const int32_t fixed_dims[3
             }
         }
         if ((e = mi::launch_pad_replicate(d_mov, c->d_moving_pad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "pad moving"); break; }
-        if ((e = dev_alloc((void**)&c->d_moving_quad, (size_t)npad * sizeof(float4), device, c->stream)) != cudaSuccess) { st = cuda_fail(nullptr, e, "cudaMalloc moving quads"); break; }
-        if ((e = mi::launch_quad_build(c->d_moving_pad, c->d_moving_quad, moving_dims[0], moving_dims[1], moving_dims[2], s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "build moving quads"); break; }
+        // the yz-quad copies (float4 / u32 per padded voxel) are built by the first call that gathers from them
         if ((e = cudaStreamSynchronize(s)) != cudaSuccess) { st = cuda_fail(nullptr, e, "mi_create sync"); break; }
     } while (false);
     dev_free(d_tmp, c->stream);
@@ -911,7 +1022,7 @@ void mi_destroy(mi_ctx* c) {
                         c->d_mi, c->d_nvalid, c->d_q, c->d_map, c->d_argmax};
         for (void* b : bufs) dev_free(b, c->stream);
         cudaStreamSynchronize(c->stream);
-        if (c->h_M) cudaFreeHost(c->h_M);
+        mi::pinned_free(c->h_M, c->cap_hM * sizeof(float));
         if (c->ev_staging) cudaEventDestroy(c->ev_staging);
         cudaGetLastError();
     }
@@ -922,6 +1033,13 @@ mi_status mi_release_cached_memory(int32_t device) {
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
     if (device < 0 || device >= ndev || device >= 64) return MI_ERR_INVALID_ARG;
+    {
+        DeviceGuard guard(device);
+        if (!guard.ok) return MI_ERR_CUDA;
+        mi::unpark_all(device);
+        mi::unpark_pinned();
+        if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
+    }
     std::lock_guard<std::mutex> lock(mi::g_pool_mutex);
     if (mi::g_pools[device] == nullptr) return MI_OK;
     if (cudaMemPoolTrimTo(mi::g_pools[device], 0) != cudaSuccess) { cudaGetLastError(); return MI_ERR_CUDA; }
@@ -1006,7 +1124,12 @@ mi_status mi_set_option(mi_ctx* c, mi_option key, int64_t v) {
     case MI_OPT_ZHIST_MATCH_ANY: c->opt_match_any = v != 0; break;
     case MI_OPT_GENERIC_GATHER:
         if (v < 0 || v > 1) return bad();
-        c->opt_gather = (int)v; break;
+        c->opt_gather = (int)v;
+        if (v == 0 && c->d_moving_quad != nullptr) {   // 16 B per padded voxel nobody reads any more
+            dev_free(c->d_moving_quad, c->stream);
+            c->d_moving_quad = nullptr;
+        }
+        break;
     case MI_OPT_GENERIC_THREADS:
         if (v != 512 && v != 768 && v != 1024) return bad();
         c->opt_gthreads = (int)v; break;
@@ -1051,6 +1174,7 @@ mi_status mi_get_option(const mi_ctx* c, mi_option key, int64_t* out) {
     case MI_OPT_GENERIC_THREADS: *out = c->opt_gthreads; break;
     case MI_OPT_GENERIC_SLAB_MB: *out = c->opt_slab_mb; break;
     case MI_INFO_LAST_UPDATES_ISSUED: *out = c->last_reds; break;
+    case MI_INFO_QUADS_BUILT: *out = (c->d_moving_quad ? 1 : 0) | (c->d_mbins_quad ? 2 : 0); break;
     case MI_INFO_NUM_SMS: *out = c->num_sms; break;
     case MI_INFO_BIN_MODE: *out = c->bin_mode; break;
     case MI_INFO_ZHIST_ROWS: *out = c->wide ? 0 : c->zrows_real; break;
@@ -1390,6 +1514,7 @@ mi_status mi_probe_gather_rate(mi_ctx* c, const double* T, int32_t n_transforms,
     if ((st = grow(c, &c->d_M, &c->cap_M, (size_t)n_transforms * 12)) != MI_OK) return st;
     MI_CUDA(c, cudaMemcpyAsync(c->d_M, hM.data(), hM.size() * sizeof(float), cudaMemcpyHostToDevice, s));
     MI_CUDA(c, cudaMemsetAsync(c->d_red_count, 0, sizeof(unsigned long long), s));
+    if ((st = ensure_moving_quads(c, c->opt_gather == 1, false)) != MI_OK) return st;
     mi::ResampleArgs a;
     a.fbins_ranked = c->d_fbins_ranked;
     a.rank_inv = c->d_rank_inv;

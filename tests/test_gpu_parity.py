@@ -430,6 +430,34 @@ def test_separable_scratch_smaller_than_one_slab(mi):
         assert np.max(np.abs(m - ref)) <= 1e-9 and np.array_equal(am, aref)
 
 
+def test_quad_copies_are_built_by_the_first_call_that_gathers_from_them(mi):
+    """a context that only runs separable maps or nearest-neighbour holds no yz-quad copy of the moving
+    side (16 + 4 B per padded voxel); the first generic trilinear call builds the float quads, the first
+    partial-volume call the bin quads, GENERIC_GATHER = 0 frees the float quads -- and results do not change."""
+    cfg = ph.get_config("C1")
+    T = rand_physical(np.random.default_rng(11), 4)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        built = lambda: mi.mi_get_option(ctx, mi.MI_INFO_QUADS_BUILT)
+        assert built() == 0
+        mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1 and built() == 0      # separable: no quads
+        mi.mi_eval_batch(ctx, T, (), 0)
+        assert built() == 0                                                            # nearest neighbour: none either
+        quad = mi.mi_eval_batch(ctx, T, (0.5,), 1, hist_out=True, nvalid_out=True)
+        assert built() == 1
+        mi.mi_eval_batch(ctx, T, (), mi.MI_INTERP_PARTIAL_VOLUME)
+        assert built() == 3
+        mi.mi_set_option(ctx, mi.MI_OPT_GENERIC_GATHER, 0)
+        assert built() == 2
+        scalar = mi.mi_eval_batch(ctx, T, (0.5,), 1, hist_out=True, nvalid_out=True)
+        assert built() == 2
+        mi.mi_set_option(ctx, mi.MI_OPT_GENERIC_GATHER, 1)
+        again = mi.mi_eval_batch(ctx, T, (0.5,), 1, hist_out=True, nvalid_out=True)
+        assert built() == 3
+        for a, b, c_ in zip(quad, scalar, again):
+            assert np.array_equal(a, b) and np.array_equal(a, c_)
+
+
 def test_rejected_option_leaves_the_context_as_it_was(mi):
     """an option value whose layout the device cannot hold (8 KB of shared memory for rows of 4096
     + 5 words) is refused AND not kept: the option reads back unchanged and the next call gives the same result."""
@@ -667,10 +695,17 @@ def test_context_cycles_reuse_the_pool_and_release(mi):
             m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
         first = m if first is None else first
         assert np.array_equal(m, first)
+    # round 3: freed blocks are parked by exact size and handed back to the next cycle -- a steady
+    # create / map / destroy loop takes nothing new from the device
     free0, _ = torch.cuda.mem_get_info()
+    for it in range(3):
+        with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+            m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert np.array_equal(m, first)
+        assert torch.cuda.mem_get_info()[0] == free0
     mi.mi_release_cached_memory(0)
     free1, _ = torch.cuda.mem_get_info()
-    assert free1 >= free0
+    assert free1 > free0, "the parked blocks and the pool were not given back"
     with pytest.raises(mi.MIError):
         mi.mi_release_cached_memory(9999)
     with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
