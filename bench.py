@@ -4,7 +4,7 @@
 grid over +-10 mm, trilinear) in voxel-transform evaluations per second.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--config C1..C5|C5ALL|PAPER51] [--all] [--shard] [--interp trilinear|nearest|pv]
+                    [--config C1..C5|C5ALL|PAPER51|PAPERROT|PAPERSCALE] [--all] [--shard] [--interp trilinear|nearest|pv]
 
 A "step" is one pass of the whole hot path (a2 transform generation, a3 resample, a4 joint
 histogram, a5 entropy reduction, a6 map assembly + arg max) over the full grid: one mi_map call.
@@ -55,7 +55,7 @@ NCU_DRAM = {
 
 METRIC = "voxel-transform evaluations per second (MI map, 260x311x260 fixed, 256 bins)"
 UNIT = "evals/s"
-PAPER_TABLE1 = {0: 116.21, 1: 86.30, 3: 99.46}   # MI evaluations/s, GTX 1060, PAPER.md:204-206 (context only)
+PAPER_TABLE1 = {0: 116.21, 1: 86.30, 2: 86.30, 3: 99.46, 4: 99.46}   # MI evaluations/s, GTX 1060, PAPER.md:204-206 (context only)
 
 
 def load_peaks():
@@ -177,7 +177,7 @@ def workload_config(cfg, interp, extra=None):
     c = {"workload": "%s: fixed %s @%.2f mm, moving %s @%.2f mm, %d bins, %s grid %s over [%g,%g], %s, q=%s"
          % (cfg.name, "x".join(str(d) for d in cfg.fixed.shape[::-1]), cfg.fixed_spacing[0],
             "x".join(str(d) for d in cfg.moving.shape[::-1]), cfg.moving_spacing[0], cfg.nbins,
-            {0: "translation", 1: "euler-rotation", 3: "scale"}.get(cfg.family, str(cfg.family)),
+            {0: "translation", 1: "euler-rotation", 2: "versor-rotation", 3: "scale", 4: "log-scale"}.get(cfg.family, str(cfg.family)),
             "x".join(str(d) for d in cfg.n), cfg.lo[0], cfg.hi[0], INTERP_NAMES[interp], list(cfg.q)),
          "fixed_voxels": int(cfg.fixed.size), "transforms": cfg.n_transforms,
          "evaluations_per_step": int(cfg.evaluations)}
@@ -558,7 +558,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "C5ALL", "PAPER51"])
+    ap.add_argument("--config", default="C5", choices=["C1", "C2", "C3", "C4", "C5", "C5ALL", "PAPER51", "PAPERROT", "PAPERSCALE"])
     ap.add_argument("--all", action="store_true", help="one line per BASELINE.json config, C5 (the headline) last")
     ap.add_argument("--shard", action="store_true", help="N > 1: map ONE grid across the ranks (strong scaling)")
     ap.add_argument("--res", type=float, default=1.0, help="development only: reduced-resolution phantom")

@@ -133,7 +133,7 @@ class Config:
     fixed_spacing: tuple
     moving_spacing: tuple
     nbins: int
-    family: int            # mi_family enum value (0 translation, 1 Euler deg, 3 scale)
+    family: int            # mi_family enum value (0 translation, 1 Euler deg, 2 versor, 3 scale, 4 log scale)
     lo: tuple
     hi: tuple
     n: tuple
@@ -283,11 +283,36 @@ def config_paper51(res=1.0, grid_n=51, seed=303) -> Config:
                   (0.0, 0.0, 0.0))
 
 
+def config_paperrot(res=1.0, grid_n=15, seed=303) -> Config:
+    """The paper's rotation parameter space (section 3.2): the versor ball -- p = axis * sin(theta/2),
+    "all points outside the sphere with radius = 1 are mapped to the sphere surface" -- so the map covers the
+    cube [-1, 1]^3 and every rotation up to 180 degrees.  Same image on both sides; an odd grid
+    puts the gold standard (0, 0, 0) on a node.  Shannon + Tsallis q = 0.5, 1.1 (Fig. 9's best order), 2.0."""
+    dims = _head_dims(res)
+    sp = (0.7 / res,) * 3
+    fixed = render(head_phantom(seed), T1_TABLE, dims, sp, None, 0.02, seed, bias_amp=0.1)
+    return Config("PAPERROT", fixed, fixed, sp, sp, 256, 2, (-1.0,) * 3, (1.0,) * 3, (grid_n,) * 3, (0.5, 1.1, 2.0),
+                  (0.0, 0.0, 0.0))
+
+
+def config_paperscale(res=1.0, grid_n=15, seed=303, half_range=0.5) -> Config:
+    """The paper's scale parameter space (section 3.3): zero-centred parameters, "parameters
+    greater than zero" = a moving image scaled bigger -- family SCALE_LOG, factor = exp(p).  The paper prints no
+    range; +-0.5 (factors 0.61 .. 1.65) is this repository's choice.  Same image on both sides; Shannon +
+    Tsallis q = 0.5, 2.0 (one order on each side of 1, Fig. 14)."""
+    dims = _head_dims(res)
+    sp = (0.7 / res,) * 3
+    fixed = render(head_phantom(seed), T1_TABLE, dims, sp, None, 0.02, seed, bias_amp=0.1)
+    return Config("PAPERSCALE", fixed, fixed, sp, sp, 256, 4, (-half_range,) * 3, (half_range,) * 3, (grid_n,) * 3,
+                  (0.5, 2.0), (0.0, 0.0, 0.0))
+
+
 @lru_cache(maxsize=8)
 def get_config(name: str, **kw) -> Config:
     """Cached access: get_config('C5'), get_config('C3', res=0.25, grid_n=5) ..."""
     return {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4,
-            "C5": config_c5, "C5ALL": config_c5all, "PAPER51": config_paper51}[name](**kw)
+            "C5": config_c5, "C5ALL": config_c5all, "PAPER51": config_paper51, "PAPERROT": config_paperrot,
+            "PAPERSCALE": config_paperscale}[name](**kw)
 
 
 def ramp_volume(dims, coeffs) -> np.ndarray:

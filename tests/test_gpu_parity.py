@@ -340,6 +340,40 @@ def test_c3_c4_full_size_full_maps_against_oracle(mi, name):
     assert all(abs(p[d] - cfg.truth[d]) <= steps[d] * 1.0001 for d in range(3)), (p, cfg.truth)   # P11 (Shannon)
 
 
+@pytest.mark.parametrize("name", ["PAPERROT", "PAPERSCALE"])
+def test_paper_rotation_and_scale_spaces_at_full_size(mi, name):
+    """The paper's own parameter spaces at 260x311x260 (Table 1's other two rows): the versor
+    ball with the outside mapped to the surface -- rotations up to 180 degrees -- through the
+    generic kernel, and zero-centred scale parameters through the separable kernels.  The
+    whole 15^3 map is computed on the GPU (Shannon + Tsallis orders); the oracle checks the subset it can
+    afford: every 5th node per axis shifted to include the corners' neighbours, the centre and its 3^3
+    neighbourhood, the eight corners (|p| > 1 -> surface) and the GPU's arg max of every channel, value by
+    value at 1e-4 nats.  Same image on both sides, so the gold standard (0,0,0) -- the centre node -- must be
+    the Shannon arg max."""
+    cfg = ph.get_config(name)
+    assert cfg.fixed.shape == (260, 311, 260) and cfg.n == (15, 15, 15)
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, cfg.q, 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == (0 if name == "PAPERROT" else 1)
+    centre = (7, 7, 7)
+    nodes = {(a, b, c) for a in (1, 4, 10, 13) for b in (1, 4, 10, 13) for c in (1, 4, 10, 13)}
+    nodes |= {(7 + a, 7 + b, 7 + c) for a in (-1, 0, 1) for b in (-1, 0, 1) for c in (-1, 0, 1)}
+    nodes |= {(a, b, c) for a in (0, 14) for b in (0, 14) for c in (0, 14)}
+    for ch in range(m.shape[0]):
+        k2, k1, k0 = np.unravel_index(int(am[ch]), m.shape[1:])
+        nodes.add((int(k0), int(k1), int(k2)))
+    nodes = sorted(nodes)
+    ref = oracle_nodes(cfg, nodes, 1)
+    got = np.stack([m[:, k2, k1, k0] for (k0, k1, k2) in nodes])
+    assert np.max(np.abs(got - ref["mi"])) <= MI_TOL, np.max(np.abs(got - ref["mi"]))
+    assert int(am[0]) == (centre[2] * 15 + centre[1]) * 15 + centre[0], "Shannon arg max is not the gold standard"
+    assert int(np.argmax(ref["mi"][:, 0])) == nodes.index(centre)
+    if name == "PAPERROT":
+        # outside the unit ball the parameters are mapped to the surface: opposite corners are the same rotation
+        # axis with angle 180 degrees, i.e. the same matrix up to rounding
+        assert abs(m[0, 0, 0, 0] - m[0, 14, 14, 14]) <= 1e-3
+
+
 def test_c3_full_size_generic_kernel_histograms(mi):
     """The generic kernel's histograms at the full C3 size (rotations): three grid nodes, nearest neighbour
     bit-exact and trilinear within 1e-5 of the voxels."""
