@@ -340,6 +340,28 @@ def test_c3_c4_full_size_full_maps_against_oracle(mi, name):
     assert all(abs(p[d] - cfg.truth[d]) <= steps[d] * 1.0001 for d in range(3)), (p, cfg.truth)   # P11 (Shannon)
 
 
+def test_c5_full_map_against_the_stored_oracle_map(mi):
+    """BASELINE.json configs[4] IN FULL ("--full runs all 68 921 for the argmax check"; north_star:
+    "the map's argmax identical"; the map of PAPER.md:57, 71 and eq. 3): all 41^3 Shannon values of
+    one mi_map -- the launch configuration bench.py times -- against the oracle's map stored in
+    tests/golden/c5_map_oracle.npy (written by tests/golden/make_c5_map.py, which calls only oracle/; about
+    half an hour on 16 cores, hence stored), at 1e-4 nats, and the arg max identical.  Four stored nodes are
+    recomputed by the oracle here, bit for bit, so a stale file (changed phantom or oracle) cannot pass."""
+    import os
+    ref = np.load(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "c5_map_oracle.npy"))
+    cfg = ph.get_config("C5")
+    assert ref.shape == (41, 41, 41) and ref.dtype == np.float64 and np.isfinite(ref).all()
+    with make_ctx(mi, cfg.fixed, cfg.moving, cfg.fixed_spacing, cfg.moving_spacing, cfg.nbins) as ctx:
+        m, am = mi.mi_map(ctx, cfg.family, cfg.lo, cfg.hi, cfg.n, (), 1)
+        assert mi.mi_get_option(ctx, mi.MI_INFO_LAST_PATH) == 1
+    assert np.max(np.abs(m[0] - ref)) <= MI_TOL, np.max(np.abs(m[0] - ref))
+    assert int(am[0]) == int(np.argmax(ref))
+    k2, k1, k0 = (int(v) for v in np.unravel_index(int(np.argmax(ref)), ref.shape))
+    nodes = [(k0, k1, k2), (0, 0, 0), (40, 3, 17), (20, 20, 20)]
+    again = oracle_nodes(cfg, nodes, 1, q=())
+    assert np.array_equal(again["mi"][:, 0], np.array([ref[c, b, a] for (a, b, c) in nodes]))
+
+
 @pytest.mark.parametrize("name", ["PAPERROT", "PAPERSCALE"])
 def test_paper_rotation_and_scale_spaces_at_full_size(mi, name):
     """The paper's own parameter spaces at 260x311x260 (Table 1's other two rows): the versor
