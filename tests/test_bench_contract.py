@@ -71,7 +71,7 @@ def test_rotation_line_c3_is_measured_against_a_hardware_floor():
 
 
 def test_all_configs_from_one_invocation():
-    lines = load("r2c_bench_all.json.txt")
+    lines = load("r3_bench_all.json.txt")
     assert [l["config"]["workload"][:2] for l in lines] == ["C1", "C2", "C3", "C4", "C5"]   # the headline last
     for d in lines:
         d = dict(d, cpu_baseline=d.get("cpu_baseline"))
@@ -79,7 +79,7 @@ def test_all_configs_from_one_invocation():
 
 
 def test_reference_arm_line():
-    (d,) = load("r2c_bench_reference.json.txt")
+    (d,) = load("r3_bench_reference.json.txt")
     check_line(d, reference=True)
     (ours,) = load("r3_bench_c5.json.txt")
     assert d["config"]["workload"] == ours["config"]["workload"] and d["metric"] == ours["metric"]
